@@ -1,0 +1,124 @@
+"""Pins for the oracle's whole Cross-DEIM Poisson solve (O5-O12): closed form (C1), the dense
+eq. (4) solver on small grids, the paper's a-posteriori bound, the discrete residual, replay."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import lrp_oracle as O
+from paper_2607_06021_b200 import workloads as W
+
+
+def _closed_form_c1(w):
+    # sin(k pi x) sin(l pi y) are discrete eigenfunctions: W = sum a_m sin sin / (d_k + d_l)
+    x = W.grid(w.n)
+    i = np.arange(1, w.n + 1)
+    dk = lambda k: 4.0 * (w.n + 1) ** 2 * math.sin(math.pi * k / (2 * (w.n + 1))) ** 2
+    Wex = np.zeros((w.n, w.n))
+    for m in range(4):
+        k, l, a = int(w.meta["k"][m]), int(w.meta["l"][m]), float(w.meta["a"][m])
+        Wex += a * np.outer(np.sin(math.pi * k * x), np.sin(math.pi * l * x)) / (dk(k) + dk(l))
+    return Wex
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_c1_closed_form_exact_rank(seed):
+    w = W.config1(seed)
+    F = (w.UF * w.SF) @ w.VF.T
+    x = W.grid(w.n)
+    Fdef = sum(w.meta["a"][m] * np.outer(np.sin(math.pi * w.meta["k"][m] * x),
+                                         np.sin(math.pi * w.meta["l"][m] * x)) for m in range(4))
+    assert np.abs(F - Fdef).max() < 1e-12            # the generator realises the stated forcing
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    assert r.converged and r.rank == 4 and r.sweeps <= 8   # rho sits on the fp64 noise floor at tol 1e-12
+    Wex = _closed_form_c1(w)
+    Wlr = (r.UW * r.SW) @ r.VW.T
+    assert np.abs(Wlr - Wex).max() < 5e-12 * np.abs(Wex).max()
+    # leverage scores of the (unit-vector) spectral factors: the 4 true modes are selected first
+    assert sorted(r.trace[0].Istar[:4].tolist()) == sorted((w.meta["k"] - 1).tolist())
+    assert sorted(r.trace[0].Jstar[:4].tolist()) == sorted((w.meta["l"] - 1).tolist())
+    assert abs(r.trace[0].scoresU.sum() - 4) < 1e-12
+    # after pruning exactly the true indices survive
+    t = r.trace[-1]
+    assert sorted(t.I[t.keepI].tolist()) == sorted((w.meta["k"] - 1).tolist())
+    assert sorted(t.J[t.keepJ].tolist()) == sorted((w.meta["l"] - 1).tolist())
+
+
+@pytest.mark.parametrize("name,n,tol", [("C2", 511, 1e-10), ("C4", 255, 1e-10)])
+def test_against_dense_solver_and_bound(name, n, tol):
+    w = W.make(name, 0, n)
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    assert r.converged
+    F = (w.UF * w.SF) @ w.VF.T
+    Wd = O.dense_poisson(n, F)
+    Wlr = (r.UW * r.SW) @ r.VW.T
+    nrm = np.linalg.norm(Wd, "fro")
+    assert np.linalg.norm(Wlr - Wd, "fro") < 20 * tol * nrm
+    # rank vs the dense truth's rank at the same tolerance (Alg. 4 lines 30-31)
+    sv = np.linalg.svd(Wd, compute_uv=False)
+    rank_true = O.final_rank(sv, tol, w.max_rank)
+    assert abs(r.rank - rank_true) <= 2
+    assert np.abs(r.SW - sv[:r.rank]).max() < 100 * tol * sv[0]
+    # a-posteriori bound (Alg. 4 line 26): ||G - USV^T||_2 <~ ind-factor * sigma_{r+1}
+    t = r.trace[-1]
+    Z = O.dst1_matrix(n)
+    Gh = Z @ Wd @ Z
+    svG = np.linalg.svd(Gh, compute_uv=False)
+    full = (r.Uhat * r.Shat) @ r.Vhat.T
+    kk = min(len(t.I), len(t.J))
+    bound = min(t.eta1 * (1 + t.eta2), t.eta2 * (1 + t.eta1)) * svG[min(kk, n - 1)]
+    assert np.linalg.norm(Gh - full, 2) < 10 * bound + 1e-13 * svG[0]
+    # discrete residual -Delta_h u - f at random interior entries (SURVEY §8(c) pin (iv))
+    rng = np.random.default_rng(0)
+    ii = rng.integers(1, n - 1, 200)
+    jj = rng.integers(1, n - 1, 200)
+    h2 = 1.0 / (n + 1) ** 2
+    lap = (4 * Wlr[ii, jj] - Wlr[ii - 1, jj] - Wlr[ii + 1, jj] - Wlr[ii, jj - 1] - Wlr[ii, jj + 1]) / h2
+    assert np.abs(lap - F[ii, jj]).max() < 8 * tol / h2 * nrm      # 8/h^2 amplification of the entry error
+
+
+def test_sampled_spectral_entries_match_G_at_larger_n():
+    # pin (iii): exact spectral entries cost O(r_F) each at any n
+    w = W.make("C3", 1, 8191)
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    t = r.trace[-1]
+    act = 4 * int(max(t.I.max(), t.J.max()))
+    i, j = W.sample_pairs(w.n, 4096, 0, active=act)
+    ge = O.G_entries(r.UhF, w.SF, r.VhF, r.d, i, j)
+    gh = O.lowrank_entries(r.Uhat, r.Shat, r.Vhat, i, j)
+    assert np.abs(ge - gh).max() < 50 * w.tol * np.linalg.norm(r.Shat)
+
+
+def test_replay_reproduces_native_run_and_union_rules():
+    w = W.make("C2", 3, 1023)
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    rep = O.trace_to_replay(r.trace, r.rank)
+    r2 = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts(), replay=rep)
+    assert r2.sweeps == r.sweeps and r2.rank == r.rank
+    assert np.array_equal(r2.UW, r.UW) and np.array_equal(r2.SW, r.SW) and np.array_equal(r2.VW, r.VW)
+    # union rules (O7): survivors first in stored order, then new members in I*'s order; k = 0 appends
+    # the first safeguard entry not in the set
+    t0, t1 = r.trace[0], r.trace[1]
+    assert t0.I[:-1].tolist() == t0.Istar.tolist()
+    first_sg = next(int(s) for s in w.safeguard if int(s) not in set(t0.Istar.tolist()))
+    assert int(t0.I[-1]) == first_sg
+    surv = t0.I[t0.keepI].tolist()
+    assert t1.I[:len(surv)].tolist() == surv
+    new = [int(v) for v in t1.Istar if int(v) not in set(surv)]
+    assert t1.I[len(surv):len(surv) + len(new)].tolist() == new
+    assert len(set(t1.I.tolist())) == len(t1.I)
+    # selection size: cols(A) + oversample
+    assert len(t0.Istar) == w.rF + w.oversample
+    assert len(t1.Istar) == t0.rank + w.oversample
+
+
+def test_max_sweeps_and_rank_cap():
+    w = W.make("C2", 0, 511)
+    o = w.opts()
+    o["max_sweeps"] = 1
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **o)
+    assert r.sweeps == 1 and not r.converged
+    o = w.opts()
+    o["max_rank"] = 5
+    r = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **o)
+    assert r.rank == 5 and r.UW.shape == (511, 5)
