@@ -1,0 +1,177 @@
+/* lrp.h -- C ABI of liblrp: the B200 (sm_100a) hot path of the Cross-DEIM low-rank Poisson solver
+ * of arxiv/paper_2607_06021 (citations: `PAPER.md:<line>` + section / equation / algorithm).
+ *
+ * Problem (eq. (2), 194-196 eq. (3)): 5-point Dirichlet Poisson on an n x n interior grid,
+ *     T W + W T^T = h^2 F,   T = tridiag(-1, 2, -1),   h = 1/(n+1),
+ * with the right-hand side held as low-rank factors F = UF diag(SF) VF^T.  The factors are
+ * taken to sine space by batched DST-I along each dimension, the spectral solution
+ *     G(i,j) = (Uh diag(S) Vh^T)(i,j) / (d_i + d_j),  d_k = lambda_k / h^2 = 4 (n+1)^2 sin^2(pi k / (2(n+1)))
+ * (eq. (4); lambda_k of PAPER.md:200 evaluated as 4 sin^2(theta/2), reading Q1) is
+ * sampled only on index sets I, J chosen by leverage scores (Alg. 3), rebuilt into
+ * factors by the stabilised cross approximation scross (Alg. 1), iterated by Cross-DEIM
+ * (Alg. 4) and brought back by a final batched DST-I.
+ *
+ * Conventions
+ *   - every `d_*` pointer is a DEVICE pointer to memory the CALLER owns; `h_*` pointers are HOST pointers.
+ *   - fp64 throughout.  "tall" matrices are column-major with an explicit leading dimension ld >= n
+ *     (each factor column contiguous).  Diagonal factors S are stored as vectors.
+ *   - indices are 0-based int32_t (grid point i <-> 1-based frequency k = i + 1); sizes are int64_t/int32_t.
+ *   - the library never allocates device memory for data: scratch comes from the workspace the caller
+ *     hands to lrp_set_workspace (sized by the lrp_*_workspace_bytes functions).  Pointers must be
+ *     8-byte aligned; the workspace must be 256-byte aligned.
+ *   - every call enqueues on the ctx's stream.  lrp_dst1_batched, lrp_sample_fibers are asynchronous;
+ *     lrp_leverage_select, lrp_scross and lrp_cross_deim_solve synchronise the stream internally where
+ *     their control flow needs device results (documented per function) and are complete on return
+ *     only where stated.
+ *   - return value: 0 = LRP_OK, negative = error, positive = warning (outputs valid).
+ *     No exceptions, no globals, no CPU fallback: without a CUDA device every compute call fails.
+ *   - n + 1 must be a power of two, 2 <= n + 1 <= 2^27 (general n: DESIGN.md "next").
+ */
+#ifndef LRP_H_
+#define LRP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LRP_OK                  0
+#define LRP_ERR_BADARG         -1   /* null / misaligned pointer, ld < n, set larger than the cap, duplicate or out-of-range index */
+#define LRP_ERR_UNSUPPORTED_N  -2   /* n + 1 not a power of two, or out of range */
+#define LRP_ERR_WORKSPACE      -3   /* workspace missing or too small */
+#define LRP_ERR_CUDA           -4   /* a CUDA call failed; see lrp_last_cuda_error */
+#define LRP_WARN_NOCONV         1   /* Cross-DEIM reached max_sweeps (or r* > max_rank): outputs valid, tolerance not certified */
+
+#define LRP_MAX_SWEEPS_INFO    32   /* per-sweep arrays in lrp_solve_info hold this many sweeps */
+
+typedef struct lrp_ctx lrp_ctx;
+
+/* Create a context bound to CUDA device `device` and to `cuda_stream` (a cudaStream_t; NULL = the
+ * legacy default stream).  The stream is borrowed, not owned.  Fails with LRP_ERR_CUDA if there is no device. */
+int lrp_create(lrp_ctx** out, int device, void* cuda_stream);
+int lrp_destroy(lrp_ctx* ctx);
+const char* lrp_strerror(int code);
+/* cudaError_t (as int) of the last failing CUDA call seen by this ctx, 0 if none. */
+int lrp_last_cuda_error(const lrp_ctx* ctx);
+/* Number of kernel launches this ctx has enqueued since creation (bench.py's `gpu_launches`). */
+int64_t lrp_launch_count(const lrp_ctx* ctx);
+
+/* Workspace sizes in bytes (host-side arithmetic only; safe to call without a GPU).
+ *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample).
+ *   lrp_dst1_workspace_bytes   : lrp_dst1_batched (0 for n <= 16383, the single-pass shared-memory regime).
+ *   lrp_leverage_workspace_bytes, lrp_scross_workspace_bytes : the standalone calls. */
+size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample);
+size_t lrp_dst1_workspace_bytes(int64_t n, int32_t batch);
+size_t lrp_leverage_workspace_bytes(int64_t n, int32_t k);
+size_t lrp_scross_workspace_bytes(int64_t n, int32_t k, int32_t l);
+/* Hand the ctx a device scratch buffer (caller-owned, must outlive the calls that use it). */
+int lrp_set_workspace(lrp_ctx* ctx, void* d_ws, size_t bytes);
+
+/* Batched DST-I:
+ *     out(k, b) = scale * sum_{j=1..n} in(j, b) sin(j k pi / (n+1)),   k = 1..n,  b = 0..batch-1,
+ * 1-based j,k stored 0-based.  scale = 1: unnormalised (applied twice = (n+1)/2 * identity);
+ * scale = sqrt(2/(n+1)): the symmetric orthogonal Z of PAPER.md:198-200 (twice = identity).
+ * in/out: tall n x batch, column b at d_in + b*ld_in.  d_in == d_out (same ld) is allowed; partial overlap is not.
+ * Each column is transformed independently along its own (contiguous) dimension: no transpose.
+ * Asynchronous.  Errors: BADARG, UNSUPPORTED_N, WORKSPACE (n > 16383 needs lrp_dst1_workspace_bytes), CUDA. */
+int lrp_dst1_batched(lrp_ctx* ctx, int64_t n, int32_t batch,
+                     const double* d_in, int64_t ld_in, double* d_out, int64_t ld_out, double scale);
+
+/* Spectral fibers of G(i,j) = (Uh diag(S) Vh^T)(i,j) / (d_i + d_j)  (eq. (4); Alg. 1
+ * line 3), O(r) per entry, never forming the n^2 matrix:
+ *     d_C  (n x nJ, ld ldc): column c = G(:, J[c]);      d_Rt (n x nI, ld ldr): column c = G(I[c], :)^T.
+ * Uh, Vh: tall n x r spectral factors; d_S: r values.  d_I / d_J: device index lists (0-based, in [0,n)).
+ * Either output (with its index list) may be NULL.  Asynchronous.  Errors: BADARG, CUDA. */
+int lrp_sample_fibers(lrp_ctx* ctx, int64_t n, int32_t r,
+                      const double* d_Uh, int64_t ldu, const double* d_S, const double* d_Vh, int64_t ldv,
+                      const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,
+                      double* d_C, int64_t ldc, double* d_Rt, int64_t ldr);
+
+/* Leverage-score selection (Alg. 3, deterministic top-k form, reading Q5):
+ * thin QR A = Q R of the tall n x k block, scores[i] = ||Q(i,:)||^2 over the columns with
+ * |R_cc| >= 1e-13 max|R_cc|, and d_idx_out = the num_select (<= n, <= 4096) largest, ordered by
+ * (score descending, index ascending).  d_scores (n) may be NULL.  assume_orthonormal = 1 skips the QR
+ * (A is used as Q).  A is not modified.  Complete on return (synchronises).  Errors: BADARG, WORKSPACE, CUDA. */
+int lrp_leverage_select(lrp_ctx* ctx, int64_t n, int32_t k, const double* d_A, int64_t lda,
+                        int32_t num_select, int assume_orthonormal,
+                        int32_t* d_idx_out, double* d_scores);
+
+/* Stabilised cross approximation, Algorithm 1 on already sampled fibers, square-grid case:
+ * C = G(:,J) is n x k (k = #J), Rt = G(I,:)^T is n x l (l = #I).  Thin QR C = Q R_C, Rt = Z R_R; the tall
+ * least-squares systems of lines 5-14 are solved by the SVD pseudo-inverse (relative cut 1e-13) folded to
+ * the k x l core M (k <= l: M = Q(I,:)^+ R_R^T;  k > l: M = (Z(J,:)^+ R_C^T)^T); M = Uc diag(S) Vc^T;
+ * numerical rank = #{S_c > 1e-14 S_1} (>= 1);  U = Q Uc, V = Z Vc.
+ * Outputs: d_U (n x rank), d_S (min(k,l) values, the first *rank_out are the kept ones), d_V (n x rank),
+ * d_rC (k) = |diag R_C|, d_rR (l) = |diag R_R| (Alg. 1 line 16), *h_rank_out, *h_smin_full_out (HOST
+ * scalars; smin_full = smallest singular value of the untruncated core, reading Q11).
+ * d_U / d_V must have room for min(k,l) columns.  C and Rt are read-only.  Complete on return.
+ * Errors: BADARG (k or l < 1 or > 1024, ld < n), WORKSPACE, CUDA. */
+int lrp_scross(lrp_ctx* ctx, int64_t n, const double* d_C, int64_t ldc, int32_t k,
+               const double* d_Rt, int64_t ldr, int32_t l,
+               const int32_t* d_I, const int32_t* d_J,
+               double* d_U, int64_t ldu, double* d_S, double* d_V, int64_t ldv,
+               double* d_rC, double* d_rR, int32_t* h_rank_out, double* h_smin_full_out);
+
+typedef struct lrp_solve_opts {
+    double  tol;               /* epsilon of Alg. 4 */
+    int32_t max_rank;          /* r_max */
+    int32_t oversample;        /* extra leverage indices per sweep (config 1: 8) */
+    int32_t max_sweeps;        /* at most this many sweeps (reading Q16) */
+    int32_t tol_mode;          /* 0: relative to ||S_k||_2 (default, reading Q15); 1: absolute, as printed in the paper */
+    const int32_t* h_safeguard;/* HOST list of pre-drawn random indices (Alg. 4 lines 7-12): randomness is input data */
+    int32_t n_safeguard;
+    const double* d_U0;        /* optional warm start / initial guess for the selection (n x r0), may be NULL -> spectral RHS factors */
+    const double* d_V0;
+    int64_t ld0;
+    int32_t r0;
+    /* replay (test hook): take the index sets and prune masks of every sweep from these HOST arrays instead of
+     * deciding them; replay_sweeps > 0 enables it.  Sets are concatenated sweep after sweep. */
+    int32_t replay_sweeps;
+    const int32_t* h_replay_nI;     /* [replay_sweeps] */
+    const int32_t* h_replay_nJ;     /* [replay_sweeps] */
+    const int32_t* h_replay_I;      /* concatenated I_k */
+    const int32_t* h_replay_J;      /* concatenated J_k */
+    const uint8_t* h_replay_keepI;  /* concatenated prune masks (1 = survives), may be NULL -> decide */
+    const uint8_t* h_replay_keepJ;
+    int32_t replay_final_rank;      /* > 0: use this final rank */
+} lrp_solve_opts;
+
+typedef struct lrp_solve_info {
+    int32_t rank, sweeps, converged;
+    double  rho, indicator, eta1, eta2, snorm, smin_full;
+    int32_t nI[LRP_MAX_SWEEPS_INFO], nJ[LRP_MAX_SWEEPS_INFO], rank_per_sweep[LRP_MAX_SWEEPS_INFO];
+    double  rho_per_sweep[LRP_MAX_SWEEPS_INFO], ind_per_sweep[LRP_MAX_SWEEPS_INFO];
+    float   ms_dst_fwd, ms_select, ms_sample, ms_qr, ms_core, ms_rebuild, ms_stop, ms_dst_inv, ms_total;
+    int64_t launches;
+} lrp_solve_info;
+
+/* Low-rank Poisson solve by Cross-DEIM (Alg. 4):
+ * solves T W + W T^T = h^2 F with F = UF diag(SF) VF^T given in PHYSICAL space (columns need not be
+ * orthonormal) and writes W ~= UW diag(SW) VW^T with rank info->rank <= max_rank.
+ * d_UW, d_VW: tall with ld >= n and room for max_rank columns; d_SW: max_rank values.
+ * Optional trace outputs (HOST, may be NULL): h_trace_I / h_trace_J receive the concatenated I_k / J_k (before
+ * pruning) of every sweep (capacity LRP_MAX_SWEEPS_INFO * K_cap each), h_trace_keepI / h_trace_keepJ the
+ * prune masks; the per-sweep counts are info->nI / nJ.
+ * Optional spectral outputs (DEVICE, may be NULL): d_Uhat / d_Vhat (n x K_cap, ld = ld_hat) and d_Shat
+ * (K_cap) receive the last spectral iterate before the final truncation (info->rank_per_sweep[sweeps-1] columns).
+ * Synchronous: complete on return.  Returns LRP_WARN_NOCONV when the stop test never passed. */
+int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
+                         const double* d_UF, int64_t ldu, const double* d_SF, const double* d_VF, int64_t ldv,
+                         const lrp_solve_opts* opts,
+                         double* d_UW, int64_t lduw, double* d_SW, double* d_VW, int64_t ldvw,
+                         lrp_solve_info* info,
+                         int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                         double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat);
+
+/* Entries (U diag(S) V^T)(rows[t], cols[t]), t < count (X(i,j) = sum_k sigma_k u_k(i) v_k(j)):
+ * the O(r) element access used to read a low-rank result without forming it.  All pointers device.  Asynchronous. */
+int lrp_lowrank_entries(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_U, int64_t ldu, const double* d_S,
+                        const double* d_V, int64_t ldv, const int64_t* d_rows, const int64_t* d_cols,
+                        int64_t count, double* d_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LRP_H_ */

@@ -1,0 +1,554 @@
+// api.cu -- the C ABI of include/lrp.h and the Cross-DEIM sweep driver (Alg. 4).
+// Host control flow only decides sets of a few hundred integers and a handful of scalars per sweep
+// (union / safeguard / prune / stop test); every step that touches an n-long axis is a kernel.
+#include "common.cuh"
+#include "tall.cuh"
+#include "qr.cuh"
+#include "core.cuh"
+#include <math.h>
+#include <string.h>
+#include <stdlib.h>
+#include <vector>
+#include <algorithm>
+#include <new>
+
+namespace {
+
+// constants the paper is silent on (readings Q4, Q6, Q12)
+constexpr double PINV_RCOND = 1e-13, RANK_RCOND = 1e-14, LEV_COL_RCOND = 1e-13, PRUNE_REL = 1e-12;
+
+bool aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
+
+int check_n(int64_t n) {
+    if (n < 1) return LRP_ERR_UNSUPPORTED_N;
+    int64_t N = n + 1;
+    if (!lrp_is_pow2(N) || N > ((int64_t)1 << 27)) return LRP_ERR_UNSUPPORTED_N;
+    return LRP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ scross on owned buffers
+struct ScrossWs {
+    double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws;
+    int32_t *scal_i, *iwork;
+    bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int kmax, int lmax) {
+        int K = kmax > lmax ? kmax : lmax;
+        RC = ar.take<double>((size_t)kmax * kmax); RR = ar.take<double>((size_t)lmax * lmax);
+        Uc = ar.take<double>((size_t)K * K); S = ar.take<double>(K); Vc = ar.take<double>((size_t)K * K);
+        rC = ar.take<double>(kmax); rR = ar.take<double>(lmax);
+        scal_d = ar.take<double>(8); scal_i = ar.take<int32_t>(8); iwork = ar.take<int32_t>(K);
+        core_work = ar.take<double>(core_work_doubles(K, K));
+        qr_ws = ar.take<double>(tall_qr_ws_doubles(ctx, n, K));
+        return ar.ok();
+    }
+};
+
+// QR of both fiber blocks (in place), the small core, and the host copies the driver needs.
+// On return (stream synchronised): Qb = Q, Zb = Z, ws.Uc/S/Vc hold the core SVD, h_S (p), h_rC (k), h_rR (l) filled.
+int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, double* Zb, int64_t ldz, int l,
+                  const int32_t* dI, const int32_t* dJ, ScrossWs& w,
+                  double* h_S, double* h_rC, double* h_rR, int* h_rank, double* h_smin,
+                  cudaEvent_t ev_qr_done) {
+    LRP_TRY(tall_qr(ctx, n, k, Qb, ldq, w.RC, k, w.qr_ws));
+    LRP_TRY(tall_qr(ctx, n, l, Zb, ldz, w.RR, l, w.qr_ws));
+    if (ev_qr_done) LRP_CUDA(ctx, cudaEventRecord(ev_qr_done, ctx->stream));
+    CoreArgs a{};
+    a.k = k; a.l = l; a.Q = Qb; a.ldq = ldq; a.Z = Zb; a.ldz = ldz; a.RC = w.RC; a.ldrc = k; a.RR = w.RR; a.ldrr = l;
+    a.I = dI; a.J = dJ; a.pinv_rcond = PINV_RCOND; a.rank_rcond = RANK_RCOND;
+    a.Uc = w.Uc; a.S = w.S; a.Vc = w.Vc; a.rC = w.rC; a.rR = w.rR; a.scal_i = w.scal_i; a.scal_d = w.scal_d;
+    a.work = w.core_work; a.iwork = w.iwork;
+    LRP_TRY(scross_core(ctx, a));
+    const int p = k < l ? k : l;
+    int32_t hi[1]; double hd[1];
+    LRP_CUDA(ctx, cudaMemcpyAsync(h_S, w.S, sizeof(double) * p, cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, cudaMemcpyAsync(h_rC, w.rC, sizeof(double) * k, cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, cudaMemcpyAsync(h_rR, w.rR, sizeof(double) * l, cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, cudaMemcpyAsync(hi, w.scal_i, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, cudaMemcpyAsync(hd, w.scal_d, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *h_rank = hi[0]; *h_smin = hd[0];
+    return LRP_OK;
+}
+
+// U = Q Uc(:, 0:rank) (n x rank) with optional squared row norms (the next sweep's leverage scores)
+int rebuild(lrp_ctx* ctx, int64_t n, const double* Qf, int64_t ldq, int kk, const double* Uc, int ldc, int rank,
+            double* U, int64_t ldu, double* rownorm2) {
+    TallGemmArgs g{};
+    g.n = n; g.k = kk; g.m = rank; g.mode = TG_PLAIN; g.A = Qf; g.lda = ldq; g.B = Uc; g.ldb = ldc;
+    g.Out = U; g.ldo = ldu; g.rownorm2 = rownorm2;
+    return tall_gemm(ctx, g);
+}
+
+int sample_side(lrp_ctx* ctx, int64_t n, int r, const double* A, int64_t lda, const double* S, const double* Bt, int64_t ldb,
+                const int32_t* idx, int nidx, double* Out, int64_t ldo) {
+    TallGemmArgs g{};
+    g.n = n; g.k = r; g.m = nidx; g.mode = TG_SAMPLE; g.A = A; g.lda = lda; g.B = Bt; g.ldb = ldb; g.idx = idx; g.scale_t = S;
+    g.Out = Out; g.ldo = ldo;
+    return tall_gemm(ctx, g);
+}
+
+// leverage scores of a tall block through a scratch copy (QR in place on the copy)
+int leverage_scores_qr(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* scratch, int64_t lds,
+                       double* R, unsigned char* mask, double* qr_ws, double* scores) {
+    LRP_TRY(tall_copy(ctx, n, k, A, lda, scratch, lds));
+    LRP_TRY(tall_qr(ctx, n, k, scratch, lds, R, k, qr_ws));
+    LRP_TRY(leverage_colmask(ctx, k, R, k, LEV_COL_RCOND, mask));
+    return tall_rownorm2(ctx, n, k, scratch, lds, mask, scores);
+}
+
+int validate_indices(const int32_t* h, int cnt, int64_t n) {
+    std::vector<int32_t> v(h, h + cnt);
+    std::sort(v.begin(), v.end());
+    for (int i = 0; i < cnt; ++i) {
+        if (v[i] < 0 || v[i] >= n) return LRP_ERR_BADARG;
+        if (i > 0 && v[i] == v[i - 1]) return LRP_ERR_BADARG;
+    }
+    return LRP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ solve workspace
+struct SolveWs {
+    double *UhF, *VhF, *Cb, *Rb, *Ua, *Va, *Ub, *Vb, *scoresU, *scoresV;
+    double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *Rlev;
+    int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
+    unsigned char* mask;
+    void *sel_ws, *dst_ws;
+    size_t eta_stride, dst_ws_bytes;
+    ScrossWs sc;
+    bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank) {
+        const size_t ld = (size_t)n;
+        UhF = ar.take<double>(ld * rF); VhF = ar.take<double>(ld * rF);
+        Cb = ar.take<double>(ld * Kc); Rb = ar.take<double>(ld * Kc);
+        Ua = ar.take<double>(ld * Kc); Va = ar.take<double>(ld * Kc);
+        Ub = ar.take<double>(ld * Kc); Vb = ar.take<double>(ld * Kc);
+        scoresU = ar.take<double>(ld); scoresV = ar.take<double>(ld);
+        Sprev = ar.take<double>(Kc);
+        Amat = ar.take<double>((size_t)Kc * Kc); Bmat = ar.take<double>((size_t)Kc * Kc);
+        GU = ar.take<double>((size_t)Kc * Kc); GV = ar.take<double>((size_t)Kc * Kc);
+        Rlev = ar.take<double>((size_t)Kc * Kc);
+        rho_out = ar.take<double>(8); eta = ar.take<double>(8);
+        eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
+        eta_work = ar.take<double>(2 * eta_stride);
+        eta_iwork = ar.take<int32_t>(2 * (size_t)Kc);
+        gemmt_ws = ar.take<double>(tall_gemm_t_ws_doubles(ctx, n, Kc, Kc));
+        dI = ar.take<int32_t>(Kc); dJ = ar.take<int32_t>(Kc); dIpr = ar.take<int32_t>(Kc); dJpr = ar.take<int32_t>(Kc);
+        dIstar = ar.take<int32_t>(2 * (size_t)Kc + 8); dJstar = ar.take<int32_t>(2 * (size_t)Kc + 8);
+        mask = ar.take<unsigned char>(Kc);
+        sel_ws = ar.take<char>(select_ws_bytes(ctx, n, 2 * Kc + 1));
+        int dcols = rF > max_rank ? rF : max_rank;
+        dst_ws_bytes = lrp_dst1_ws_impl(n, dcols);
+        dst_ws = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
+        bool ok = sc.carve(ar, ctx, n, Kc, Kc);
+        return ok && ar.ok();
+    }
+};
+
+struct EventPool {
+    std::vector<cudaEvent_t> ev;
+    ~EventPool() { for (auto e : ev) cudaEventDestroy(e); }
+    cudaEvent_t rec(lrp_ctx* ctx) {
+        cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        ev.push_back(e); cudaEventRecord(e, ctx->stream); return e;
+    }
+    static float ms(cudaEvent_t a, cudaEvent_t b) { float t = 0.f; if (a && b) cudaEventElapsedTime(&t, a, b); return t; }
+};
+
+void host_union(std::vector<int32_t>& cur, const int32_t* star, int nstar, int* added) {
+    *added = 0;
+    for (int i = 0; i < nstar; ++i) {
+        int32_t v = star[i];
+        if (v < 0) continue;
+        if (std::find(cur.begin(), cur.end(), v) == cur.end()) { cur.push_back(v); ++*added; }
+    }
+}
+
+int final_rank_host(const double* S, int cnt, double tol, int max_rank, int tol_mode) {
+    double tot = 0.0;
+    for (int c = 0; c < cnt; ++c) tot += S[c] * S[c];
+    const double thresh = tol * tol * (tol_mode == 0 ? tot : 1.0);
+    int rstar = cnt; double tail = 0.0;
+    for (int c = cnt - 1; c >= 0; --c) { tail += S[c] * S[c]; if (tail < thresh) rstar = c; else break; }
+    int r = rstar < max_rank ? rstar : max_rank;
+    return r < 1 ? 1 : r;
+}
+
+}  // namespace
+
+// ================================================================================================ C ABI
+extern "C" {
+
+int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
+    if (!out) return LRP_ERR_BADARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || device < 0 || device >= count) return LRP_ERR_CUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return LRP_ERR_CUDA;
+    lrp_ctx* c = new (std::nothrow) lrp_ctx();
+    if (!c) return LRP_ERR_BADARG;
+    c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    *out = c;
+    return LRP_OK;
+}
+
+int lrp_destroy(lrp_ctx* ctx) { delete ctx; return LRP_OK; }
+
+const char* lrp_strerror(int code) {
+    switch (code) {
+        case LRP_OK: return "ok";
+        case LRP_ERR_BADARG: return "bad argument";
+        case LRP_ERR_UNSUPPORTED_N: return "n + 1 must be a power of two in [2, 2^27]";
+        case LRP_ERR_WORKSPACE: return "workspace missing or too small";
+        case LRP_ERR_CUDA: return "CUDA error (see lrp_last_cuda_error)";
+        case LRP_WARN_NOCONV: return "warning: stop test not passed within max_sweeps";
+        default: return "unknown code";
+    }
+}
+
+int lrp_last_cuda_error(const lrp_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+int64_t lrp_launch_count(const lrp_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int lrp_set_workspace(lrp_ctx* ctx, void* d_ws, size_t bytes) {
+    if (!ctx) return LRP_ERR_BADARG;
+    if (d_ws && ((uintptr_t)d_ws & 255u)) return LRP_ERR_BADARG;
+    ctx->ws = d_ws; ctx->ws_bytes = d_ws ? bytes : 0;
+    return LRP_OK;
+}
+
+size_t lrp_dst1_workspace_bytes(int64_t n, int32_t batch) {
+    if (check_n(n) != LRP_OK || batch < 0) return 0;
+    return lrp_dst1_ws_impl(n, batch);
+}
+
+size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample) {
+    if (check_n(n) != LRP_OK || rF < 1 || max_rank < 1 || oversample < 0) return 0;
+    int Kc = 2 * (max_rank + oversample);
+    if (Kc < rF + oversample + 1) Kc = rF + oversample + 1;
+    lrp_arena ar((void*)256, (size_t)-1 / 2);
+    SolveWs w;
+    w.carve(ar, nullptr, n, rF, Kc, max_rank);
+    return ar.off + 256;
+}
+
+size_t lrp_leverage_workspace_bytes(int64_t n, int32_t k) {
+    if (n < 1 || k < 1) return 0;
+    lrp_arena ar((void*)256, (size_t)-1 / 2);
+    ar.take<double>((size_t)n * k); ar.take<double>((size_t)k * k); ar.take<double>((size_t)n);
+    ar.take<unsigned char>(k); ar.take<double>(tall_qr_ws_doubles(nullptr, n, k));
+    ar.take<char>(select_ws_bytes(nullptr, n, 4096));
+    return ar.off + 256;
+}
+
+size_t lrp_scross_workspace_bytes(int64_t n, int32_t k, int32_t l) {
+    if (n < 1 || k < 1 || l < 1) return 0;
+    lrp_arena ar((void*)256, (size_t)-1 / 2);
+    ar.take<double>((size_t)n * k); ar.take<double>((size_t)n * l);
+    ScrossWs w; w.carve(ar, nullptr, n, k, l);
+    return ar.off + 256;
+}
+
+int lrp_dst1_batched(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, int64_t ld_in,
+                     double* d_out, int64_t ld_out, double scale) {
+    if (!ctx) return LRP_ERR_BADARG;
+    LRP_TRY(check_n(n));
+    if (batch < 0) return LRP_ERR_BADARG;
+    if (batch == 0) return LRP_OK;
+    if (!d_in || !d_out || !aligned8(d_in) || !aligned8(d_out) || ld_in < n || ld_out < n) return LRP_ERR_BADARG;
+    if (d_in == d_out && ld_in != ld_out) return LRP_ERR_BADARG;
+    return lrp_dst1_impl(ctx, n, batch, d_in, ld_in, d_out, ld_out, scale, ctx->ws, ctx->ws_bytes);
+}
+
+int lrp_sample_fibers(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_Uh, int64_t ldu, const double* d_S,
+                      const double* d_Vh, int64_t ldv, const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,
+                      double* d_C, int64_t ldc, double* d_Rt, int64_t ldr) {
+    if (!ctx || n < 1 || r < 1 || r > 1024 || !d_Uh || !d_S || !d_Vh || ldu < n || ldv < n) return LRP_ERR_BADARG;
+    if (nI < 0 || nJ < 0) return LRP_ERR_BADARG;
+    if (d_C && nJ > 0) {
+        if (!d_J || ldc < n) return LRP_ERR_BADARG;
+        LRP_TRY(sample_side(ctx, n, r, d_Uh, ldu, d_S, d_Vh, ldv, d_J, nJ, d_C, ldc));
+    }
+    if (d_Rt && nI > 0) {
+        if (!d_I || ldr < n) return LRP_ERR_BADARG;
+        LRP_TRY(sample_side(ctx, n, r, d_Vh, ldv, d_S, d_Uh, ldu, d_I, nI, d_Rt, ldr));
+    }
+    return LRP_OK;
+}
+
+int lrp_leverage_select(lrp_ctx* ctx, int64_t n, int32_t k, const double* d_A, int64_t lda,
+                        int32_t num_select, int assume_orthonormal, int32_t* d_idx_out, double* d_scores) {
+    if (!ctx || n < 1 || k < 1 || k > 1024 || !d_A || lda < n || !d_idx_out) return LRP_ERR_BADARG;
+    if (num_select < 0 || num_select > n || num_select > 4096 || (!assume_orthonormal && k > n)) return LRP_ERR_BADARG;
+    if (ctx->ws_bytes < lrp_leverage_workspace_bytes(n, k)) return LRP_ERR_WORKSPACE;
+    lrp_arena ar(ctx->ws, ctx->ws_bytes);
+    double* scratch = ar.take<double>((size_t)n * k);
+    double* R = ar.take<double>((size_t)k * k);
+    double* scores = ar.take<double>((size_t)n);
+    unsigned char* mask = ar.take<unsigned char>(k);
+    double* qr_ws = ar.take<double>(tall_qr_ws_doubles(ctx, n, k));
+    void* sel_ws = ar.take<char>(select_ws_bytes(ctx, n, 4096));
+    if (!ar.ok()) return LRP_ERR_WORKSPACE;
+    double* sc = d_scores ? d_scores : scores;
+    if (assume_orthonormal) LRP_TRY(tall_rownorm2(ctx, n, k, d_A, lda, nullptr, sc));
+    else LRP_TRY(leverage_scores_qr(ctx, n, k, d_A, lda, scratch, n, R, mask, qr_ws, sc));
+    LRP_TRY(select_topk(ctx, n, sc, num_select, d_idx_out, sel_ws));
+    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return LRP_OK;
+}
+
+int lrp_scross(lrp_ctx* ctx, int64_t n, const double* d_C, int64_t ldc, int32_t k, const double* d_Rt, int64_t ldr, int32_t l,
+               const int32_t* d_I, const int32_t* d_J, double* d_U, int64_t ldu, double* d_S, double* d_V, int64_t ldv,
+               double* d_rC, double* d_rR, int32_t* h_rank_out, double* h_smin_full_out) {
+    if (!ctx || n < 1 || k < 1 || l < 1 || k > 1024 || l > 1024 || k > n || l > n) return LRP_ERR_BADARG;
+    if (!d_C || !d_Rt || !d_I || !d_J || !d_U || !d_S || !d_V || ldc < n || ldr < n || ldu < n || ldv < n) return LRP_ERR_BADARG;
+    if (ctx->ws_bytes < lrp_scross_workspace_bytes(n, k, l)) return LRP_ERR_WORKSPACE;
+    {   // index validation (host copy)
+        std::vector<int32_t> hI(l), hJ(k);
+        LRP_CUDA(ctx, cudaMemcpyAsync(hI.data(), d_I, sizeof(int32_t) * l, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(hJ.data(), d_J, sizeof(int32_t) * k, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        LRP_TRY(validate_indices(hI.data(), l, n));
+        LRP_TRY(validate_indices(hJ.data(), k, n));
+    }
+    lrp_arena ar(ctx->ws, ctx->ws_bytes);
+    double* Qb = ar.take<double>((size_t)n * k);
+    double* Zb = ar.take<double>((size_t)n * l);
+    ScrossWs w;
+    if (!w.carve(ar, ctx, n, k, l)) return LRP_ERR_WORKSPACE;
+    LRP_TRY(tall_copy(ctx, n, k, d_C, ldc, Qb, n));
+    LRP_TRY(tall_copy(ctx, n, l, d_Rt, ldr, Zb, n));
+    const int p = k < l ? k : l;
+    std::vector<double> hS(p), hrC(k), hrR(l);
+    int rank = 0; double smin = 0.0;
+    LRP_TRY(scross_factor(ctx, n, Qb, n, k, Zb, n, l, d_I, d_J, w, hS.data(), hrC.data(), hrR.data(), &rank, &smin, nullptr));
+    LRP_TRY(rebuild(ctx, n, Qb, n, k, w.Uc, k, rank, d_U, ldu, nullptr));
+    LRP_TRY(rebuild(ctx, n, Zb, n, l, w.Vc, l, rank, d_V, ldv, nullptr));
+    LRP_CUDA(ctx, cudaMemcpyAsync(d_S, w.S, sizeof(double) * p, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (d_rC) LRP_CUDA(ctx, cudaMemcpyAsync(d_rC, w.rC, sizeof(double) * k, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (d_rR) LRP_CUDA(ctx, cudaMemcpyAsync(d_rR, w.rR, sizeof(double) * l, cudaMemcpyDeviceToDevice, ctx->stream));
+    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (h_rank_out) *h_rank_out = rank;
+    if (h_smin_full_out) *h_smin_full_out = smin;
+    return LRP_OK;
+}
+
+int lrp_lowrank_entries(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_U, int64_t ldu, const double* d_S,
+                        const double* d_V, int64_t ldv, const int64_t* d_rows, const int64_t* d_cols,
+                        int64_t count, double* d_out) {
+    if (!ctx || n < 1 || r < 0 || !d_U || !d_S || !d_V || !d_rows || !d_cols || !d_out || ldu < n || ldv < n || count < 0)
+        return LRP_ERR_BADARG;
+    return tall_lowrank_entries(ctx, r, d_U, ldu, d_S, d_V, ldv, d_rows, d_cols, count, d_out);
+}
+
+int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF, int64_t ldu, const double* d_SF,
+                         const double* d_VF, int64_t ldv, const lrp_solve_opts* opts,
+                         double* d_UW, int64_t lduw, double* d_SW, double* d_VW, int64_t ldvw, lrp_solve_info* info,
+                         int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                         double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
+    if (!ctx || !opts || !info) return LRP_ERR_BADARG;
+    LRP_TRY(check_n(n));
+    if (rF < 1 || !d_UF || !d_SF || !d_VF || !d_UW || !d_SW || !d_VW || ldu < n || ldv < n || lduw < n || ldvw < n) return LRP_ERR_BADARG;
+    if (opts->max_rank < 1 || opts->oversample < 0 || opts->max_sweeps < 1 || !(opts->tol > 0.0)) return LRP_ERR_BADARG;
+    const int max_rank = opts->max_rank, p_os = opts->oversample;
+    int Kc = 2 * (max_rank + p_os);
+    if (Kc < rF + p_os + 1) Kc = rF + p_os + 1;
+    if (Kc > n || rF > n) return LRP_ERR_BADARG;
+    const bool replay = opts->replay_sweeps > 0;
+    const int max_sweeps = replay ? opts->replay_sweeps : opts->max_sweeps;
+    if (max_sweeps > LRP_MAX_SWEEPS_INFO) return LRP_ERR_BADARG;
+    const double* U0 = opts->d_U0; const double* V0 = opts->d_V0; int r0 = opts->r0; int64_t ld0 = opts->ld0;
+    if ((U0 == nullptr) != (V0 == nullptr)) return LRP_ERR_BADARG;
+    if (U0 && (r0 < 1 || r0 + p_os + 1 > Kc || ld0 < n)) return LRP_ERR_BADARG;
+    if (ctx->ws_bytes < lrp_workspace_bytes(n, rF, max_rank, p_os)) return LRP_ERR_WORKSPACE;
+    lrp_arena ar(ctx->ws, ctx->ws_bytes);
+    SolveWs w;
+    if (!w.carve(ar, ctx, n, rF, Kc, max_rank)) return LRP_ERR_WORKSPACE;
+    memset(info, 0, sizeof(*info));
+    const int64_t launches0 = ctx->launches;
+    const int64_t ld = n;
+    const double scale = sqrt(2.0 / (double)(n + 1));
+    EventPool ep;
+    cudaEvent_t e_start = ep.rec(ctx);
+
+    // O3: spectral RHS factors
+    LRP_TRY(lrp_dst1_impl(ctx, n, rF, d_UF, ldu, w.UhF, ld, scale, w.dst_ws, w.dst_ws_bytes));
+    LRP_TRY(lrp_dst1_impl(ctx, n, rF, d_VF, ldv, w.VhF, ld, scale, w.dst_ws, w.dst_ws_bytes));
+    cudaEvent_t e_dst = ep.rec(ctx);
+    info->ms_dst_fwd = 0.f;
+
+    double* Uk = w.Ua; double* Vk = w.Va; double* Up = w.Ub; double* Vp = w.Vb;
+    int r_prev = 0;                       // rank of the previous iterate (0 at k = 0: previous iterate = 0, reading Q13)
+    const double* selU = U0 ? U0 : w.UhF; const double* selV = U0 ? V0 : w.VhF;
+    int64_t sel_ld = U0 ? ld0 : ld; int sel_cols = U0 ? r0 : rF;
+    std::vector<int32_t> I_prev, J_prev, I_k, J_k, hstar(2 * (size_t)Kc + 8);
+    std::vector<double> hS(Kc), hrC(Kc), hrR(Kc), hS_last;
+    std::vector<uint8_t> keepI, keepJ;
+    int rank = 0; double smin = 0.0;
+    bool converged = false;
+    size_t rep_offI = 0, rep_offJ = 0, tr_offI = 0, tr_offJ = 0;
+    int sweeps = 0;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_sel, t_sample, t_qr, t_core, t_rebuild, t_stop;
+
+    for (int k = 0; k < max_sweeps; ++k) {
+        cudaEvent_t e0 = ep.rec(ctx);
+        // ---- O6/O7: selection, union, safeguard
+        if (!replay) {
+            if (k == 0) {
+                LRP_TRY(leverage_scores_qr(ctx, n, sel_cols, selU, sel_ld, w.Cb, ld, w.Rlev, w.mask, w.sc.qr_ws, w.scoresU));
+                LRP_TRY(leverage_scores_qr(ctx, n, sel_cols, selV, sel_ld, w.Cb, ld, w.Rlev, w.mask, w.sc.qr_ws, w.scoresV));
+            }
+            int64_t numsel64 = (int64_t)sel_cols + p_os; if (numsel64 > n) numsel64 = n;
+            if (numsel64 > 2 * (int64_t)Kc) numsel64 = 2 * (int64_t)Kc;
+            const int numsel = (int)numsel64;
+            for (int side = 0; side < 2; ++side) {
+                std::vector<int32_t>& cur = side == 0 ? I_k : J_k;
+                const std::vector<int32_t>& prev = side == 0 ? I_prev : J_prev;
+                double* sc = side == 0 ? w.scoresU : w.scoresV;
+                int32_t* dstar = side == 0 ? w.dIstar : w.dJstar;
+                LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
+                LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                cur = prev;
+                int added = 0;
+                host_union(cur, hstar.data(), numsel, &added);
+                if (added == 0 || k == 0) {       // Alg. 4 lines 7-12, reading Q9
+                    bool done = false;
+                    for (int s = 0; s < opts->n_safeguard && opts->h_safeguard; ++s) {
+                        int32_t cand = opts->h_safeguard[s];
+                        if (cand < 0 || cand >= n) continue;
+                        if (std::find(cur.begin(), cur.end(), cand) == cur.end()) { cur.push_back(cand); done = true; break; }
+                    }
+                    if (!done && (int64_t)cur.size() < n) {   // list exhausted: best-scoring index not in the set
+                        int want = (int)cur.size() + 1; if (want > Kc + 1) want = Kc + 1;
+                        std::vector<int32_t> more(want);
+                        LRP_TRY(select_topk(ctx, n, sc, want, dstar, w.sel_ws));
+                        LRP_CUDA(ctx, cudaMemcpyAsync(more.data(), dstar, sizeof(int32_t) * want, cudaMemcpyDeviceToHost, ctx->stream));
+                        LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                        for (int32_t cand : more)
+                            if (cand >= 0 && std::find(cur.begin(), cur.end(), cand) == cur.end()) { cur.push_back(cand); break; }
+                    }
+                }
+                if ((int)cur.size() > Kc) cur.resize(Kc);       // reading Q10
+            }
+        } else {
+            const int nI = opts->h_replay_nI[k], nJ = opts->h_replay_nJ[k];
+            if (nI < 1 || nJ < 1 || nI > Kc || nJ > Kc) return LRP_ERR_BADARG;
+            I_k.assign(opts->h_replay_I + rep_offI, opts->h_replay_I + rep_offI + nI);
+            J_k.assign(opts->h_replay_J + rep_offJ, opts->h_replay_J + rep_offJ + nJ);
+            LRP_TRY(validate_indices(I_k.data(), nI, n));
+            LRP_TRY(validate_indices(J_k.data(), nJ, n));
+        }
+        const int l = (int)I_k.size(), kk = (int)J_k.size();
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.dI, I_k.data(), sizeof(int32_t) * l, cudaMemcpyHostToDevice, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.dJ, J_k.data(), sizeof(int32_t) * kk, cudaMemcpyHostToDevice, ctx->stream));
+        cudaEvent_t e1 = ep.rec(ctx);
+        // ---- O4: fibers  C = G(:,J) (n x kk), Rt = G(I,:)^T (n x l)
+        LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ, kk, w.Cb, ld));
+        LRP_TRY(sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI, l, w.Rb, ld));
+        cudaEvent_t e2 = ep.rec(ctx);
+        // ---- O8: scross
+        cudaEvent_t e3 = nullptr;
+        { cudaEvent_t tmp; if (cudaEventCreate(&tmp) == cudaSuccess) { ep.ev.push_back(tmp); e3 = tmp; } }
+        LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, w.Rb, ld, l, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
+        cudaEvent_t e4 = ep.rec(ctx);
+        const int p = kk < l ? kk : l;
+        LRP_TRY(rebuild(ctx, n, w.Cb, ld, kk, w.sc.Uc, kk, rank, Uk, ld, w.scoresU));
+        LRP_TRY(rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
+        cudaEvent_t e5 = ep.rec(ctx);
+        // ---- O9: prune (Alg. 4 lines 14-23; reading Q12)
+        keepI.assign(l, 1); keepJ.assign(kk, 1);
+        if (replay && opts->h_replay_keepI && opts->h_replay_keepJ) {
+            for (int c = 0; c < l; ++c) keepI[c] = opts->h_replay_keepI[rep_offI + c] ? 1 : 0;
+            for (int c = 0; c < kk; ++c) keepJ[c] = opts->h_replay_keepJ[rep_offJ + c] ? 1 : 0;
+        } else {
+            double mR = 0.0, mC = 0.0;
+            for (int c = 0; c < l; ++c) mR = std::max(mR, hrR[c]);
+            for (int c = 0; c < kk; ++c) mC = std::max(mC, hrC[c]);
+            for (int c = 0; c < l; ++c) keepI[c] = hrR[c] >= PRUNE_REL * mR;
+            for (int c = 0; c < kk; ++c) keepJ[c] = hrC[c] >= PRUNE_REL * mC;
+        }
+        std::vector<int32_t> I_pr, J_pr;
+        for (int c = 0; c < l; ++c) if (keepI[c]) I_pr.push_back(I_k[c]);
+        for (int c = 0; c < kk; ++c) if (keepJ[c]) J_pr.push_back(J_k[c]);
+        if (h_trace_I) memcpy(h_trace_I + tr_offI, I_k.data(), sizeof(int32_t) * l);
+        if (h_trace_J) memcpy(h_trace_J + tr_offJ, J_k.data(), sizeof(int32_t) * kk);
+        if (h_trace_keepI) memcpy(h_trace_keepI + tr_offI, keepI.data(), l);
+        if (h_trace_keepJ) memcpy(h_trace_keepJ + tr_offJ, keepJ.data(), kk);
+        tr_offI += l; tr_offJ += kk; rep_offI += l; rep_offJ += kk;
+        // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
+        RhoArgs ra{};
+        ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
+        ra.out = w.rho_out;
+        if (r_prev > 0) {
+            for (int side = 0; side < 2; ++side) {
+                const double* Xk = side == 0 ? Uk : Vk; const double* Xp = side == 0 ? Up : Vp;
+                double* Am = side == 0 ? w.Amat : w.Bmat; double* G = side == 0 ? w.GU : w.GV;
+                double* E = side == 0 ? w.Cb : w.Rb;                      // fiber buffers are free after the rebuild
+                LRP_TRY(tall_gemm_t(ctx, n, Xk, ld, rank, Xp, ld, r_prev, Am, rank, 0, w.gemmt_ws));
+                TallGemmArgs g{};
+                g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Xk; g.lda = ld; g.B = Am; g.ldb = rank;
+                g.Cin = Xp; g.ldc = ld; g.Out = E; g.ldo = ld;
+                LRP_TRY(tall_gemm(ctx, g));
+                LRP_TRY(tall_gemm_t(ctx, n, E, ld, r_prev, E, ld, r_prev, G, r_prev, 0, w.gemmt_ws));
+            }
+        }
+        LRP_TRY(rho_small(ctx, ra));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream));
+        EtaArgs ea{};
+        ea.r = rank; ea.U = Uk; ea.ldu = ld; ea.I = w.dIpr; ea.nI = (int)I_pr.size(); ea.V = Vk; ea.ldv = ld; ea.J = w.dJpr; ea.nJ = (int)J_pr.size();
+        ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
+        LRP_TRY(eta_pair(ctx, ea));
+        double h_rho[2], h_eta[2];
+        LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(h_eta, w.eta, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.Sprev, w.sc.S, sizeof(double) * rank, cudaMemcpyDeviceToDevice, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaEvent_t e6 = ep.rec(ctx);
+        const double rho = h_rho[0], snorm = h_rho[1], eta1 = h_eta[0], eta2 = h_eta[1];
+        const double ind = (smin == 0.0) ? 0.0 : std::min(eta1 * (1.0 + eta2), eta2 * (1.0 + eta1)) * smin;
+        info->nI[k] = l; info->nJ[k] = kk; info->rank_per_sweep[k] = rank; info->rho_per_sweep[k] = rho; info->ind_per_sweep[k] = ind;
+        info->rho = rho; info->indicator = ind; info->eta1 = eta1; info->eta2 = eta2; info->snorm = snorm; info->smin_full = smin;
+        t_sel.push_back({e0, e1}); t_sample.push_back({e1, e2}); t_qr.push_back({e2, e3}); t_core.push_back({e3, e4});
+        t_rebuild.push_back({e4, e5}); t_stop.push_back({e5, e6});
+        hS_last.assign(hS.begin(), hS.begin() + p);
+        sweeps = k + 1;
+        // next sweep: warm start from this iterate
+        std::swap(Uk, Up); std::swap(Vk, Vp);
+        r_prev = rank; sel_cols = rank;
+        I_prev = I_pr; J_prev = J_pr;
+        const double thresh = opts->tol * (opts->tol_mode == 0 ? snorm : 1.0);
+        if (!replay && std::max(rho, ind) < thresh) { converged = true; break; }   // Alg. 4 line 26
+    }
+    // after the swap the last iterate lives in (Up, Vp), rank r_prev
+    int r;
+    if (replay && opts->replay_final_rank > 0) { r = opts->replay_final_rank; converged = true; }
+    else r = final_rank_host(hS_last.data(), r_prev, opts->tol, max_rank, opts->tol_mode);     // O11 over the kept values
+    if (r > r_prev) r = r_prev;
+    if (r > max_rank) r = max_rank;
+    cudaEvent_t e_inv0 = ep.rec(ctx);
+    LRP_TRY(lrp_dst1_impl(ctx, n, r, Up, ld, d_UW, lduw, scale, w.dst_ws, w.dst_ws_bytes));      // O12
+    LRP_TRY(lrp_dst1_impl(ctx, n, r, Vp, ld, d_VW, ldvw, scale, w.dst_ws, w.dst_ws_bytes));
+    LRP_CUDA(ctx, cudaMemcpyAsync(d_SW, w.Sprev, sizeof(double) * r, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (d_Uhat && d_Vhat && d_Shat && ld_hat >= n) {
+        LRP_TRY(tall_copy(ctx, n, r_prev, Up, ld, d_Uhat, ld_hat));
+        LRP_TRY(tall_copy(ctx, n, r_prev, Vp, ld, d_Vhat, ld_hat));
+        LRP_CUDA(ctx, cudaMemcpyAsync(d_Shat, w.Sprev, sizeof(double) * r_prev, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    cudaEvent_t e_end = ep.rec(ctx);
+    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    info->rank = r; info->sweeps = sweeps; info->converged = converged ? 1 : 0;
+    info->ms_dst_fwd = EventPool::ms(e_start, e_dst);
+    for (auto& pr : t_sel) info->ms_select += EventPool::ms(pr.first, pr.second);
+    for (auto& pr : t_sample) info->ms_sample += EventPool::ms(pr.first, pr.second);
+    for (auto& pr : t_qr) info->ms_qr += EventPool::ms(pr.first, pr.second);
+    for (auto& pr : t_core) info->ms_core += EventPool::ms(pr.first, pr.second);
+    for (auto& pr : t_rebuild) info->ms_rebuild += EventPool::ms(pr.first, pr.second);
+    for (auto& pr : t_stop) info->ms_stop += EventPool::ms(pr.first, pr.second);
+    info->ms_dst_inv = EventPool::ms(e_inv0, e_end);
+    info->ms_total = EventPool::ms(e_start, e_end);
+    info->launches = ctx->launches - launches0;
+    return converged ? LRP_OK : LRP_WARN_NOCONV;
+}
+
+}  // extern "C"

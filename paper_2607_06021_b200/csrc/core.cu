@@ -1,0 +1,320 @@
+// core.cu -- the small dense core of scross and of the Cross-DEIM stop test, one CTA per problem:
+//   one-sided (Hestenes) Jacobi SVD, SVD pseudo-inverse, the k x l core M of Alg. 1 lines 5-15,
+//   eta = 1/sigma_min(U_k(I_k,:)) (Alg. 4 line 25) and rho (Alg. 4 line 24).
+// Everything here is K x K (K <= a few hundred): latency-bound, not a roofline item.  Matrices live in the
+// caller's workspace (L1/L2 resident for the single CTA that touches them), column-major.
+#include "common.cuh"
+#include "core.cuh"
+#include <math.h>
+#include <float.h>
+
+namespace {
+
+constexpr int CORE_NT = 1024;
+constexpr int JACOBI_MAX_SWEEPS = 60;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+// One-sided Jacobi on A (m x n, m >= n, ld lda), accumulating the rotations into V (n x n, ld ldv, must be I on
+// entry).  Round-robin tournament ordering; one warp per column pair.  On exit A = U diag(s), columns orthogonal.
+__device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int np = (n + 1) & ~1;                 // players (padded to even)
+    if (n < 2) return;
+    for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
+        if (tid == 0) *s_flag = 0;
+        __syncthreads();
+        for (int r = 0; r < np - 1; ++r) {
+            for (int i = warp; i < np / 2; i += nwarps) {
+                int p, q;
+                if (i == 0) { p = np - 1; q = r; }
+                else { p = (r + i) % (np - 1); q = (r - i + (np - 1)) % (np - 1); }
+                if (p > q) { int t = p; p = q; q = t; }
+                if (q >= n) continue;
+                double* ap = A + (size_t)p * lda;
+                double* aq = A + (size_t)q * lda;
+                double al = 0.0, be = 0.0, ga = 0.0;
+                for (int t = lane; t < m; t += 32) {
+                    double x = ap[t], y = aq[t];
+                    al = fma(x, x, al); be = fma(y, y, be); ga = fma(x, y, ga);
+                }
+                al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
+                if (ga == 0.0 || fabs(ga) <= DBL_EPSILON * sqrt(al * be)) continue;
+                double zeta = (be - al) / (2.0 * ga);
+                double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+                double c = 1.0 / sqrt(1.0 + tt * tt), s = c * tt;
+                for (int t = lane; t < m; t += 32) {
+                    double x = ap[t], y = aq[t];
+                    ap[t] = c * x - s * y; aq[t] = s * x + c * y;
+                }
+                double* vp = V + (size_t)p * ldv;
+                double* vq = V + (size_t)q * ldv;
+                for (int t = lane; t < n; t += 32) {
+                    double x = vp[t], y = vq[t];
+                    vp[t] = c * x - s * y; vq[t] = s * x + c * y;
+                }
+                if (lane == 0) *s_flag = 1;
+            }
+            __syncthreads();
+        }
+        int again = *s_flag;
+        __syncthreads();
+        if (!again) break;
+    }
+}
+
+// Thin SVD of M (m x n, ld ldm): U (m x p), s (p, descending), V (n x p), p = min(m, n).
+// work: max(m,n)*p + p*p + p doubles, iwork: p ints.  Columns of U for exactly-zero singular values are zero.
+__device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int ldu, double* s, double* V, int ldv,
+                        double* work, int* iwork, int* s_flag) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const bool tr = m < n;
+    const int T = tr ? n : m, p = tr ? m : n;
+    double* A = work;               // T x p
+    double* W = A + (size_t)T * p;  // p x p
+    double* sv = W + (size_t)p * p; // p
+    for (int e = tid; e < T * p; e += nt) {
+        int t = e % T, c = e / T;
+        A[e] = tr ? M[c + (size_t)t * ldm] : M[t + (size_t)c * ldm];
+    }
+    for (int e = tid; e < p * p; e += nt) W[e] = (e % p == e / p) ? 1.0 : 0.0;
+    __syncthreads();
+    cta_jacobi(A, T, T, p, W, p, s_flag);
+    __syncthreads();
+    {   // column norms, one warp per column
+        const int lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
+        for (int c = warp; c < p; c += nwarps) {
+            double acc = 0.0;
+            for (int t = lane; t < T; t += 32) { double x = A[t + (size_t)c * T]; acc = fma(x, x, acc); }
+            acc = warp_sum(acc);
+            if (lane == 0) sv[c] = sqrt(acc);
+        }
+    }
+    __syncthreads();
+    for (int c = tid; c < p; c += nt) {   // rank by (value desc, index asc)
+        int rk = 0; double v = sv[c];
+        for (int o = 0; o < p; ++o) rk += (sv[o] > v) || (sv[o] == v && o < c);
+        iwork[c] = rk;
+    }
+    __syncthreads();
+    double* Ubig = tr ? V : U; int ldbig = tr ? ldv : ldu;       // receives the normalised A columns (T rows)
+    double* Usml = tr ? U : V; int ldsml = tr ? ldu : ldv;       // receives the rotation columns (p rows)
+    for (int e = tid; e < T * p; e += nt) {
+        int t = e % T, c = e / T; double v = sv[c];
+        Ubig[t + (size_t)iwork[c] * ldbig] = v > 0.0 ? A[e] / v : 0.0;
+    }
+    for (int e = tid; e < p * p; e += nt) {
+        int t = e % p, c = e / p;
+        Usml[t + (size_t)iwork[c] * ldsml] = W[e];
+    }
+    for (int c = tid; c < p; c += nt) s[iwork[c]] = sv[c];
+    __syncthreads();
+}
+
+// C (m x n, ldc) = op(A) op(B) with explicit strides: A(i,t) = A[i*sai + t*sat], B(t,j) = B[t*sbt + j*sbj]
+__device__ void cta_matmul(double* C, int ldc, int m, int n, int kk, const double* A, int sai, int sat,
+                           const double* B, int sbt, int sbj) {
+    for (int e = threadIdx.x; e < m * n; e += blockDim.x) {
+        int i = e % m, j = e / m;
+        double acc = 0.0;
+        for (int t = 0; t < kk; ++t) acc = fma(A[(size_t)i * sai + (size_t)t * sat], B[(size_t)t * sbt + (size_t)j * sbj], acc);
+        C[i + (size_t)j * ldc] = acc;
+    }
+    __syncthreads();
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// scross core.  QR factors: Qf (n x k) with R_C (k x k), Zf (n x l) with R_R (l x l).
+__global__ void __launch_bounds__(CORE_NT)
+scross_core_kernel(CoreArgs a) {
+    __shared__ int s_flag;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int k = a.k, l = a.l;
+    const bool kle = k <= l;
+    // X = Q(I,:) (l x k) if k <= l else Z(J,:) (k x l)
+    const int xm = kle ? l : k, xn = kle ? k : l;      // xm >= xn
+    const double* F = kle ? a.Q : a.Z; const int64_t ldf = kle ? a.ldq : a.ldz;
+    const int32_t* idx = kle ? a.I : a.J;
+    double* X = a.work;                                 // xm x xn
+    double* Ux = X + (size_t)xm * xn;                   // xm x xn
+    double* sx = Ux + (size_t)xm * xn;                  // xn
+    double* Vx = sx + xn;                               // xn x xn
+    double* P = Vx + (size_t)xn * xn;                   // xn x xm   (pseudo-inverse)
+    double* Mc = P + (size_t)xn * xm;                   // k x l
+    double* svdw = Mc + (size_t)k * l;                  // SVD scratch
+    for (int e = tid; e < xm * xn; e += nt) {
+        int r = e % xm, c = e / xm;
+        X[e] = F[(int64_t)idx[r] + (int64_t)c * ldf];
+    }
+    for (int c = tid; c < k; c += nt) a.rC[c] = fabs(a.RC[c + (size_t)c * a.ldrc]);
+    for (int c = tid; c < l; c += nt) a.rR[c] = fabs(a.RR[c + (size_t)c * a.ldrr]);
+    __syncthreads();
+    cta_svd(X, xm, xm, xn, Ux, xm, sx, Vx, xn, svdw, a.iwork, &s_flag);
+    // P = Vx diag(1/sx) Ux^T over the kept singular values (relative cut, reading Q4)
+    {
+        const double cut = a.pinv_rcond * sx[0];
+        for (int e = tid; e < xn * xm; e += nt) {
+            int i = e % xn, j = e / xn;
+            double acc = 0.0;
+            for (int t = 0; t < xn; ++t) {
+                double sv = sx[t];
+                if (sv > cut) acc = fma(Vx[i + (size_t)t * xn] / sv, Ux[j + (size_t)t * xm], acc);
+            }
+            P[e] = acc;
+        }
+        __syncthreads();
+    }
+    if (kle) {
+        // M = P (k x l) * R_R^T (l x l):  M(i,j) = sum_t P(i,t) R_R(j,t)
+        cta_matmul(Mc, k, k, l, l, P, 1, k, a.RR, (int)a.ldrr, 1);
+    } else {
+        // M = R_C (k x k) * P^T (k x l): M(i,j) = sum_t R_C(i,t) P(j,t),  P is l x k
+        cta_matmul(Mc, k, k, l, k, a.RC, 1, (int)a.ldrc, P, l, 1);
+    }
+    const int p = k < l ? k : l;
+    cta_svd(Mc, k, k, l, a.Uc, k, a.S, a.Vc, l, svdw, a.iwork, &s_flag);
+    if (tid == 0) {
+        double s1 = a.S[0];
+        int rank = 0;
+        for (int c = 0; c < p; ++c) rank += a.S[c] > a.rank_rcond * s1;
+        if (rank < 1) rank = 1;
+        a.scal_i[0] = rank;
+        a.scal_d[0] = a.S[p - 1];                       // smin_full (reading Q11)
+    }
+}
+
+// eta_side = 1 / sigma_min(F(idx,:)), F tall n x r, idx: nidx indices.  blockIdx.x selects the side (U/I or V/J).
+__global__ void __launch_bounds__(CORE_NT)
+eta_kernel(EtaArgs a) {
+    __shared__ int s_flag;
+    const int side = blockIdx.x;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const double* F = side == 0 ? a.U : a.V; const int64_t ldf = side == 0 ? a.ldu : a.ldv;
+    const int32_t* idx = side == 0 ? a.I : a.J; const int nidx = side == 0 ? a.nI : a.nJ;
+    const int r = a.r;
+    double* out = a.eta + side;
+    if (nidx == 0 || r == 0) { if (tid == 0) *out = INFINITY; return; }
+    double* work = a.work + (size_t)side * a.work_stride;
+    int* iwork = a.iwork + (size_t)side * a.iwork_stride;
+    const int p = nidx < r ? nidx : r;
+    double* X = work;                                    // nidx x r
+    double* Ux = X + (size_t)nidx * r;                   // nidx x p
+    double* sx = Ux + (size_t)nidx * p;                  // p
+    double* Vx = sx + p;                                 // r x p
+    double* svdw = Vx + (size_t)r * p;
+    for (int e = tid; e < nidx * r; e += nt) {
+        int i = e % nidx, c = e / nidx;
+        X[e] = F[(int64_t)idx[i] + (int64_t)c * ldf];
+    }
+    __syncthreads();
+    cta_svd(X, nidx, nidx, r, Ux, nidx, sx, Vx, r, svdw, iwork, &s_flag);
+    if (tid == 0) { double sm = sx[p - 1]; *out = sm == 0.0 ? INFINITY : 1.0 / sm; }
+}
+
+// rho^2 = ||S_k - A S' B^T||_F^2 + ||A S' E_V^T||_F^2 + ||E_U S' B^T||_F^2 + ||E_U S' E_V^T||_F^2 with
+// U_{k-1} = U_k A + E_U, V_{k-1} = V_k B + E_V (A = U_k^T U_{k-1}, B = V_k^T V_{k-1}, GU = E_U^T E_U, GV = E_V^T E_V).
+// All four terms are non-negative (no Gram expansion of the difference; reading Q13).
+__global__ void __launch_bounds__(CORE_NT)
+rho_kernel(RhoArgs a) {
+    __shared__ double red[32];
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int r = a.r, rp = a.rp;
+    double acc = 0.0;
+    // T1 = A diag(Sp)  (r x rp);  term1: sum_{i,j} (Sk(i) delta_ij - sum_t T1(i,t) B(j,t))^2
+    for (int e = tid; e < r * r; e += nt) {
+        int i = e % r, j = e / r;
+        double v = (i == j) ? a.Sk[i] : 0.0;
+        for (int t = 0; t < rp; ++t) v = fma(-a.A[i + (size_t)t * r] * a.Sp[t], a.B[j + (size_t)t * r], v);
+        acc = fma(v, v, acc);
+    }
+    // term2: ||A S' E_V^T||_F^2 = sum_i sum_{t,u} A(i,t) Sp(t) GV(t,u) Sp(u) A(i,u);  term3 likewise with B, GU
+    for (int e = tid; e < 2 * r; e += nt) {
+        int i = e % r; const double* Mx = e < r ? a.A : a.B; const double* G = e < r ? a.GV : a.GU;
+        double s = 0.0;
+        for (int t = 0; t < rp; ++t) {
+            double w = 0.0;
+            for (int u = 0; u < rp; ++u) w = fma(G[t + (size_t)u * rp], a.Sp[u] * Mx[i + (size_t)u * r], w);
+            s = fma(Mx[i + (size_t)t * r] * a.Sp[t], w, s);
+        }
+        acc += s > 0.0 ? s : 0.0;
+    }
+    // term4: ||E_U S' E_V^T||_F^2 = sum_{t,u} GU(t,u) Sp(t) Sp(u) GV(t,u)
+    for (int e = tid; e < rp * rp; e += nt) {
+        int t = e % rp, u = e / rp;
+        acc = fma(a.GU[e] * a.Sp[t] * a.Sp[u], a.GV[e], acc);
+    }
+    acc = warp_sum(acc);
+    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < nt / 32; ++w) t += red[w];
+        double sn = 0.0;
+        for (int c = 0; c < r; ++c) sn = fma(a.Sk[c], a.Sk[c], sn);
+        a.out[0] = sqrt(t > 0.0 ? t : 0.0);
+        a.out[1] = sqrt(sn);
+    }
+}
+
+__global__ void snorm_kernel(int r, const double* S, double* out) {
+    if (threadIdx.x == 0) {
+        double sn = 0.0;
+        for (int c = 0; c < r; ++c) sn = fma(S[c], S[c], sn);
+        out[0] = sqrt(sn); out[1] = sqrt(sn);
+    }
+}
+
+__global__ void colmask_kernel(int k, const double* R, int64_t ldr, double rcond, unsigned char* mask) {
+    __shared__ double mx;
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int c = 0; c < k; ++c) m = fmax(m, fabs(R[c + (size_t)c * ldr]));
+        mx = m;
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c < k; c += blockDim.x) mask[c] = (mx > 0.0 && fabs(R[c + (size_t)c * ldr]) >= rcond * mx) ? 1 : 0;
+}
+
+}  // namespace
+
+size_t core_work_doubles(int k, int l) {
+    size_t xm = k > l ? k : l, xn = k > l ? l : k;
+    size_t d = 0;
+    d += xm * xn * 2 + xn + xn * xn + xn * xm + (size_t)k * l;
+    d += xm * xn + xn * xn + xn + 64;       // SVD scratch (T*p + p*p + p)
+    return d;
+}
+
+int scross_core(lrp_ctx* ctx, const CoreArgs& a) {
+    scross_core_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+
+size_t eta_work_doubles(int nmax, int r) {
+    size_t p = nmax < r ? nmax : r, T = nmax > r ? nmax : r;
+    return (size_t)nmax * r + (size_t)nmax * p + p + (size_t)r * p + T * p + p * p + p + 64;
+}
+
+int eta_pair(lrp_ctx* ctx, const EtaArgs& a) {
+    eta_kernel<<<2, CORE_NT, 0, ctx->stream>>>(a);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+
+int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
+    if (a.rp == 0) snorm_kernel<<<1, 32, 0, ctx->stream>>>(a.r, a.Sk, a.out);
+    else rho_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+
+int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double rcond, unsigned char* mask) {
+    colmask_kernel<<<1, 128, 0, ctx->stream>>>(k, R, ldr, rcond, mask);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}

@@ -1,0 +1,44 @@
+// core.cuh -- one-CTA small dense kernels (core.cu) and index selection (select.cu)
+#pragma once
+#include "common.cuh"
+
+struct CoreArgs {
+    int k, l;                                   // k = #J (columns of C), l = #I (columns of Rt)
+    const double* Q; int64_t ldq;               // n x k, orthonormal factor of C
+    const double* Z; int64_t ldz;               // n x l, orthonormal factor of Rt
+    const double* RC; int64_t ldrc;             // k x k
+    const double* RR; int64_t ldrr;             // l x l
+    const int32_t* I; const int32_t* J;         // device index lists
+    double pinv_rcond, rank_rcond;
+    double* Uc; double* S; double* Vc;          // k x p (ld k), p, l x p (ld l), p = min(k, l)
+    double* rC; double* rR;                     // |diag R_C| (k), |diag R_R| (l)
+    int32_t* scal_i; double* scal_d;            // [0] = numerical rank ; [0] = smin_full
+    double* work; int32_t* iwork;               // core_work_doubles(k, l) doubles, max(k, l) ints
+};
+size_t core_work_doubles(int k, int l);
+int scross_core(lrp_ctx* ctx, const CoreArgs& a);
+
+struct EtaArgs {
+    int r;
+    const double* U; int64_t ldu; const int32_t* I; int nI;
+    const double* V; int64_t ldv; const int32_t* J; int nJ;
+    double* eta;                                // [2] device: eta1, eta2
+    double* work; size_t work_stride; int32_t* iwork; size_t iwork_stride;
+};
+size_t eta_work_doubles(int nmax, int r);
+int eta_pair(lrp_ctx* ctx, const EtaArgs& a);
+
+struct RhoArgs {
+    int r, rp;                                  // ranks of the current and previous iterate
+    const double* Sk; const double* Sp;
+    const double* A; const double* B;           // r x rp (ld r): U_k^T U_{k-1}, V_k^T V_{k-1}
+    const double* GU; const double* GV;         // rp x rp (ld rp): E_U^T E_U, E_V^T E_V
+    double* out;                                // [2] device: rho, ||S_k||_2
+};
+int rho_small(lrp_ctx* ctx, const RhoArgs& a);
+
+int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double rcond, unsigned char* mask);
+
+// top-`num` of scores[0..n) ordered by (score desc, index asc) -> idx_out (device).  ws: select_ws_bytes(ctx, n, num).
+size_t select_ws_bytes(const lrp_ctx* ctx, int64_t n, int num);
+int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t* idx_out, void* ws);

@@ -1,0 +1,32 @@
+// tall.cuh -- host-side entry points of the tall-matrix streaming kernels (tall.cu).
+#pragma once
+#include "common.cuh"
+
+enum { TG_PLAIN = 0, TG_SAMPLE = 1, TG_SUBTRACT = 2 };
+
+// Out(n x m, ld ldo) = epilogue( A(n x k, ld lda) * B(k x m) )
+//   TG_PLAIN    : B column-major k x m with ld ldb;                 Out = A B
+//   TG_SUBTRACT : same B;                                          Out = Cin - A B   (Cin may alias Out)
+//   TG_SAMPLE   : B(t,c) = scale_t[t] * Bsrc[idx[c] + t*ldb] (gathered rows of a tall factor);
+//                 Out(i,c) = (A B)(i,c) / (d_i + d_idx[c])         eq. (4)
+//   rownorm2 (may be NULL): rownorm2[i] = sum_c Out(i,c)^2          (next sweep's leverage scores, Alg. 3 line 3)
+struct TallGemmArgs {
+    int64_t n; int k; int m; int mode;
+    const double* A; int64_t lda;
+    const double* B; int64_t ldb;
+    const int32_t* idx; const double* scale_t;
+    const double* Cin; int64_t ldc;
+    double* Out; int64_t ldo;
+    double* rownorm2;
+};
+
+int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p);
+// S(k x m, ld lds) (+)= A(n x k)^T B(n x m); partial_ws: tall_gemm_t_ws_doubles(ctx, n, k, m) doubles of scratch
+size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m);
+int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
+                double* S, int64_t lds, int accumulate, double* partial_ws);
+int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, const unsigned char* colmask, double* out);
+int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const int32_t* idx, int nidx, double* Out, int ldo);
+int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb);
+int tall_lowrank_entries(lrp_ctx* ctx, int r, const double* U, int64_t ldu, const double* S, const double* V, int64_t ldv,
+                         const int64_t* rows, const int64_t* cols, int64_t count, double* out);

@@ -1,0 +1,296 @@
+"""Thin ctypes binding of liblrp (include/lrp.h): argument marshalling only -- every step of the hot path
+runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory and streams.
+
+Layout convention of this binding: a "tall" n x k matrix (column-major, ld = n, as the C ABI wants) is a
+contiguous CUDA float64 tensor of shape (k, n): element (i, c) lives at t[c, i].  `tall_from_numpy` /
+`tall_to_numpy` convert from/to ordinary (n, k) numpy arrays.
+
+There is no CPU fallback: if liblrp.so is missing (run `python -m paper_2607_06021_b200.build`) or no CUDA
+device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblrp.so")
+
+LRP_OK, LRP_ERR_BADARG, LRP_ERR_UNSUPPORTED_N, LRP_ERR_WORKSPACE, LRP_ERR_CUDA, LRP_WARN_NOCONV = 0, -1, -2, -3, -4, 1
+MAX_SWEEPS_INFO = 32
+
+EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "lrp_launch_count",
+           "lrp_workspace_bytes", "lrp_dst1_workspace_bytes", "lrp_leverage_workspace_bytes",
+           "lrp_scross_workspace_bytes", "lrp_set_workspace", "lrp_dst1_batched", "lrp_sample_fibers",
+           "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries"]
+
+
+class SolveOpts(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_rank", C.c_int32), ("oversample", C.c_int32), ("max_sweeps", C.c_int32),
+                ("tol_mode", C.c_int32), ("h_safeguard", C.c_void_p), ("n_safeguard", C.c_int32),
+                ("d_U0", C.c_void_p), ("d_V0", C.c_void_p), ("ld0", C.c_int64), ("r0", C.c_int32),
+                ("replay_sweeps", C.c_int32), ("h_replay_nI", C.c_void_p), ("h_replay_nJ", C.c_void_p),
+                ("h_replay_I", C.c_void_p), ("h_replay_J", C.c_void_p), ("h_replay_keepI", C.c_void_p),
+                ("h_replay_keepJ", C.c_void_p), ("replay_final_rank", C.c_int32)]
+
+
+class SolveInfo(C.Structure):
+    _fields_ = [("rank", C.c_int32), ("sweeps", C.c_int32), ("converged", C.c_int32),
+                ("rho", C.c_double), ("indicator", C.c_double), ("eta1", C.c_double), ("eta2", C.c_double),
+                ("snorm", C.c_double), ("smin_full", C.c_double),
+                ("nI", C.c_int32 * MAX_SWEEPS_INFO), ("nJ", C.c_int32 * MAX_SWEEPS_INFO),
+                ("rank_per_sweep", C.c_int32 * MAX_SWEEPS_INFO),
+                ("rho_per_sweep", C.c_double * MAX_SWEEPS_INFO), ("ind_per_sweep", C.c_double * MAX_SWEEPS_INFO),
+                ("ms_dst_fwd", C.c_float), ("ms_select", C.c_float), ("ms_sample", C.c_float), ("ms_qr", C.c_float),
+                ("ms_core", C.c_float), ("ms_rebuild", C.c_float), ("ms_stop", C.c_float), ("ms_dst_inv", C.c_float),
+                ("ms_total", C.c_float), ("launches", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library():
+    """Load liblrp.so and declare the prototypes; raises if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2607_06021_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_size_t
+    lib.lrp_create.argtypes = [C.POINTER(vp), C.c_int, vp]; lib.lrp_create.restype = C.c_int
+    lib.lrp_destroy.argtypes = [vp]; lib.lrp_destroy.restype = C.c_int
+    lib.lrp_strerror.argtypes = [C.c_int]; lib.lrp_strerror.restype = C.c_char_p
+    lib.lrp_last_cuda_error.argtypes = [vp]; lib.lrp_last_cuda_error.restype = C.c_int
+    lib.lrp_launch_count.argtypes = [vp]; lib.lrp_launch_count.restype = i64
+    lib.lrp_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_workspace_bytes.restype = sz
+    lib.lrp_dst1_workspace_bytes.argtypes = [i64, i32]; lib.lrp_dst1_workspace_bytes.restype = sz
+    lib.lrp_leverage_workspace_bytes.argtypes = [i64, i32]; lib.lrp_leverage_workspace_bytes.restype = sz
+    lib.lrp_scross_workspace_bytes.argtypes = [i64, i32, i32]; lib.lrp_scross_workspace_bytes.restype = sz
+    lib.lrp_set_workspace.argtypes = [vp, vp, sz]; lib.lrp_set_workspace.restype = C.c_int
+    lib.lrp_dst1_batched.argtypes = [vp, i64, i32, vp, i64, vp, i64, dbl]; lib.lrp_dst1_batched.restype = C.c_int
+    lib.lrp_sample_fibers.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, i32, vp, i32, vp, i64, vp, i64]
+    lib.lrp_sample_fibers.restype = C.c_int
+    lib.lrp_leverage_select.argtypes = [vp, i64, i32, vp, i64, i32, C.c_int, vp, vp]; lib.lrp_leverage_select.restype = C.c_int
+    lib.lrp_scross.argtypes = [vp, i64, vp, i64, i32, vp, i64, i32, vp, vp, vp, i64, vp, vp, i64, vp, vp,
+                               C.POINTER(i32), C.POINTER(dbl)]
+    lib.lrp_scross.restype = C.c_int
+    lib.lrp_cross_deim_solve.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64,
+                                         C.POINTER(SolveInfo), vp, vp, vp, vp, vp, vp, vp, i64]
+    lib.lrp_cross_deim_solve.restype = C.c_int
+    lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+    lib.lrp_lowrank_entries.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+class LrpError(RuntimeError):
+    def __init__(self, code, where, cuda=0):
+        msg = load_library().lrp_strerror(code).decode()
+        super().__init__(f"{where}: {msg} (code {code}, cudaError {cuda})")
+        self.code = code
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def tall_from_numpy(a: np.ndarray, device="cuda:0"):
+    """(n, k) numpy -> device tall tensor of shape (k, n)."""
+    torch = _torch()
+    a = np.asarray(a, dtype=np.float64)
+    if a.ndim == 1:
+        a = a[:, None]
+    return torch.from_numpy(np.ascontiguousarray(a.T)).to(device)
+
+
+def tall_to_numpy(t) -> np.ndarray:
+    return t.detach().cpu().numpy().T.copy()
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _check_tall(t, name):
+    torch = _torch()
+    if not (t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and t.stride(1) == 1):
+        raise ValueError(f"{name}: expected a CUDA float64 tensor of shape (cols, n) with contiguous rows")
+    return t.shape[0], t.shape[1], t.stride(0) if t.shape[0] > 1 else max(t.stride(0), t.shape[1])
+
+
+class Context:
+    """Owns an lrp_ctx bound to a device and to torch's current stream on it, plus the workspace tensor."""
+
+    def __init__(self, device: int = 0, stream=None):
+        torch = _torch()
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("liblrp needs a CUDA device (no CPU fallback)")
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        rc = self.lib.lrp_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream))
+        if rc != 0:
+            raise LrpError(rc, "lrp_create")
+        self.h = h
+        self._ws = None
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.lrp_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, where):
+        if rc < 0:
+            raise LrpError(rc, where, self.lib.lrp_last_cuda_error(self.h))
+        return rc
+
+    def launch_count(self) -> int:
+        return int(self.lib.lrp_launch_count(self.h))
+
+    def ensure_workspace(self, nbytes: int):
+        torch = _torch()
+        if self._ws is None or self._ws.numel() < nbytes:
+            self._ws = None
+            self._ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
+            self._check(self.lib.lrp_set_workspace(self.h, _ptr(self._ws), self._ws.numel()), "lrp_set_workspace")
+
+    # ------------------------------------------------------------------ the five calls of the boundary
+    def dst1_batched(self, x, out=None, scale: float = 1.0):
+        """out(:, b) = scale * DST-I(x(:, b)); x, out tall tensors of shape (batch, n).  out may be x."""
+        torch = _torch()
+        batch, n, ld_in = _check_tall(x, "x")
+        if out is None:
+            out = torch.empty_like(x)
+        _, _, ld_out = _check_tall(out, "out")
+        self.ensure_workspace(self.lib.lrp_dst1_workspace_bytes(n, batch))
+        self._check(self.lib.lrp_dst1_batched(self.h, n, batch, _ptr(x), ld_in, _ptr(out), ld_out, float(scale)),
+                    "lrp_dst1_batched")
+        return out
+
+    def sample_fibers(self, Uh, S, Vh, I=None, J=None):
+        """C = G(:, J) and Rt = G(I, :)^T as tall tensors (|J|, n), (|I|, n); I, J int32 CUDA tensors."""
+        torch = _torch()
+        r, n, ldu = _check_tall(Uh, "Uh")
+        _, _, ldv = _check_tall(Vh, "Vh")
+        Cm = torch.empty((J.numel(), n), dtype=torch.float64, device=Uh.device) if J is not None else None
+        Rt = torch.empty((I.numel(), n), dtype=torch.float64, device=Uh.device) if I is not None else None
+        self._check(self.lib.lrp_sample_fibers(self.h, n, r, _ptr(Uh), ldu, _ptr(S), _ptr(Vh), ldv,
+                                               _ptr(I), I.numel() if I is not None else 0,
+                                               _ptr(J), J.numel() if J is not None else 0,
+                                               _ptr(Cm), n, _ptr(Rt), n), "lrp_sample_fibers")
+        return Cm, Rt
+
+    def leverage_select(self, A, num_select: int, assume_orthonormal: bool = False):
+        torch = _torch()
+        k, n, lda = _check_tall(A, "A")
+        idx = torch.empty(max(num_select, 1), dtype=torch.int32, device=A.device)
+        scores = torch.empty(n, dtype=torch.float64, device=A.device)
+        self.ensure_workspace(self.lib.lrp_leverage_workspace_bytes(n, k))
+        self._check(self.lib.lrp_leverage_select(self.h, n, k, _ptr(A), lda, num_select, int(assume_orthonormal),
+                                                 _ptr(idx), _ptr(scores)), "lrp_leverage_select")
+        return idx[:num_select], scores
+
+    def scross(self, Cm, Rt, I, J):
+        torch = _torch()
+        k, n, ldc = _check_tall(Cm, "C")
+        l, _, ldr = _check_tall(Rt, "Rt")
+        p = min(k, l)
+        U = torch.empty((p, n), dtype=torch.float64, device=Cm.device)
+        V = torch.empty((p, n), dtype=torch.float64, device=Cm.device)
+        S = torch.empty(p, dtype=torch.float64, device=Cm.device)
+        rC = torch.empty(k, dtype=torch.float64, device=Cm.device)
+        rR = torch.empty(l, dtype=torch.float64, device=Cm.device)
+        rank = C.c_int32(0)
+        smin = C.c_double(0.0)
+        self.ensure_workspace(self.lib.lrp_scross_workspace_bytes(n, k, l))
+        self._check(self.lib.lrp_scross(self.h, n, _ptr(Cm), ldc, k, _ptr(Rt), ldr, l, _ptr(I), _ptr(J),
+                                        _ptr(U), n, _ptr(S), _ptr(V), n, _ptr(rC), _ptr(rR),
+                                        C.byref(rank), C.byref(smin)), "lrp_scross")
+        r = rank.value
+        return dict(U=U[:r], S=S[:r], V=V[:r], S_full=S, rC=rC, rR=rR, rank=r, smin_full=smin.value)
+
+    def cross_deim_solve(self, UF, SF, VF, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
+                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False):
+        """Low-rank Poisson solve.  UF, VF: tall tensors (rF, n) in physical space, SF: (rF,) CUDA tensor.
+        replay: list of dicts {I, J, keepI, keepJ} (numpy) + optional 'final_rank' on the last one."""
+        torch = _torch()
+        rF, n, ldu = _check_tall(UF, "UF")
+        _, _, ldv = _check_tall(VF, "VF")
+        dev = UF.device
+        Kc = max(2 * (max_rank + oversample), rF + oversample + 1)
+        self.ensure_workspace(self.lib.lrp_workspace_bytes(n, rF, max_rank, oversample))
+        UW = torch.zeros((max_rank, n), dtype=torch.float64, device=dev)
+        VW = torch.zeros((max_rank, n), dtype=torch.float64, device=dev)
+        SW = torch.zeros(max_rank, dtype=torch.float64, device=dev)
+        o = SolveOpts()
+        o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
+        keep = []
+        if safeguard is not None:
+            sg = np.ascontiguousarray(safeguard, dtype=np.int32); keep.append(sg)
+            o.h_safeguard, o.n_safeguard = sg.ctypes.data, sg.size
+        if U0 is not None:
+            r0, _, ld0 = _check_tall(U0, "U0")
+            o.d_U0, o.d_V0, o.ld0, o.r0 = U0.data_ptr(), V0.data_ptr(), ld0, r0
+        if replay is not None:
+            nI = np.array([len(s["I"]) for s in replay], dtype=np.int32)
+            nJ = np.array([len(s["J"]) for s in replay], dtype=np.int32)
+            Icat = np.ascontiguousarray(np.concatenate([np.asarray(s["I"], dtype=np.int32) for s in replay]))
+            Jcat = np.ascontiguousarray(np.concatenate([np.asarray(s["J"], dtype=np.int32) for s in replay]))
+            keep += [nI, nJ, Icat, Jcat]
+            o.replay_sweeps = len(replay)
+            o.h_replay_nI, o.h_replay_nJ, o.h_replay_I, o.h_replay_J = nI.ctypes.data, nJ.ctypes.data, Icat.ctypes.data, Jcat.ctypes.data
+            if replay[0].get("keepI") is not None:
+                kI = np.ascontiguousarray(np.concatenate([np.asarray(s["keepI"], dtype=np.uint8) for s in replay]))
+                kJ = np.ascontiguousarray(np.concatenate([np.asarray(s["keepJ"], dtype=np.uint8) for s in replay]))
+                keep += [kI, kJ]
+                o.h_replay_keepI, o.h_replay_keepJ = kI.ctypes.data, kJ.ctypes.data
+            o.replay_final_rank = int(replay[-1].get("final_rank") or 0)
+        info = SolveInfo()
+        trI = np.zeros(MAX_SWEEPS_INFO * Kc, dtype=np.int32); trJ = np.zeros_like(trI)
+        tkI = np.zeros(MAX_SWEEPS_INFO * Kc, dtype=np.uint8); tkJ = np.zeros_like(tkI)
+        Uhat = Vhat = Shat = None
+        if want_spectral:
+            Uhat = torch.zeros((Kc, n), dtype=torch.float64, device=dev)
+            Vhat = torch.zeros((Kc, n), dtype=torch.float64, device=dev)
+            Shat = torch.zeros(Kc, dtype=torch.float64, device=dev)
+        rc = self._check(self.lib.lrp_cross_deim_solve(
+            self.h, n, rF, _ptr(UF), ldu, _ptr(SF), _ptr(VF), ldv, C.byref(o), _ptr(UW), n, _ptr(SW), _ptr(VW), n,
+            C.byref(info), trI.ctypes.data, trJ.ctypes.data, tkI.ctypes.data, tkJ.ctypes.data,
+            _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_solve")
+        del keep
+        sweeps, r = info.sweeps, info.rank
+        trace, oi, oj = [], 0, 0
+        for s in range(sweeps):
+            a, b = info.nI[s], info.nJ[s]
+            trace.append(dict(I=trI[oi:oi + a].copy(), J=trJ[oj:oj + b].copy(),
+                              keepI=tkI[oi:oi + a].astype(bool), keepJ=tkJ[oj:oj + b].astype(bool),
+                              rank=info.rank_per_sweep[s], rho=info.rho_per_sweep[s], ind=info.ind_per_sweep[s]))
+            oi += a; oj += b
+        res = dict(UW=UW[:r], SW=SW[:r], VW=VW[:r], rank=r, sweeps=sweeps, converged=bool(info.converged),
+                   code=rc, trace=trace, info=info)
+        if want_spectral:
+            rk = info.rank_per_sweep[sweeps - 1]
+            res.update(Uhat=Uhat[:rk], Shat=Shat[:rk], Vhat=Vhat[:rk])
+        return res
+
+    def lowrank_entries(self, U, S, V, rows, cols):
+        torch = _torch()
+        r, n, ldu = _check_tall(U, "U")
+        _, _, ldv = _check_tall(V, "V")
+        out = torch.empty(rows.numel(), dtype=torch.float64, device=U.device)
+        self._check(self.lib.lrp_lowrank_entries(self.h, n, r, _ptr(U), ldu, _ptr(S), _ptr(V), ldv,
+                                                 _ptr(rows), _ptr(cols), rows.numel(), _ptr(out)), "lrp_lowrank_entries")
+        return out

@@ -1,0 +1,125 @@
+"""GPU parity of lrp_cross_deim_solve against the CPU oracle: free-running (discrete decisions compared)
+and under replay in both directions (continuous parity <= 1e-10 on reconstructed entries and selected fibers)."""
+import numpy as np
+import pytest
+
+from oracle import lrp_oracle as O
+from paper_2607_06021_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10          # north_star: relative error <= 1e-10 on reconstructed solution entries
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2607_06021_b200 import build, lrp
+    build.build()
+    c = lrp.Context(0)
+    yield c
+    c.close()
+
+
+def _gpu_solve(ctx, w, **kw):
+    import torch
+    from paper_2607_06021_b200 import lrp
+    return ctx.cross_deim_solve(lrp.tall_from_numpy(w.UF), torch.from_numpy(w.SF).cuda(), lrp.tall_from_numpy(w.VF),
+                                tol=w.tol, max_rank=w.max_rank, oversample=w.oversample, max_sweeps=w.max_sweeps,
+                                safeguard=w.safeguard, want_spectral=True, **kw)
+
+
+def _entries(U, S, V, rows, cols):
+    return np.einsum("tk,k,tk->t", U[rows], S, V[cols])
+
+
+def _continuous_parity(res, ref, w, replay_sets):
+    from paper_2607_06021_b200 import lrp
+    n = w.n
+    UW, VW, SW = lrp.tall_to_numpy(res["UW"]), lrp.tall_to_numpy(res["VW"]), res["SW"].cpu().numpy()
+    assert res["rank"] == ref.rank
+    rows, cols = W.sample_pairs(n, 4096, seed=1)
+    a = _entries(UW, SW, VW, rows, cols); b = _entries(ref.UW, ref.SW, ref.VW, rows, cols)
+    wmax = np.abs(ref.UW[:, 0]).max() * ref.SW[0] * np.abs(ref.VW[:, 0]).max()
+    assert np.abs(a - b).max() <= TOL * wmax
+    # all selected fibers of the spectral iterate
+    Uh, Vh, Sh = lrp.tall_to_numpy(res["Uhat"]), lrp.tall_to_numpy(res["Vhat"]), res["Shat"].cpu().numpy()
+    assert Uh.shape[1] == ref.Uhat.shape[1]
+    I, J = replay_sets
+    ghat = np.abs(ref.Uhat[:, 0]).max() * ref.Shat[0] * np.abs(ref.Vhat[:, 0]).max()
+    colsG = (Uh * Sh) @ Vh[J].T; colsR = (ref.Uhat * ref.Shat) @ ref.Vhat[J].T
+    rowsG = (Vh * Sh) @ Uh[I].T; rowsR = (ref.Vhat * ref.Shat) @ ref.Uhat[I].T
+    assert np.abs(colsG - colsR).max() <= TOL * ghat and np.abs(rowsG - rowsR).max() <= TOL * ghat
+    assert np.abs(Sh - ref.Shat).max() <= TOL * ref.Shat[0]
+
+
+CASES = [("C1", 0, None), ("C1", 3, None), ("C2", 0, None), ("C2", 1, None), ("C3", 0, None), ("C4", 0, (1 << 14) - 1)]
+
+
+@pytest.mark.parametrize("name,seed,n", CASES)
+def test_solve_free_run_and_replay(ctx, name, seed, n):
+    w = W.make(name, seed, n)
+    ref = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    res = _gpu_solve(ctx, w)
+    # ---- discrete parity of the free run: ordered selections equal where the deciding leverage gaps exceed 1e-12
+    same = res["sweeps"] == ref.sweeps
+    nchk = min(res["sweeps"], ref.sweeps)
+    clear = True
+    for s in range(nchk):
+        t = ref.trace[s]
+        for sc, star in ((t.scoresU, t.Istar), (t.scoresV, t.Jstar)):
+            srt = np.sort(sc)[::-1][:len(star) + 1]
+            clear &= bool(np.abs(np.diff(srt)).min() > 1e-12)
+        rr = t.rR / t.rR.max(); rc = t.rC / t.rC.max()
+        clear &= not (((rr > 1e-13) & (rr < 1e-11)).any() or ((rc > 1e-13) & (rc < 1e-11)).any())
+        if not clear:
+            break
+        g = res["trace"][s]
+        assert g["I"].tolist() == t.I.tolist() and g["J"].tolist() == t.J.tolist(), f"sweep {s}"
+        assert g["keepI"].tolist() == t.keepI.tolist() and g["keepJ"].tolist() == t.keepJ.tolist()
+        assert g["rank"] == t.rank
+    # sweep count may differ by one when rho / indicator sits within 10x of the threshold
+    assert abs(res["sweeps"] - ref.sweeps) <= 1
+    if clear and same:
+        assert res["converged"] == ref.converged
+        _continuous_parity(res, ref, w, (ref.trace[-1].I, ref.trace[-1].J))
+    # ---- replay oracle -> GPU
+    rep = O.trace_to_replay(ref.trace, ref.rank)
+    res2 = _gpu_solve(ctx, w, replay=rep)
+    assert res2["sweeps"] == ref.sweeps
+    _continuous_parity(res2, ref, w, (ref.trace[-1].I, ref.trace[-1].J))
+    # ---- replay GPU -> oracle
+    rep_g = [dict(I=t["I"], J=t["J"], keepI=t["keepI"], keepJ=t["keepJ"]) for t in res["trace"]]
+    rep_g[-1]["final_rank"] = res["rank"]
+    ref2 = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, replay=rep_g, **w.opts())
+    _continuous_parity(res, ref2, w, (res["trace"][-1]["I"], res["trace"][-1]["J"]))
+
+
+def test_c1_closed_form_on_gpu(ctx):
+    """sin(k pi x) sin(l pi y) forcing: exact solution f / (d_k + d_l), exact rank 4 (north_star pin, on the GPU path)."""
+    import math
+    from paper_2607_06021_b200 import lrp
+    w = W.config1(5)
+    res = _gpu_solve(ctx, w)
+    assert res["rank"] == 4 and res["converged"]
+    x = W.grid(w.n)
+    dk = lambda k: 4.0 * (w.n + 1) ** 2 * math.sin(math.pi * k / (2 * (w.n + 1))) ** 2
+    Wex = sum(w.meta["a"][m] * np.outer(np.sin(math.pi * w.meta["k"][m] * x), np.sin(math.pi * w.meta["l"][m] * x))
+              / (dk(int(w.meta["k"][m])) + dk(int(w.meta["l"][m]))) for m in range(4))
+    Wg = (lrp.tall_to_numpy(res["UW"]) * res["SW"].cpu().numpy()) @ lrp.tall_to_numpy(res["VW"]).T
+    assert np.abs(Wg - Wex).max() < 5e-12 * np.abs(Wex).max()
+
+
+def test_solve_argument_errors(ctx):
+    import torch
+    from paper_2607_06021_b200 import lrp
+    w = W.config1(0)
+    UF = lrp.tall_from_numpy(w.UF); VF = lrp.tall_from_numpy(w.VF); SF = torch.from_numpy(w.SF).cuda()
+    with pytest.raises(lrp.LrpError) as e:
+        ctx.cross_deim_solve(UF, SF, VF, tol=-1.0, max_rank=16)
+    assert e.value.code == lrp.LRP_ERR_BADARG
+    with pytest.raises(lrp.LrpError) as e:
+        ctx.cross_deim_solve(UF[:, :254].contiguous(), SF, VF[:, :254].contiguous(), tol=1e-10, max_rank=16)
+    assert e.value.code == lrp.LRP_ERR_UNSUPPORTED_N
+    # max_sweeps = 1 cannot pass the stop test -> warning code, outputs still valid
+    r = ctx.cross_deim_solve(UF, SF, VF, tol=1e-12, max_rank=16, max_sweeps=1, safeguard=w.safeguard)
+    assert r["code"] == lrp.LRP_WARN_NOCONV and r["rank"] >= 1
