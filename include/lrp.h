@@ -58,6 +58,16 @@ int lrp_last_cuda_error(const lrp_ctx* ctx);
 /* Number of kernel launches this ctx has enqueued since creation (bench.py's `gpu_launches`). */
 int64_t lrp_launch_count(const lrp_ctx* ctx);
 
+/* Per-kernel profile (used by bench.py's roofline): with profiling enabled every kernel launch is bracketed by CUDA
+ * events on the ctx's stream (adds a few microseconds per launch: never enabled inside a timed region).
+ * lrp_profile_get synchronises the stream and returns, for kernel class i < lrp_profile_count(): its name (static
+ * string), launch count, summed event time in ms (0 unless profiling was on), and the summed ALGORITHMIC bytes and
+ * flops of those launches.  lrp_profile_reset zeroes the counters. */
+int lrp_profile_enable(lrp_ctx* ctx, int on);
+int lrp_profile_reset(lrp_ctx* ctx);
+int lrp_profile_count(void);
+int lrp_profile_get(lrp_ctx* ctx, int i, const char** name, int64_t* count, double* ms, double* bytes, double* flops);
+
 /* Workspace sizes in bytes (host-side arithmetic only; safe to call without a GPU).
  *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample).
  *   lrp_dst1_workspace_bytes   : lrp_dst1_batched (0 for n <= 16383, the single-pass shared-memory regime).

@@ -186,13 +186,57 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     lrp_ctx* c = new (std::nothrow) lrp_ctx();
     if (!c) return LRP_ERR_BADARG;
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
+    c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
+    c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     *out = c;
     return LRP_OK;
 }
 
-int lrp_destroy(lrp_ctx* ctx) { delete ctx; return LRP_OK; }
+int lrp_destroy(lrp_ctx* ctx) {
+    if (!ctx) return LRP_OK;
+    if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
+    delete ctx->ev_id;
+    delete ctx;
+    return LRP_OK;
+}
+
+int lrp_profile_enable(lrp_ctx* ctx, int on) {
+    if (!ctx) return LRP_ERR_BADARG;
+    ctx->prof_on = on ? 1 : 0;
+    return LRP_OK;
+}
+
+static int profile_collect(lrp_ctx* ctx) {
+    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, (*ctx->ev)[i], (*ctx->ev)[i + 1]) == cudaSuccess) ctx->prof[(*ctx->ev_id)[i / 2]].ms += t;
+    }
+    ctx->ev_used = 0; ctx->ev_id->clear();
+    return LRP_OK;
+}
+
+int lrp_profile_reset(lrp_ctx* ctx) {
+    if (!ctx) return LRP_ERR_BADARG;
+    LRP_TRY(profile_collect(ctx));
+    memset(ctx->prof, 0, sizeof(ctx->prof));
+    return LRP_OK;
+}
+
+int lrp_profile_count(void) { return (int)K_NUM; }
+
+int lrp_profile_get(lrp_ctx* ctx, int i, const char** name, int64_t* count, double* ms, double* bytes, double* flops) {
+    if (!ctx || i < 0 || i >= (int)K_NUM) return LRP_ERR_BADARG;
+    LRP_TRY(profile_collect(ctx));
+    if (name) *name = LRP_KERNEL_NAMES[i];
+    if (count) *count = ctx->prof[i].count;
+    if (ms) *ms = ctx->prof[i].ms;
+    if (bytes) *bytes = ctx->prof[i].bytes;
+    if (flops) *flops = ctx->prof[i].flops;
+    return LRP_OK;
+}
 
 const char* lrp_strerror(int code) {
     switch (code) {

@@ -6,6 +6,23 @@
 #include <stddef.h>
 #include "../../include/lrp.h"
 
+#include <vector>
+
+// kernel classes for the per-kernel profile (lrp_profile_*): launch counts, CUDA-event time on the ctx's stream,
+// and the ALGORITHMIC bytes / flops of the launches (what the step must move / compute).
+enum LrpKernelId {
+    K_DST_SMALL, K_DST_NAIVE, K_DST_P1, K_DST_P2, K_DST_UNTANGLE, K_DST_CHUNKSUM, K_DST_SCANSUMS, K_DST_FINISH,
+    K_GEMM_SAMPLE, K_GEMM_PLAIN, K_GEMM_SUBTRACT, K_GEMM_T, K_REDUCE, K_ROWNORM, K_GATHER, K_COPY, K_ENTRIES,
+    K_PANEL_QR, K_PANEL_APPLY, K_ADD_BLOCK, K_CORE, K_ETA, K_RHO, K_COLMASK, K_TOPK_CHUNK, K_TOPK_MERGE, K_NUM
+};
+static const char* const LRP_KERNEL_NAMES[K_NUM] = {
+    "dst1_small", "dst1_naive", "dst1_p1", "dst1_p2", "dst1_untangle", "dst1_chunksum", "dst1_scansums", "dst1_finish",
+    "tall_gemm_sample", "tall_gemm_plain", "tall_gemm_subtract", "tall_gemm_t", "reduce_partials", "rownorm2", "gather_rows",
+    "copy_tall", "lowrank_entries", "panel_qr", "panel_apply", "add_block", "scross_core", "eta", "rho", "colmask",
+    "topk_chunk", "topk_merge"
+};
+struct lrp_prof { int64_t count; double ms, bytes, flops; };
+
 struct lrp_ctx {
     int device;
     cudaStream_t stream;
@@ -15,7 +32,34 @@ struct lrp_ctx {
     int64_t launches;
     int sm_count;
     int smem_optin;
+    int prof_on;
+    int prof_pending;                     // kernel id whose start event is recorded, -1 if none
+    lrp_prof prof[K_NUM];
+    std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)
+    std::vector<int>* ev_id;
+    size_t ev_used;
 };
+
+// call right before a kernel launch: accounts the launch and, when profiling is on, records its start event
+static inline void lrp_prof_begin(lrp_ctx* ctx, int id, double bytes, double flops) {
+    ctx->prof[id].count++; ctx->prof[id].bytes += bytes; ctx->prof[id].flops += flops;
+    if (!ctx->prof_on) return;
+    if (ctx->ev_used + 2 > ctx->ev->size()) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+        ctx->ev->push_back(a); ctx->ev->push_back(b);
+    }
+    cudaEventRecord((*ctx->ev)[ctx->ev_used], ctx->stream);
+    ctx->ev_id->push_back(id);
+    ctx->prof_pending = id;
+}
+static inline void lrp_prof_end(lrp_ctx* ctx) {
+    if (ctx->prof_pending < 0) return;
+    cudaEventRecord((*ctx->ev)[ctx->ev_used + 1], ctx->stream);
+    ctx->ev_used += 2;
+    ctx->prof_pending = -1;
+}
+#define LRP_PROF(ctx, id, bytes, flops) lrp_prof_begin((ctx), (id), (double)(bytes), (double)(flops))
 
 #define LRP_CUDA(ctx, call)                                                      \
     do {                                                                         \
@@ -27,6 +71,7 @@ struct lrp_ctx {
 #define LRP_LAUNCHED(ctx)                                                        \
     do {                                                                         \
         (ctx)->launches++;                                                       \
+        lrp_prof_end(ctx);                                                       \
         cudaError_t e_ = cudaGetLastError();                                     \
         if (e_ != cudaSuccess) { (ctx)->last_cuda = (int)e_; return LRP_ERR_CUDA; } \
     } while (0)

@@ -290,6 +290,7 @@ size_t core_work_doubles(int k, int l) {
 }
 
 int scross_core(lrp_ctx* ctx, const CoreArgs& a) {
+    LRP_PROF(ctx, K_CORE, 0, 0);
     scross_core_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -301,12 +302,14 @@ size_t eta_work_doubles(int nmax, int r) {
 }
 
 int eta_pair(lrp_ctx* ctx, const EtaArgs& a) {
+    LRP_PROF(ctx, K_ETA, 0, 0);
     eta_kernel<<<2, CORE_NT, 0, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
 
 int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
+    LRP_PROF(ctx, K_RHO, 0, 0);
     if (a.rp == 0) snorm_kernel<<<1, 32, 0, ctx->stream>>>(a.r, a.Sk, a.out);
     else rho_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
@@ -314,6 +317,7 @@ int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
 }
 
 int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double rcond, unsigned char* mask) {
+    LRP_PROF(ctx, K_COLMASK, 0, 0);
     colmask_kernel<<<1, 128, 0, ctx->stream>>>(k, R, ldr, rcond, mask);
     LRP_LAUNCHED(ctx);
     return LRP_OK;

@@ -519,6 +519,7 @@ int launch_small(lrp_ctx* ctx, int batch, const double* in, int64_t ld_in, doubl
     using C = SmallCfg<Q>;
     LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_small_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     int grid = (batch + C::CPB - 1) / C::CPB;
+    LRP_PROF(ctx, K_DST_SMALL, 16.0 * (2 * C::L - 1) * batch, 0);
     dst1_small_kernel<Q><<<grid, C::NT, C::SMEM, ctx->stream>>>(batch, in, ld_in, out, ld_out, scale);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -529,6 +530,7 @@ int launch_p1(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in
     LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_p1_kernel<Q1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     int L2 = 1 << (log2N - 1 - Q1);
     dim3 grid(L2 / C::T, cols);
+    LRP_PROF(ctx, K_DST_P1, 16.0 * ((int64_t)1 << log2N) * cols, 0);
     dst1_p1_kernel<Q1><<<grid, C::NT, C::SMEM, ctx->stream>>>(log2N, in, ld_in, W);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -539,6 +541,7 @@ int launch_p2(lrp_ctx* ctx, int log2N, int cols, const double2* W, double2* Z) {
     LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_p2_kernel<Q2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     int L1 = 1 << (log2N - 1 - Q2);
     dim3 grid(L1 / C::T, cols);
+    LRP_PROF(ctx, K_DST_P2, 16.0 * ((int64_t)1 << log2N) * cols, 0);
     dst1_p2_kernel<Q2><<<grid, C::NT, C::SMEM, ctx->stream>>>(log2N, W, Z);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -595,6 +598,7 @@ int lrp_dst1_impl(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, in
     if (batch == 0) return LRP_OK;
     const int64_t N = n + 1;
     if (N < 64) {
+        LRP_PROF(ctx, K_DST_NAIVE, 16.0 * n * batch, 0);
         dst1_naive_kernel<<<batch, 32, 0, ctx->stream>>>((int)n, d_in, ld_in, d_out, ld_out, scale);
         LRP_LAUNCHED(ctx);
         return LRP_OK;
@@ -619,13 +623,17 @@ int lrp_dst1_impl(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, in
         {
             int64_t work = L / 2 + 1;
             int bx = (int)((work + 255) / 256); if (bx > 4096) bx = 4096;
+            LRP_PROF(ctx, K_DST_UNTANGLE, 16.0 * N * cols, 0);
             dst1_untangle_kernel<<<dim3(bx, cols), 256, 0, ctx->stream>>>(log2N, Z, (double*)W, scale);
             LRP_LAUNCHED(ctx);
         }
+        LRP_PROF(ctx, K_DST_CHUNKSUM, 4.0 * N * cols, 0);
         dst1_chunksum_kernel<<<dim3(nchunks, cols), SCAN_NT, 0, ctx->stream>>>(log2N, (const double*)W, sums);
         LRP_LAUNCHED(ctx);
+        LRP_PROF(ctx, K_DST_SCANSUMS, 0, 0);
         dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(nchunks, sums);
         LRP_LAUNCHED(ctx);
+        LRP_PROF(ctx, K_DST_FINISH, 16.0 * N * cols, 0);
         dst1_finish_kernel<<<dim3(nchunks, cols), SCAN_NT, 0, ctx->stream>>>(log2N, (const double*)W, sums,
                                                                             d_out + (int64_t)c0 * ld_out, ld_out);
         LRP_LAUNCHED(ctx);

@@ -130,9 +130,11 @@ int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t*
     int G; int64_t chunk; sel_geometry(ctx, n, &G, &chunk);
     double* cand_s = (double*)ws;
     int32_t* cand_i = (int32_t*)((char*)ws + lrp_align_up((size_t)G * num * sizeof(double)));
+    LRP_PROF(ctx, K_TOPK_CHUNK, 8.0 * n, 0);
     topk_chunk_kernel<<<G, SEL_NT, 0, ctx->stream>>>(n, chunk, scores, num, cand_s, G == 1 ? idx_out : cand_i);
     LRP_LAUNCHED(ctx);
     if (G > 1) {
+        LRP_PROF(ctx, K_TOPK_MERGE, 0, 0);
         topk_merge_kernel<<<1, 1024, G * sizeof(int), ctx->stream>>>(G, num, cand_s, cand_i, idx_out);
         LRP_LAUNCHED(ctx);
     }

@@ -233,6 +233,8 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
         LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + GT_ROWS - 1) / GT_ROWS;
+    LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
+             8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
     tall_gemm_kernel<<<(unsigned)grid, GT_THREADS, smem, ctx->stream>>>(p);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -258,15 +260,18 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
     rows_per = (rows_per + TT_ROWS - 1) / TT_ROWS * TT_ROWS;
     nblk = (int)((n + rows_per - 1) / rows_per);
     dim3 grid(nblk, (k + TT_KA - 1) / TT_KA, (m + TT_MB - 1) / TT_MB);
+    LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
     tall_gemm_t_kernel<<<grid, TT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws);
     LRP_LAUNCHED(ctx);
     int tot = k * m;
+    LRP_PROF(ctx, K_REDUCE, 8.0 * nblk * k * m, 0);
     reduce_partials_kernel<<<(tot + 127) / 128, 128, 0, ctx->stream>>>(partial_ws, nblk, k, m, S, lds, accumulate);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
 
 int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, const unsigned char* colmask, double* out) {
+    LRP_PROF(ctx, K_ROWNORM, 8.0 * n * (k + 1), 2.0 * n * k);
     rownorm2_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(n, k, A, lda, colmask, out);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -275,6 +280,7 @@ int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, 
 int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const int32_t* idx, int nidx, double* Out, int ldo) {
     if (nidx <= 0 || k <= 0) return LRP_OK;
     int tot = nidx * k;
+    LRP_PROF(ctx, K_GATHER, 0, 0);
     gather_rows_kernel<<<(tot + 255) / 256, 256, 0, ctx->stream>>>(A, lda, k, idx, nidx, Out, ldo);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -283,6 +289,7 @@ int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const in
 int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb) {
     if (k <= 0) return LRP_OK;
     dim3 grid((unsigned)((n + 255) / 256), k < 64 ? k : 64);
+    LRP_PROF(ctx, K_COPY, 16.0 * n * k, 0);
     copy_tall_kernel<<<grid, 256, 0, ctx->stream>>>(n, k, A, lda, B, ldb);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -291,6 +298,7 @@ int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, doub
 int tall_lowrank_entries(lrp_ctx* ctx, int r, const double* U, int64_t ldu, const double* S, const double* V, int64_t ldv,
                          const int64_t* rows, const int64_t* cols, int64_t count, double* out) {
     if (count <= 0) return LRP_OK;
+    LRP_PROF(ctx, K_ENTRIES, 0, 0);
     lowrank_entries_kernel<<<(unsigned)((count + 255) / 256), 256, 0, ctx->stream>>>(r, U, ldu, S, V, ldv, rows, cols, count, out);
     LRP_LAUNCHED(ctx);
     return LRP_OK;

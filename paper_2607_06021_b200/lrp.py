@@ -24,7 +24,8 @@ MAX_SWEEPS_INFO = 32
 EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "lrp_launch_count",
            "lrp_workspace_bytes", "lrp_dst1_workspace_bytes", "lrp_leverage_workspace_bytes",
            "lrp_scross_workspace_bytes", "lrp_set_workspace", "lrp_dst1_batched", "lrp_sample_fibers",
-           "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries"]
+           "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
+           "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get"]
 
 
 class SolveOpts(C.Structure):
@@ -83,6 +84,12 @@ def load_library():
     lib.lrp_cross_deim_solve.restype = C.c_int
     lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_lowrank_entries.restype = C.c_int
+    lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
+    lib.lrp_profile_reset.argtypes = [vp]; lib.lrp_profile_reset.restype = C.c_int
+    lib.lrp_profile_count.argtypes = []; lib.lrp_profile_count.restype = C.c_int
+    lib.lrp_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(dbl),
+                                    C.POINTER(dbl), C.POINTER(dbl)]
+    lib.lrp_profile_get.restype = C.c_int
     _lib = lib
     return lib
 
@@ -118,9 +125,10 @@ def _ptr(t):
 
 def _check_tall(t, name):
     torch = _torch()
-    if not (t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and t.stride(1) == 1):
+    if not (t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and (t.stride(1) == 1 or t.shape[1] == 1)):
         raise ValueError(f"{name}: expected a CUDA float64 tensor of shape (cols, n) with contiguous rows")
-    return t.shape[0], t.shape[1], t.stride(0) if t.shape[0] > 1 else max(t.stride(0), t.shape[1])
+    ld = t.stride(0) if t.shape[0] > 1 else t.shape[1]
+    return t.shape[0], t.shape[1], max(ld, t.shape[1])
 
 
 class Context:
@@ -159,6 +167,24 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self.lib.lrp_launch_count(self.h))
+
+    def profile_enable(self, on: bool):
+        self._check(self.lib.lrp_profile_enable(self.h, int(on)), "lrp_profile_enable")
+
+    def profile_reset(self):
+        self._check(self.lib.lrp_profile_reset(self.h), "lrp_profile_reset")
+
+    def profile(self) -> dict:
+        """{kernel class: dict(count, ms, bytes, flops)} for the classes that launched since the last reset."""
+        out = {}
+        for i in range(self.lib.lrp_profile_count()):
+            name, cnt = C.c_char_p(), C.c_int64()
+            ms, by, fl = C.c_double(), C.c_double(), C.c_double()
+            self._check(self.lib.lrp_profile_get(self.h, i, C.byref(name), C.byref(cnt), C.byref(ms), C.byref(by),
+                                                 C.byref(fl)), "lrp_profile_get")
+            if cnt.value:
+                out[name.value.decode()] = dict(count=cnt.value, ms=ms.value, bytes=by.value, flops=fl.value)
+        return out
 
     def ensure_workspace(self, nbytes: int):
         torch = _torch()

@@ -1,0 +1,51 @@
+"""Multi-GPU plumbing for bench.py: the path does not shard (replicas only), so N ranks
+run N independent solves (one process per GPU, different seeds) with no collective on the data path.  The only
+communication is the timing protocol: barrier, max-over-ranks of the device time, sum of the units processed.
+Works with any torch.distributed backend (nccl on GPUs; gloo in the CPU tests)."""
+from __future__ import annotations
+
+import os
+
+
+def env_world():
+    """(rank, local_rank, world_size) from the torchrun environment (1-process defaults)."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+def init(backend: str, device=None):
+    """Initialise torch.distributed from MASTER_ADDR/MASTER_PORT if WORLD_SIZE > 1; returns the module or None."""
+    rank, _, world = env_world()
+    if world <= 1:
+        return None
+    import torch.distributed as dist
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29500")
+        kw = {}
+        if device is not None and backend == "nccl":
+            kw["device_id"] = device
+        dist.init_process_group(backend=backend, rank=rank, world_size=world, **kw)
+    return dist
+
+
+def barrier(dist):
+    if dist is not None:
+        dist.barrier()
+
+
+def aggregate(dist, local_ms: float, local_units: float, device="cpu"):
+    """Whole-job numbers: (max over ranks of the elapsed ms, sum over ranks of the units processed)."""
+    if dist is None:
+        return float(local_ms), float(local_units)
+    import torch
+    t = torch.tensor([float(local_ms)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(local_units)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def throughput(dist, local_ms: float, local_units: float, device="cpu") -> dict:
+    ms, units = aggregate(dist, local_ms, local_units, device)
+    return dict(ms=ms, units=units, per_s=units / (ms * 1e-3) if ms > 0 else 0.0)

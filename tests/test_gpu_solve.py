@@ -32,22 +32,32 @@ def _entries(U, S, V, rows, cols):
     return np.einsum("tk,k,tk->t", U[rows], S, V[cols])
 
 
+def _parity_tol(ref):
+    """1e-10 when the stop test passed.  A run that the sweep cap ends first (C3 as configured: 5 sweeps) still has
+    a residual of size rho, part of which is fitted by the QR's rounding-level directions: two fp64 implementations
+    then differ by O(0.1 rho / ||S||) -- DESIGN.md "Parity tolerance", pinned on the oracle itself in
+    tests/test_oracle_solve.py::test_unconverged_run_sensitivity."""
+    t = ref.trace[-1]
+    return TOL if ref.converged else max(TOL, 0.1 * max(t.rho, t.ind) / t.snorm)
+
+
 def _continuous_parity(res, ref, w, replay_sets):
     from paper_2607_06021_b200 import lrp
     n = w.n
+    TOL = _parity_tol(ref)
     UW, VW, SW = lrp.tall_to_numpy(res["UW"]), lrp.tall_to_numpy(res["VW"]), res["SW"].cpu().numpy()
     assert res["rank"] == ref.rank
     rows, cols = W.sample_pairs(n, 4096, seed=1)
     a = _entries(UW, SW, VW, rows, cols); b = _entries(ref.UW, ref.SW, ref.VW, rows, cols)
-    wmax = np.abs(ref.UW[:, 0]).max() * ref.SW[0] * np.abs(ref.VW[:, 0]).max()
-    assert np.abs(a - b).max() <= TOL * wmax
+    wmax = np.abs(b).max()                                   # max |W| over the 4096 samples of the smooth solution
+    assert np.abs(a - b).max() <= TOL * wmax, (np.abs(a - b).max() / wmax, TOL)
     # all selected fibers of the spectral iterate
     Uh, Vh, Sh = lrp.tall_to_numpy(res["Uhat"]), lrp.tall_to_numpy(res["Vhat"]), res["Shat"].cpu().numpy()
     assert Uh.shape[1] == ref.Uhat.shape[1]
     I, J = replay_sets
-    ghat = np.abs(ref.Uhat[:, 0]).max() * ref.Shat[0] * np.abs(ref.Vhat[:, 0]).max()
     colsG = (Uh * Sh) @ Vh[J].T; colsR = (ref.Uhat * ref.Shat) @ ref.Vhat[J].T
     rowsG = (Vh * Sh) @ Uh[I].T; rowsR = (ref.Vhat * ref.Shat) @ ref.Uhat[I].T
+    ghat = max(np.abs(colsR).max(), np.abs(rowsR).max())      # max |What| (the selected fibers carry it)
     assert np.abs(colsG - colsR).max() <= TOL * ghat and np.abs(rowsG - rowsR).max() <= TOL * ghat
     assert np.abs(Sh - ref.Shat).max() <= TOL * ref.Shat[0]
 
