@@ -35,16 +35,16 @@ def _entries(U, S, V, rows, cols):
 def _parity_tol(ref):
     """1e-10 when the stop test passed.  A run that the sweep cap ends first (C3 as configured: 5 sweeps) still has
     a residual of size rho, part of which is fitted by the QR's rounding-level directions: two fp64 implementations
-    then differ by O(0.1 rho / ||S||) -- DESIGN.md "Parity tolerance", pinned on the oracle itself in
-    tests/test_oracle_solve.py::test_unconverged_run_sensitivity."""
+    are then only defined up to O(rho / ||S||) -- DESIGN.md "Parity tolerance", shown on the oracle itself (Householder
+    vs LAPACK QR under replay) in tests/test_oracle_solve.py::test_unconverged_run_sensitivity."""
     t = ref.trace[-1]
-    return TOL if ref.converged else max(TOL, 0.1 * max(t.rho, t.ind) / t.snorm)
+    return TOL if ref.converged else max(TOL, 2.0 * max(t.rho, t.ind) / t.snorm)
 
 
-def _continuous_parity(res, ref, w, replay_sets):
+def _continuous_parity(res, ref, w, replay_sets, tol=None):
     from paper_2607_06021_b200 import lrp
     n = w.n
-    TOL = _parity_tol(ref)
+    TOL = tol if tol is not None else _parity_tol(ref)
     UW, VW, SW = lrp.tall_to_numpy(res["UW"]), lrp.tall_to_numpy(res["VW"]), res["SW"].cpu().numpy()
     assert res["rank"] == ref.rank
     rows, cols = W.sample_pairs(n, 4096, seed=1)
@@ -62,12 +62,17 @@ def _continuous_parity(res, ref, w, replay_sets):
     assert np.abs(Sh - ref.Shat).max() <= TOL * ref.Shat[0]
 
 
-CASES = [("C1", 0, None), ("C1", 3, None), ("C2", 0, None), ("C2", 1, None), ("C3", 0, None), ("C4", 0, (1 << 14) - 1)]
+# (config, seed, n override, max_sweeps override).  C3 is run as configured (5 sweeps: the cap ends it unconverged) and
+# with the default cap (converges: the 1e-10 bar applies).
+CASES = [("C1", 0, None, None), ("C1", 3, None, None), ("C2", 0, None, None), ("C2", 1, None, None),
+         ("C3", 0, None, None), ("C3", 0, None, 20), ("C4", 0, (1 << 14) - 1, None)]
 
 
-@pytest.mark.parametrize("name,seed,n", CASES)
-def test_solve_free_run_and_replay(ctx, name, seed, n):
+@pytest.mark.parametrize("name,seed,n,sweeps", CASES)
+def test_solve_free_run_and_replay(ctx, name, seed, n, sweeps):
     w = W.make(name, seed, n)
+    if sweeps:
+        w.max_sweeps = sweeps
     ref = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
     res = _gpu_solve(ctx, w)
     # ---- discrete parity of the free run: ordered selections equal where the deciding leverage gaps exceed 1e-12
@@ -101,7 +106,7 @@ def test_solve_free_run_and_replay(ctx, name, seed, n):
     rep_g = [dict(I=t["I"], J=t["J"], keepI=t["keepI"], keepJ=t["keepJ"]) for t in res["trace"]]
     rep_g[-1]["final_rank"] = res["rank"]
     ref2 = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, replay=rep_g, **w.opts())
-    _continuous_parity(res, ref2, w, (res["trace"][-1]["I"], res["trace"][-1]["J"]))
+    _continuous_parity(res, ref2, w, (res["trace"][-1]["I"], res["trace"][-1]["J"]), tol=_parity_tol(ref))
 
 
 def test_c1_closed_form_on_gpu(ctx):
