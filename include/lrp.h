@@ -25,7 +25,7 @@
  *     only where stated.
  *   - return value: 0 = LRP_OK, negative = error, positive = warning (outputs valid).
  *     No exceptions, no globals, no CPU fallback: without a CUDA device every compute call fails.
- *   - n + 1 must be a power of two, 2 <= n + 1 <= 2^27 (general n: DESIGN.md "next").
+ *   - n + 1 must be a power of two, 2 <= n + 1 <= 2^25 (general n: DESIGN.md "next").
  */
 #ifndef LRP_H_
 #define LRP_H_

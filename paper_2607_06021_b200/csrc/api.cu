@@ -22,7 +22,7 @@ bool aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
 int check_n(int64_t n) {
     if (n < 1) return LRP_ERR_UNSUPPORTED_N;
     int64_t N = n + 1;
-    if (!lrp_is_pow2(N) || N > ((int64_t)1 << 27)) return LRP_ERR_UNSUPPORTED_N;
+    if (!lrp_is_pow2(N) || N > ((int64_t)1 << 25)) return LRP_ERR_UNSUPPORTED_N;
     return LRP_OK;
 }
 
@@ -242,7 +242,7 @@ const char* lrp_strerror(int code) {
     switch (code) {
         case LRP_OK: return "ok";
         case LRP_ERR_BADARG: return "bad argument";
-        case LRP_ERR_UNSUPPORTED_N: return "n + 1 must be a power of two in [2, 2^27]";
+        case LRP_ERR_UNSUPPORTED_N: return "n + 1 must be a power of two in [2, 2^25]";
         case LRP_ERR_WORKSPACE: return "workspace missing or too small";
         case LRP_ERR_CUDA: return "CUDA error (see lrp_last_cuda_error)";
         case LRP_WARN_NOCONV: return "warning: stop test not passed within max_sweeps";

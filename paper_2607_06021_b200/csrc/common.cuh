@@ -100,3 +100,7 @@ struct lrp_arena {
 int lrp_dst1_impl(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, int64_t ld_in,
                   double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes);
 size_t lrp_dst1_ws_impl(int64_t n, int32_t batch);
+// four-step regime (dst1_large.cu), N = n + 1 > 16384
+size_t dst1_large_ws(int64_t N, int32_t batch);
+int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
+               double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes);
