@@ -24,30 +24,27 @@ __device__ __forceinline__ double eig_d(int64_t i, double invN, double fourN2) {
     return fourN2 * s * s;
 }
 
-constexpr int MG_THREADS = 128, MG_CT = 32;          // 4 warps x 32 rows; 32-column tiles
+constexpr int MG_THREADS = 128;                      // 4 warps x 32 rows; column tiles of 8*NJ (NJ = 2 for m <= 16: fewer
+                                                     // accumulator registers -> more CTAs per SM for the memory-bound shapes)
 
 __host__ __device__ inline int mg_kp(int k) {         // padded k: multiple of 4 rounded up to (kp % 16 == 4)
     int k4 = (k + 3) & ~3;
     return k4 + (((4 - k4 % 16) + 16) % 16);
 }
 
+template <int NJ>
 __global__ void __launch_bounds__(MG_THREADS)
 tall_gemm_mma_kernel(TallGemmArgs p) {
+    constexpr int MG_CT = 8 * NJ;
     extern __shared__ __align__(16) double smem[];
     const int kp = mg_kp(p.k), k4 = (p.k + 3) & ~3;
     double* Bs = smem;                                // [MG_CT][kp]: Bs[c*kp + t] = B(t, c0 + c)
     double* dcol = smem + (size_t)MG_CT * kp;         // [MG_CT]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, tg = lane & 3;
-    const int64_t R0 = (int64_t)blockIdx.x * (MG_THREADS) + warp * 32;
     const double invN = 1.0 / (double)(p.n + 1);
     const double fourN2 = 4.0 * (double)(p.n + 1) * (double)(p.n + 1);
-    int64_t rows[4]; bool valid[4]; double drow[4], nrm[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        rows[i] = R0 + 8 * i + g; valid[i] = rows[i] < p.n;
-        drow[i] = (p.mode == TG_SAMPLE && valid[i]) ? eig_d(rows[i], invN, fourN2) : 0.0;
-        nrm[i] = 0.0;
-    }
+    const int64_t nslab = (p.n + MG_THREADS - 1) / MG_THREADS;
+    const bool single_tile = p.m <= MG_CT;             // B staged once, the CTA then streams its row slabs
     for (int c0 = 0; c0 < p.m; c0 += MG_CT) {
         __syncthreads();
         for (int e = tid; e < MG_CT * k4; e += MG_THREADS) {
@@ -62,29 +59,38 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
         if (p.mode == TG_SAMPLE)
             for (int c = tid; c < MG_CT; c += MG_THREADS) dcol[c] = (c0 + c < p.m) ? eig_d(p.idx[c0 + c], invN, fourN2) : 1.0;
         __syncthreads();
-        double acc[4][4][2];
+      for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
+        const int64_t R0 = slab * MG_THREADS + warp * 32;
+        int64_t rows[4]; bool valid[4]; double drow[4], nrm[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            rows[i] = R0 + 8 * i + g; valid[i] = rows[i] < p.n;
+            drow[i] = (p.mode == TG_SAMPLE && valid[i]) ? eig_d(rows[i], invN, fourN2) : 0.0;
+            nrm[i] = 0.0;
+        }
+        double acc[4][NJ][2];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
-#pragma unroll 2
+            for (int j = 0; j < NJ; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+#pragma unroll 4
         for (int t0 = 0; t0 < k4; t0 += 4) {
             const int t = t0 + tg;
-            double a[4], b[4];
+            double a[4], b[NJ];
 #pragma unroll
             for (int i = 0; i < 4; ++i) a[i] = (valid[i] && t < p.k) ? p.A[rows[i] + (int64_t)t * p.lda] : 0.0;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = Bs[(8 * j + g) * kp + t];
+            for (int j = 0; j < NJ; ++j) b[j] = Bs[(8 * j + g) * kp + t];
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                for (int j = 0; j < NJ; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             if (!valid[i]) continue;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+            for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int cl = 8 * j + 2 * tg + e, col = c0 + cl;
@@ -97,53 +103,72 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
                     }
                 }
         }
-    }
-    if (p.rownorm2) {
+        if (p.rownorm2) {                              // row norms accumulate over the column tiles
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            double s = nrm[i];
-            s += __shfl_xor_sync(0xffffffffu, s, 1);
-            s += __shfl_xor_sync(0xffffffffu, s, 2);
-            if (tg == 0 && valid[i]) p.rownorm2[rows[i]] = s;
+            for (int i = 0; i < 4; ++i) {
+                double s = nrm[i];
+                s += __shfl_xor_sync(0xffffffffu, s, 1);
+                s += __shfl_xor_sync(0xffffffffu, s, 2);
+                if (tg == 0 && valid[i]) p.rownorm2[rows[i]] = (c0 == 0 ? 0.0 : p.rownorm2[rows[i]]) + s;
+            }
         }
+      }
     }
+    (void)single_tile;
 }
 
-// ---- S = A^T B: every warp owns one 16 x 16 tile of S over the CTA's row slab -------------------------------
+// ---- S = A^T B: 8 warps per CTA; the CTA owns ntc <= 8 tiles (16 x 16) of S and its row slab; the 8/ntc warps
+//      that share a tile split the slab's rows and are summed through shared memory in a fixed order -------------
 constexpr int MT_THREADS = 256;
 
 __global__ void __launch_bounds__(MT_THREADS)
 tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const double* __restrict__ B, int64_t ldb, int m,
-                       int64_t n, int64_t rows_per_cta, double* __restrict__ partial, int na, int nb) {
+                       int64_t n, int64_t rows_per_cta, double* __restrict__ partial, int na, int nb, int ntc) {
+    __shared__ double red[MT_THREADS / 32][8][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, tg = lane & 3;
-    const int tile = blockIdx.y * (MT_THREADS / 32) + warp;
-    if (tile >= na * nb) return;
+    const int nsub = (MT_THREADS / 32) / ntc;               // warps per tile
+    const int tl = warp % ntc, sub = warp / ntc;
+    const int tile = blockIdx.y * ntc + tl;
+    const bool active = tile < na * nb && sub < nsub;
     const int a0 = 16 * (tile % na), b0 = 16 * (tile / na);
-    const int64_t r_begin = (int64_t)blockIdx.x * rows_per_cta;
-    int64_t r_end = r_begin + rows_per_cta; if (r_end > n) r_end = n;
-    const int ca0 = a0 + g, ca1 = a0 + 8 + g, cb0 = b0 + g, cb1 = b0 + 8 + g;
-    const double* pa0 = A + (int64_t)(ca0 < k ? ca0 : 0) * lda; const double* pa1 = A + (int64_t)(ca1 < k ? ca1 : 0) * lda;
-    const double* pb0 = B + (int64_t)(cb0 < m ? cb0 : 0) * ldb; const double* pb1 = B + (int64_t)(cb1 < m ? cb1 : 0) * ldb;
+    const int64_t c_begin = (int64_t)blockIdx.x * rows_per_cta;
+    int64_t c_end = c_begin + rows_per_cta; if (c_end > n) c_end = n;
     double acc[2][2][2] = {};
-    int64_t rb = r_begin;                             // warp-uniform row base (mma.sync needs the whole warp)
-    for (; rb + 16 <= r_end; rb += 16) {              // 4 k-steps in flight
-        const int64_t r = rb + tg;
-        double x0[4], x1[4], y0[4], y1[4];
+    if (active) {
+        const int ca0 = a0 + g, ca1 = a0 + 8 + g, cb0 = b0 + g, cb1 = b0 + 8 + g;
+        const double* pa0 = A + (int64_t)(ca0 < k ? ca0 : 0) * lda; const double* pa1 = A + (int64_t)(ca1 < k ? ca1 : 0) * lda;
+        const double* pb0 = B + (int64_t)(cb0 < m ? cb0 : 0) * ldb; const double* pb1 = B + (int64_t)(cb1 < m ? cb1 : 0) * ldb;
+        // the warps sharing a tile take interleaved 16-row chunks, so that at any time the CTA streams one contiguous
+        // 16*nsub-row run of every column (DRAM row-buffer locality; blocked sub-slabs measured 28 % of HBM peak)
+        for (int64_t rb = c_begin + 16 * sub; rb < c_end; rb += 16 * nsub) {   // warp-uniform (mma.sync needs the whole warp)
+            const int64_t r = rb + tg;
+            double x0[4], x1[4], y0[4], y1[4];
+            if (rb + 16 <= c_end) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { x0[u] = pa0[r + 4 * u]; x1[u] = pa1[r + 4 * u]; y0[u] = pb0[r + 4 * u]; y1[u] = pb1[r + 4 * u]; }
+                for (int u = 0; u < 4; ++u) { x0[u] = pa0[r + 4 * u]; x1[u] = pa1[r + 4 * u]; y0[u] = pb0[r + 4 * u]; y1[u] = pb1[r + 4 * u]; }
+            } else {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            dmma(acc[0][0][0], acc[0][0][1], x0[u], y0[u]); dmma(acc[0][1][0], acc[0][1][1], x0[u], y1[u]);
-            dmma(acc[1][0][0], acc[1][0][1], x1[u], y0[u]); dmma(acc[1][1][0], acc[1][1][1], x1[u], y1[u]);
+                for (int u = 0; u < 4; ++u) {
+                    const bool rv = r + 4 * u < c_end;
+                    x0[u] = rv ? pa0[r + 4 * u] : 0.0; x1[u] = rv ? pa1[r + 4 * u] : 0.0;
+                    y0[u] = rv ? pb0[r + 4 * u] : 0.0; y1[u] = rv ? pb1[r + 4 * u] : 0.0;
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                dmma(acc[0][0][0], acc[0][0][1], x0[u], y0[u]); dmma(acc[0][1][0], acc[0][1][1], x0[u], y1[u]);
+                dmma(acc[1][0][0], acc[1][0][1], x1[u], y0[u]); dmma(acc[1][1][0], acc[1][1][1], x1[u], y1[u]);
+            }
         }
     }
-    for (; rb < r_end; rb += 4) {                     // ragged tail
-        const int64_t r = rb + tg;
-        const bool rv = r < r_end;
-        double x0 = rv ? pa0[r] : 0.0, x1 = rv ? pa1[r] : 0.0, y0 = rv ? pb0[r] : 0.0, y1 = rv ? pb1[r] : 0.0;
-        dmma(acc[0][0][0], acc[0][0][1], x0, y0); dmma(acc[0][1][0], acc[0][1][1], x0, y1);
-        dmma(acc[1][0][0], acc[1][0][1], x1, y0); dmma(acc[1][1][0], acc[1][1][1], x1, y1);
-    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 2; ++j)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) red[warp][(i * 2 + j) * 2 + e][lane] = acc[i][j][e];
+    __syncthreads();
+    if (sub != 0 || tile >= na * nb) return;
     double* P = partial + (int64_t)blockIdx.x * k * m;
 #pragma unroll
     for (int i = 0; i < 2; ++i)
@@ -151,18 +176,25 @@ tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const d
         for (int j = 0; j < 2; ++j)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
+                double v = 0.0;
+                for (int s2 = 0; s2 < nsub; ++s2) v += red[tl + s2 * ntc][(i * 2 + j) * 2 + e][lane];
                 int a = a0 + 8 * i + g, b = b0 + 8 * j + 2 * tg + e;
-                if (a < k && b < m) P[a + (int64_t)b * k] = acc[i][j][e];
+                if (a < k && b < m) P[a + (int64_t)b * k] = v;
             }
 }
 
 // S(a,b) = sum_blk partial[blk](a,b) (+ S(a,b) if accumulate), fixed summation order (deterministic)
 __global__ void reduce_partials_kernel(const double* __restrict__ partial, int nblk, int k, int m,
                                        double* __restrict__ S, int64_t lds, int accumulate) {
-    int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= k * m) return;
+    const int part = threadIdx.x & 7;                       // 8 lanes per output element, fixed order -> deterministic
+    const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
+    const bool ok = e < k * m;
     double s = 0.0;
-    for (int b = 0; b < nblk; ++b) s += partial[(int64_t)b * k * m + e];
+    if (ok) for (int b = part; b < nblk; b += 8) s += partial[(int64_t)b * k * m + e];
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    s += __shfl_xor_sync(0xffffffffu, s, 4);
+    if (!ok || part != 0) return;
     int a = e % k, c = e / k;
     double* o = S + a + (int64_t)c * lds;
     *o = accumulate ? (*o + s) : s;
@@ -172,46 +204,56 @@ __global__ void reduce_partials_kernel(const double* __restrict__ partial, int n
 
 int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
     if (p.n <= 0 || p.m <= 0) return LRP_OK;
-    size_t smem = sizeof(double) * ((size_t)MG_CT * mg_kp(p.k > 0 ? p.k : 1) + MG_CT);
+    const int nj = p.m <= 16 ? 2 : 4;
+    size_t smem = sizeof(double) * ((size_t)(8 * nj) * mg_kp(p.k > 0 ? p.k : 1) + 8 * nj);
     if (smem > 48 * 1024) {
         if (smem > (size_t)ctx->smem_optin) return LRP_ERR_BADARG;
-        LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_mma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
+    if (grid > 148 * 8) grid = 148 * 8;            // persistent over row slabs: B is staged once per column tile per CTA
     LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
              8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
-    tall_gemm_mma_kernel<<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
+    if (nj == 2) tall_gemm_mma_kernel<2><<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
+    else tall_gemm_mma_kernel<4><<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
 
-static int tall_gemm_t_nblk(int64_t n) {
-    int64_t want = 148 * 4;                    // B200: 148 SMs; fixed so that workspace sizes need no device query
-    int64_t by_rows = (n + 255) / 256;
+static int tall_gemm_t_ntc(int k, int m) {       // tiles per CTA: 1, 2, 4 or 8 (the 8 warps split rows when fewer)
+    int nt = ((k + 15) / 16) * ((m + 15) / 16);
+    return nt >= 8 ? 8 : (nt >= 4 ? 4 : (nt >= 2 ? 2 : 1));
+}
+static int tall_gemm_t_nblk(int64_t n, int k, int m) {
+    (void)k; (void)m;
+    int64_t want = 148 * 4;                            // B200: 148 SMs; fixed so that workspace sizes need no device query
+    int64_t by_rows = (n + 511) / 512;
     int64_t nb = want < by_rows ? want : by_rows;
     return (int)(nb < 1 ? 1 : nb);
 }
 
 size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m) {
     (void)ctx;
-    return (size_t)tall_gemm_t_nblk(n) * k * m;
+    return (size_t)tall_gemm_t_nblk(n, k, m) * k * m;
 }
 
 int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
                 double* S, int64_t lds, int accumulate, double* partial_ws) {
     if (k <= 0 || m <= 0) return LRP_OK;
-    int nblk = tall_gemm_t_nblk(n);
+    int nblk = tall_gemm_t_nblk(n, k, m);
+    const int ntc = tall_gemm_t_ntc(k, m);
     int64_t rows_per = (n + nblk - 1) / nblk;
     rows_per = (rows_per + 15) / 16 * 16;
     nblk = (int)((n + rows_per - 1) / rows_per);
     const int na = (k + 15) / 16, nb = (m + 15) / 16;
-    dim3 grid(nblk, (na * nb + MT_THREADS / 32 - 1) / (MT_THREADS / 32));
+    dim3 grid(nblk, (na * nb + ntc - 1) / ntc);
     LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
-    tall_gemm_t_mma_kernel<<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb);
+    tall_gemm_t_mma_kernel<<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
     LRP_LAUNCHED(ctx);
     int tot = k * m;
     LRP_PROF(ctx, K_REDUCE, 8.0 * nblk * k * m, 0);
-    reduce_partials_kernel<<<(tot + 127) / 128, 128, 0, ctx->stream>>>(partial_ws, nblk, k, m, S, lds, accumulate);
+    reduce_partials_kernel<<<(tot * 8 + 127) / 128, 128, 0, ctx->stream>>>(partial_ws, nblk, k, m, S, lds, accumulate);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
