@@ -19,6 +19,10 @@ constexpr double PINV_RCOND = 1e-13, RANK_RCOND = 1e-14, LEV_COL_RCOND = 1e-13, 
 
 bool aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
 
+// leading dimension of the library's own tall buffers: even (16-byte aligned columns -> 128-bit loads) and not a
+// multiple of a large power of two (n + 1 is one: columns would alias in the memory-channel hash)
+int64_t internal_ld(int64_t n) { return n + 74 + (n & 1); }
+
 int check_n(int64_t n) {
     if (n < 1) return LRP_ERR_UNSUPPORTED_N;
     int64_t N = n + 1;
@@ -115,7 +119,7 @@ struct SolveWs {
     size_t eta_stride, dst_ws_bytes;
     ScrossWs sc;
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank) {
-        const size_t ld = (size_t)n;
+        const size_t ld = (size_t)internal_ld(n);
         UhF = ar.take<double>(ld * rF); VhF = ar.take<double>(ld * rF);
         Cb = ar.take<double>(ld * Kc); Rb = ar.take<double>(ld * Kc);
         Ua = ar.take<double>(ld * Kc); Va = ar.take<double>(ld * Kc);
@@ -409,7 +413,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     if (!w.carve(ar, ctx, n, rF, Kc, max_rank)) return LRP_ERR_WORKSPACE;
     memset(info, 0, sizeof(*info));
     const int64_t launches0 = ctx->launches;
-    const int64_t ld = n;
+    const int64_t ld = internal_ld(n);
     const double scale = sqrt(2.0 / (double)(n + 1));
     EventPool ep;
     cudaEvent_t e_start = ep.rec(ctx);

@@ -70,13 +70,16 @@ __device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv,
 // Thin SVD of M (m x n, ld ldm): U (m x p), s (p, descending), V (n x p), p = min(m, n).
 // work: max(m,n)*p + p*p + p doubles, iwork: p ints.  Columns of U for exactly-zero singular values are zero.
 __device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int ldu, double* s, double* V, int ldv,
-                        double* work, int* iwork, int* s_flag) {
+                        double* work, int* iwork, int* s_flag, double* sm = nullptr, int sm_doubles = 0) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const bool tr = m < n;
     const int T = tr ? n : m, p = tr ? m : n;
-    double* A = work;               // T x p
-    double* W = A + (size_t)T * p;  // p x p
-    double* sv = W + (size_t)p * p; // p
+    // the Jacobi working set (T x p columns + p x p rotations) lives in shared memory when it fits: every round of
+    // the sweep is a dependent read-modify-write of two columns per warp, i.e. pure latency
+    const bool in_smem = sm != nullptr && (size_t)T * p + (size_t)p * p <= (size_t)sm_doubles;
+    double* A = in_smem ? sm : work;                 // T x p
+    double* W = A + (size_t)T * p;                   // p x p
+    double* sv = work + (size_t)T * p + (size_t)p * p; // p
     for (int e = tid; e < T * p; e += nt) {
         int t = e % T, c = e / T;
         A[e] = tr ? M[c + (size_t)t * ldm] : M[t + (size_t)c * ldm];
@@ -153,7 +156,8 @@ scross_core_kernel(CoreArgs a) {
     for (int c = tid; c < k; c += nt) a.rC[c] = fabs(a.RC[c + (size_t)c * a.ldrc]);
     for (int c = tid; c < l; c += nt) a.rR[c] = fabs(a.RR[c + (size_t)c * a.ldrr]);
     __syncthreads();
-    cta_svd(X, xm, xm, xn, Ux, xm, sx, Vx, xn, svdw, a.iwork, &s_flag);
+    extern __shared__ __align__(16) double dyn_smem[];
+    cta_svd(X, xm, xm, xn, Ux, xm, sx, Vx, xn, svdw, a.iwork, &s_flag, dyn_smem, a.smem_doubles);
     // P = Vx diag(1/sx) Ux^T over the kept singular values (relative cut, reading Q4)
     {
         const double cut = a.pinv_rcond * sx[0];
@@ -176,7 +180,7 @@ scross_core_kernel(CoreArgs a) {
         cta_matmul(Mc, k, k, l, k, a.RC, 1, (int)a.ldrc, P, l, 1);
     }
     const int p = k < l ? k : l;
-    cta_svd(Mc, k, k, l, a.Uc, k, a.S, a.Vc, l, svdw, a.iwork, &s_flag);
+    cta_svd(Mc, k, k, l, a.Uc, k, a.S, a.Vc, l, svdw, a.iwork, &s_flag, dyn_smem, a.smem_doubles);
     if (tid == 0) {
         double s1 = a.S[0];
         int rank = 0;
@@ -211,7 +215,8 @@ eta_kernel(EtaArgs a) {
         X[e] = F[(int64_t)idx[i] + (int64_t)c * ldf];
     }
     __syncthreads();
-    cta_svd(X, nidx, nidx, r, Ux, nidx, sx, Vx, r, svdw, iwork, &s_flag);
+    extern __shared__ __align__(16) double dyn_smem[];
+    cta_svd(X, nidx, nidx, r, Ux, nidx, sx, Vx, r, svdw, iwork, &s_flag, dyn_smem, a.smem_doubles);
     if (tid == 0) { double sm = sx[p - 1]; *out = sm == 0.0 ? INFINITY : 1.0 / sm; }
 }
 
@@ -289,9 +294,21 @@ size_t core_work_doubles(int k, int l) {
     return d;
 }
 
-int scross_core(lrp_ctx* ctx, const CoreArgs& a) {
+static size_t jacobi_smem_bytes(const lrp_ctx* ctx, int T, int p) {
+    size_t need = ((size_t)T * p + (size_t)p * p) * sizeof(double);
+    size_t cap = (size_t)ctx->smem_optin > 2048 ? (size_t)ctx->smem_optin - 2048 : 0;
+    return need <= cap ? need : 0;                 // 0: stay in global memory
+}
+
+int scross_core(lrp_ctx* ctx, const CoreArgs& a0) {
+    CoreArgs a = a0;
+    const int T = a.k > a.l ? a.k : a.l, p = a.k > a.l ? a.l : a.k;
+    const size_t smem = jacobi_smem_bytes(ctx, T, p);
+    a.smem_doubles = (int)(smem / sizeof(double));
+    if (smem > 48 * 1024)
+        LRP_CUDA(ctx, cudaFuncSetAttribute(scross_core_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_CORE, 0, 0);
-    scross_core_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
+    scross_core_kernel<<<1, CORE_NT, smem, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
@@ -301,9 +318,16 @@ size_t eta_work_doubles(int nmax, int r) {
     return (size_t)nmax * r + (size_t)nmax * p + p + (size_t)r * p + T * p + p * p + p + 64;
 }
 
-int eta_pair(lrp_ctx* ctx, const EtaArgs& a) {
+int eta_pair(lrp_ctx* ctx, const EtaArgs& a0) {
+    EtaArgs a = a0;
+    const int nmax = a.nI > a.nJ ? a.nI : a.nJ;
+    const int T = nmax > a.r ? nmax : a.r, p = nmax > a.r ? a.r : nmax;
+    const size_t smem = jacobi_smem_bytes(ctx, T, p > 0 ? p : 1);
+    a.smem_doubles = (int)(smem / sizeof(double));
+    if (smem > 48 * 1024)
+        LRP_CUDA(ctx, cudaFuncSetAttribute(eta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_ETA, 0, 0);
-    eta_kernel<<<2, CORE_NT, 0, ctx->stream>>>(a);
+    eta_kernel<<<2, CORE_NT, smem, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }

@@ -14,6 +14,7 @@ struct CoreArgs {
     double* rC; double* rR;                     // |diag R_C| (k), |diag R_R| (l)
     int32_t* scal_i; double* scal_d;            // [0] = numerical rank ; [0] = smin_full
     double* work; int32_t* iwork;               // core_work_doubles(k, l) doubles, max(k, l) ints
+    int smem_doubles;                           // set by scross_core: dynamic shared memory available to the Jacobi sweeps
 };
 size_t core_work_doubles(int k, int l);
 int scross_core(lrp_ctx* ctx, const CoreArgs& a);
@@ -24,6 +25,7 @@ struct EtaArgs {
     const double* V; int64_t ldv; const int32_t* J; int nJ;
     double* eta;                                // [2] device: eta1, eta2
     double* work; size_t work_stride; int32_t* iwork; size_t iwork_stride;
+    int smem_doubles;
 };
 size_t eta_work_doubles(int nmax, int r);
 int eta_pair(lrp_ctx* ctx, const EtaArgs& a);

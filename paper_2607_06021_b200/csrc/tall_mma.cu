@@ -32,7 +32,10 @@ __host__ __device__ inline int mg_kp(int k) {         // padded k: multiple of 4
     return k4 + (((4 - k4 % 16) + 16) % 16);
 }
 
-template <int NJ>
+// Row mapping of a warp's 32 rows: fragment i (0..3) of lane group g holds row R0 + 16 (i>>1) + 2 g + (i&1), so that
+// a thread owns row PAIRS and, when the operands are 16-byte aligned with even leading dimensions (VEC), moves them
+// with 128-bit loads / stores (the output-row order of an MMA is bookkeeping only).
+template <int NJ, bool VEC>
 __global__ void __launch_bounds__(MG_THREADS)
 tall_gemm_mma_kernel(TallGemmArgs p) {
     constexpr int MG_CT = 8 * NJ;
@@ -44,7 +47,6 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
     const double invN = 1.0 / (double)(p.n + 1);
     const double fourN2 = 4.0 * (double)(p.n + 1) * (double)(p.n + 1);
     const int64_t nslab = (p.n + MG_THREADS - 1) / MG_THREADS;
-    const bool single_tile = p.m <= MG_CT;             // B staged once, the CTA then streams its row slabs
     for (int c0 = 0; c0 < p.m; c0 += MG_CT) {
         __syncthreads();
         for (int e = tid; e < MG_CT * k4; e += MG_THREADS) {
@@ -59,12 +61,12 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
         if (p.mode == TG_SAMPLE)
             for (int c = tid; c < MG_CT; c += MG_THREADS) dcol[c] = (c0 + c < p.m) ? eig_d(p.idx[c0 + c], invN, fourN2) : 1.0;
         __syncthreads();
-      for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
+      for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {   // B staged once, the CTA streams its row slabs
         const int64_t R0 = slab * MG_THREADS + warp * 32;
         int64_t rows[4]; bool valid[4]; double drow[4], nrm[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            rows[i] = R0 + 8 * i + g; valid[i] = rows[i] < p.n;
+            rows[i] = R0 + 16 * (i >> 1) + 2 * g + (i & 1); valid[i] = rows[i] < p.n;
             drow[i] = (p.mode == TG_SAMPLE && valid[i]) ? eig_d(rows[i], invN, fourN2) : 0.0;
             nrm[i] = 0.0;
         }
@@ -77,8 +79,17 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
         for (int t0 = 0; t0 < k4; t0 += 4) {
             const int t = t0 + tg;
             double a[4], b[NJ];
+            if (VEC) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = (valid[i] && t < p.k) ? p.A[rows[i] + (int64_t)t * p.lda] : 0.0;
+                for (int h = 0; h < 2; ++h) {
+                    double2 v = make_double2(0.0, 0.0);
+                    if (valid[2 * h] && t < p.k) v = *reinterpret_cast<const double2*>(p.A + rows[2 * h] + (int64_t)t * p.lda);
+                    a[2 * h] = v.x; a[2 * h + 1] = v.y;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) a[i] = (valid[i] && t < p.k) ? p.A[rows[i] + (int64_t)t * p.lda] : 0.0;
+            }
 #pragma unroll
             for (int j = 0; j < NJ; ++j) b[j] = Bs[(8 * j + g) * kp + t];
 #pragma unroll
@@ -87,19 +98,33 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
                 for (int j = 0; j < NJ; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            if (!valid[i]) continue;
+        for (int h = 0; h < 2; ++h) {
+            if (!valid[2 * h]) continue;
+            const bool pair = VEC && valid[2 * h + 1];
 #pragma unroll
             for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int cl = 8 * j + 2 * tg + e, col = c0 + cl;
-                    if (col < p.m) {
-                        double v = acc[i][j][e];
-                        if (p.mode == TG_SAMPLE) v = v / (drow[i] + dcol[cl]);
-                        else if (p.mode == TG_SUBTRACT) v = p.Cin[rows[i] + (int64_t)col * p.ldc] - v;
-                        p.Out[rows[i] + (int64_t)col * p.ldo] = v;
-                        nrm[i] = fma(v, v, nrm[i]);
+                    if (col >= p.m) continue;
+                    double v0 = acc[2 * h][j][e], v1 = acc[2 * h + 1][j][e];
+                    if (p.mode == TG_SAMPLE) { v0 = v0 / (drow[2 * h] + dcol[cl]); v1 = v1 / (drow[2 * h + 1] + dcol[cl]); }
+                    if (pair) {
+                        if (p.mode == TG_SUBTRACT) {
+                            double2 cin = *reinterpret_cast<const double2*>(p.Cin + rows[2 * h] + (int64_t)col * p.ldc);
+                            v0 = cin.x - v0; v1 = cin.y - v1;
+                        }
+                        *reinterpret_cast<double2*>(p.Out + rows[2 * h] + (int64_t)col * p.ldo) = make_double2(v0, v1);
+                        nrm[2 * h] = fma(v0, v0, nrm[2 * h]); nrm[2 * h + 1] = fma(v1, v1, nrm[2 * h + 1]);
+                    } else {
+                        if (p.mode == TG_SUBTRACT) v0 = p.Cin[rows[2 * h] + (int64_t)col * p.ldc] - v0;
+                        p.Out[rows[2 * h] + (int64_t)col * p.ldo] = v0;
+                        nrm[2 * h] = fma(v0, v0, nrm[2 * h]);
+                        if (valid[2 * h + 1]) {
+                            if (p.mode == TG_SUBTRACT) v1 = p.Cin[rows[2 * h + 1] + (int64_t)col * p.ldc] - v1;
+                            p.Out[rows[2 * h + 1] + (int64_t)col * p.ldo] = v1;
+                            nrm[2 * h + 1] = fma(v1, v1, nrm[2 * h + 1]);
+                        }
                     }
                 }
         }
@@ -114,13 +139,13 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
         }
       }
     }
-    (void)single_tile;
 }
 
 // ---- S = A^T B: 8 warps per CTA; the CTA owns ntc <= 8 tiles (16 x 16) of S and its row slab; the 8/ntc warps
 //      that share a tile split the slab's rows and are summed through shared memory in a fixed order -------------
 constexpr int MT_THREADS = 256;
 
+template <bool VEC>
 __global__ void __launch_bounds__(MT_THREADS)
 tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const double* __restrict__ B, int64_t ldb, int m,
                        int64_t n, int64_t rows_per_cta, double* __restrict__ partial, int na, int nb, int ntc) {
@@ -143,7 +168,18 @@ tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const d
         for (int64_t rb = c_begin + 16 * sub; rb < c_end; rb += 16 * nsub) {   // warp-uniform (mma.sync needs the whole warp)
             const int64_t r = rb + tg;
             double x0[4], x1[4], y0[4], y1[4];
-            if (rb + 16 <= c_end) {
+            if (VEC && rb + 16 <= c_end) {
+                // 128-bit loads of row pairs: MMA step 2u takes rows rb + 8u + 2 tg, step 2u+1 the rows after them (the
+                // order of the summed rows is free as long as both operands use the same one)
+                const int64_t rv2 = rb + 2 * tg;
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    double2 a0 = *reinterpret_cast<const double2*>(pa0 + rv2 + 8 * u), a1 = *reinterpret_cast<const double2*>(pa1 + rv2 + 8 * u);
+                    double2 b0 = *reinterpret_cast<const double2*>(pb0 + rv2 + 8 * u), b1 = *reinterpret_cast<const double2*>(pb1 + rv2 + 8 * u);
+                    x0[2 * u] = a0.x; x0[2 * u + 1] = a0.y; x1[2 * u] = a1.x; x1[2 * u + 1] = a1.y;
+                    y0[2 * u] = b0.x; y0[2 * u + 1] = b0.y; y1[2 * u] = b1.x; y1[2 * u + 1] = b1.y;
+                }
+            } else if (rb + 16 <= c_end) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) { x0[u] = pa0[r + 4 * u]; x1[u] = pa1[r + 4 * u]; y0[u] = pb0[r + 4 * u]; y1[u] = pb1[r + 4 * u]; }
             } else {
@@ -206,17 +242,20 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
     if (p.n <= 0 || p.m <= 0) return LRP_OK;
     const int nj = p.m <= 16 ? 2 : 4;
     size_t smem = sizeof(double) * ((size_t)(8 * nj) * mg_kp(p.k > 0 ? p.k : 1) + 8 * nj);
+    auto al16 = [](const void* q) { return ((uintptr_t)q & 15u) == 0; };
+    const bool vec = (p.lda % 2 == 0) && (p.ldo % 2 == 0) && al16(p.A) && al16(p.Out) &&
+                     (p.mode != TG_SUBTRACT || ((p.ldc % 2 == 0) && al16(p.Cin)));
+    void (*kern)(TallGemmArgs) = nj == 2 ? (vec ? tall_gemm_mma_kernel<2, true> : tall_gemm_mma_kernel<2, false>)
+                                         : (vec ? tall_gemm_mma_kernel<4, true> : tall_gemm_mma_kernel<4, false>);
     if (smem > 48 * 1024) {
         if (smem > (size_t)ctx->smem_optin) return LRP_ERR_BADARG;
-        LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_mma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        LRP_CUDA(ctx, cudaFuncSetAttribute(tall_gemm_mma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
     if (grid > 148 * 8) grid = 148 * 8;            // persistent over row slabs: B is staged once per column tile per CTA
     LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
              8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
-    if (nj == 2) tall_gemm_mma_kernel<2><<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
-    else tall_gemm_mma_kernel<4><<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
+    kern<<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
@@ -249,7 +288,9 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
     const int na = (k + 15) / 16, nb = (m + 15) / 16;
     dim3 grid(nblk, (na * nb + ntc - 1) / ntc);
     LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
-    tall_gemm_t_mma_kernel<<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
+    const bool vec = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) & 15u) == 0;
+    if (vec) tall_gemm_t_mma_kernel<true><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
+    else tall_gemm_t_mma_kernel<false><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
     LRP_LAUNCHED(ctx);
     int tot = k * m;
     LRP_PROF(ctx, K_REDUCE, 8.0 * nblk * k * m, 0);
