@@ -35,7 +35,7 @@ template <int Q> struct SmallCfg {
     static constexpr int L = 1 << Q, N = 2 * L, GS = L / 8;
     static constexpr int CPB = GS >= 256 ? 1 : 256 / GS;
     static constexpr int NT = GS * CPB;
-    static constexpr int PL = PADI(L) + 1;
+    static constexpr int PL = L + 1;
     static constexpr int NHI = N / 64 + 1;
     static constexpr size_t SMEM = sizeof(double2) * (64 + NHI) + sizeof(double) * ((size_t)CPB * 2 * PL + 32 * CPB);
 };

@@ -13,12 +13,13 @@
 #include "common.cuh"
 #include "fft_smem.cuh"
 #include <math.h>
+#include <stdlib.h>
 
 namespace {
 
 constexpr int row_stride(int Lrow, int nrows) {            // padded row length with (stride mod 16) == max(1, 16/nrows)
     int want = (16 / nrows) > 0 ? (16 / nrows) : 1;
-    int base = PADI(Lrow);
+    int base = Lrow;
     return base + (((want - base) % 16) + 16) % 16;
 }
 
@@ -31,13 +32,13 @@ template <int Q1, int TL> struct PACfg {
     static constexpr int IMOFF = T2 * RS + 8;
     static constexpr int NHI = (2 * L1) / 64 + 1;
     static constexpr int TW_LO = 32, TW_HI = (L1 + 31) / 32;
-    static constexpr int CH = TL >= 13 ? 4 : 8;                  // loads in flight per thread (register budget)
+    static constexpr int CH = 4;                  // loads in flight per thread (register budget)
     static constexpr size_t SMEM = sizeof(double2) * (64 + NHI + 2 * T2 + (size_t)T2 * (TW_LO + TW_HI)) +
                                    sizeof(double) * ((size_t)2 * IMOFF);
 };
 
 template <int Q1, int TL>
-__global__ void __launch_bounds__(PACfg<Q1, TL>::NT)
+__global__ void __launch_bounds__(PACfg<Q1, TL>::NT, TL <= 12 ? 2 : 1)
 dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2* __restrict__ W) {
     using C = PACfg<Q1, TL>;
     constexpr int L1 = C::L1, GS = C::GS, T2 = C::T2, T = C::T, RS = C::RS, NT = C::NT;
@@ -132,7 +133,7 @@ __device__ __forceinline__ void untangle_pair(double2& zk, double2& zm, double2 
 }
 
 template <int Q2, int TL>
-__global__ void __launch_bounds__(PBCfg<Q2, TL>::NT)
+__global__ void __launch_bounds__(PBCfg<Q2, TL>::NT, TL <= 12 ? 2 : 1)
 dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out, double scale) {
     using C = PBCfg<Q2, TL>;
     constexpr int L2 = C::L2, GS = C::GS, R2 = C::R2, T = C::T, RS = C::RS, NT = C::NT;
@@ -319,12 +320,16 @@ void plan(int log2N, int* tl, int* q1, int* q2) {
     const int q = log2N - 1;
     *tl = q <= 22 ? 12 : 13;
     *q2 = q / 2; *q1 = q - *q2;
+    if (const char* e = getenv("LRP_DST_TL")) { int v = atoi(e); if (v == 13 && q >= 14) *tl = 13; }
+    if (const char* e = getenv("LRP_DST_Q1")) { int v = atoi(e); if (v >= 7 && v <= *tl - 1 && q - v >= 7 && q - v <= *tl - 1) { *q1 = v; *q2 = q - v; } }
 }
 
 // columns per group: W + output of one group should stay L2-resident between the sweeps
 int group_cols(int64_t N, int batch) {
     int64_t per_col = N * 16;
-    int g = (int)(((int64_t)48 << 20) / per_col);
+    static int64_t budget_mb = 0;
+    if (budget_mb == 0) { const char* e = getenv("LRP_DST_GROUP_MB"); budget_mb = e ? atoll(e) : 4096; if (budget_mb < 1) budget_mb = 4096; }
+    int g = (int)((budget_mb << 20) / per_col);
     if (g < 1) g = 1;
     if (g > batch) g = batch;
     return g;

@@ -5,7 +5,9 @@
 
 namespace {
 
-__host__ __device__ constexpr int PADI(int i) { return i + (i >> 5); }
+// bank swizzle of a shared-memory sequence index (a bijection on every aligned block of 16): stride-1, stride-8 and
+// the 8-wide interleaved store patterns of the Stockham passes all become conflict-free for 8-byte accesses
+__host__ __device__ constexpr int PADI(int i) { return i ^ ((i >> 3) & 15); }
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
