@@ -32,7 +32,7 @@ int check_n(int64_t n) {
 
 // ------------------------------------------------------------------------------------------------ scross on owned buffers
 struct ScrossWs {
-    double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws;
+    double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws, *qr_ws2;
     int32_t *scal_i, *iwork;
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int kmax, int lmax) {
         int K = kmax > lmax ? kmax : lmax;
@@ -42,6 +42,7 @@ struct ScrossWs {
         scal_d = ar.take<double>(8); scal_i = ar.take<int32_t>(8); iwork = ar.take<int32_t>(K);
         core_work = ar.take<double>(core_work_doubles(K, K));
         qr_ws = ar.take<double>(tall_qr_ws_doubles(ctx, n, K));
+        qr_ws2 = ar.take<double>(tall_qr_ws_doubles(ctx, n, K));
         return ar.ok();
     }
 };
@@ -52,8 +53,7 @@ int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, doubl
                   const int32_t* dI, const int32_t* dJ, ScrossWs& w,
                   double* h_S, double* h_rC, double* h_rR, int* h_rank, double* h_smin,
                   cudaEvent_t ev_qr_done) {
-    LRP_TRY(tall_qr(ctx, n, k, Qb, ldq, w.RC, k, w.qr_ws));
-    LRP_TRY(tall_qr(ctx, n, l, Zb, ldz, w.RR, l, w.qr_ws));
+    LRP_TRY(tall_qr_pair(ctx, n, k, Qb, ldq, w.RC, k, w.qr_ws, l, Zb, ldz, w.RR, l, w.qr_ws2));
     if (ev_qr_done) LRP_CUDA(ctx, cudaEventRecord(ev_qr_done, ctx->stream));
     CoreArgs a{};
     a.k = k; a.l = l; a.Q = Qb; a.ldq = ldq; a.Z = Zb; a.ldz = ldz; a.RC = w.RC; a.ldrc = k; a.RR = w.RR; a.ldrr = l;
@@ -192,6 +192,11 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
     c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
+    c->aux = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->pinned = nullptr;
+    if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+        cudaHostAlloc((void**)&c->pinned, 8192, cudaHostAllocDefault) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     *out = c;
@@ -201,6 +206,10 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
 int lrp_destroy(lrp_ctx* ctx) {
     if (!ctx) return LRP_OK;
     if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
+    if (ctx->aux) cudaStreamDestroy(ctx->aux);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    if (ctx->pinned) cudaFreeHost(ctx->pinned);
     delete ctx->ev_id;
     delete ctx;
     return LRP_OK;
@@ -524,6 +533,27 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (h_trace_keepJ) memcpy(h_trace_keepJ + tr_offJ, keepJ.data(), kk);
         tr_offI += l; tr_offJ += kk; rep_offI += l; rep_offJ += kk;
         // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
+        // eta (two one-CTA Jacobi SVDs) runs on the auxiliary stream while the rho contractions fill the GPU
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0));
+        {
+            cudaStream_t main_stream = ctx->stream;
+            ctx->stream = ctx->aux;
+            int rc_eta = LRP_OK;
+            cudaError_t e1 = cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
+            cudaError_t e2 = cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
+            if (e1 != cudaSuccess || e2 != cudaSuccess) { ctx->last_cuda = (int)(e1 != cudaSuccess ? e1 : e2); rc_eta = LRP_ERR_CUDA; }
+            if (rc_eta == LRP_OK) {
+                EtaArgs ea{};
+                ea.r = rank; ea.U = Uk; ea.ldu = ld; ea.I = w.dIpr; ea.nI = (int)I_pr.size(); ea.V = Vk; ea.ldv = ld; ea.J = w.dJpr; ea.nJ = (int)J_pr.size();
+                ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
+                rc_eta = eta_pair(ctx, ea);
+            }
+            cudaError_t e3 = cudaEventRecord(ctx->ev_join, ctx->stream);
+            ctx->stream = main_stream;
+            if (rc_eta < 0) return rc_eta;
+            if (e3 != cudaSuccess) { ctx->last_cuda = (int)e3; return LRP_ERR_CUDA; }
+        }
         RhoArgs ra{};
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
         ra.out = w.rho_out;
@@ -541,12 +571,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             }
         }
         LRP_TRY(rho_small(ctx, ra));
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream));
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream));
-        EtaArgs ea{};
-        ea.r = rank; ea.U = Uk; ea.ldu = ld; ea.I = w.dIpr; ea.nI = (int)I_pr.size(); ea.V = Vk; ea.ldv = ld; ea.J = w.dJpr; ea.nJ = (int)J_pr.size();
-        ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
-        LRP_TRY(eta_pair(ctx, ea));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
         double h_rho[2], h_eta[2];
         LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(h_eta, w.eta, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));

@@ -5,3 +5,12 @@
 // ws: tall_qr_ws_doubles(ctx, n, K) doubles of scratch.
 size_t tall_qr_ws_doubles(const lrp_ctx* ctx, int64_t n, int K);
 int tall_qr(lrp_ctx* ctx, int64_t n, int K, double* A, int64_t lda, double* R, int64_t ldr, double* ws);
+// Two independent factorizations advanced panel by panel on ctx->stream and ctx->aux (joined on return into ctx->stream).
+int tall_qr_pair(lrp_ctx* ctx, int64_t n, int K1, double* A1, int64_t lda1, double* R1, int64_t ldr1, double* ws1,
+                 int K2, double* A2, int64_t lda2, double* R2, int64_t ldr2, double* ws2);
+
+struct QrJob {
+    int64_t n; int K; double* A; int64_t lda; double* R; int64_t ldr; double* ws; cudaStream_t stream;
+    double* hR;                                   // pinned host scratch, 256 doubles
+    double *stack, *partial, *Stmp, *d_runmax;    // carved from ws by tall_qr_begin
+};
