@@ -232,6 +232,19 @@ def main():
         roof = {"bound": "hbm", "achieved": top["alg_GBps"], "peak": hbm_peak, "unit": "GB/s",
                 "frac": top["alg_GBps"] / hbm_peak, "traffic": None, "peak_source": peak_src}
     roof["kernel"] = top["kernel"]; roof["share_of_step"] = top["share"]
+    # measured DRAM traffic of that kernel class from the committed ncu capture (ratio to its algorithmic bytes), per launch
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r01b_traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == top["kernel"]:
+                    ratio = float(row["dram_bytes_per_launch"]) / float(row["alg_bytes_per_launch"])
+                    v = prof[top["kernel"]]
+                    roof["traffic"] = ratio * v["bytes"] / v["count"]
+                    roof["alg_bytes_per_launch"] = v["bytes"] / v["count"]
+                    roof["traffic_source"] = row["capture"]
+    except Exception:
+        pass
 
     # ---- batched DST-I side measurement (metric's second half): n = 2^p - 1, batch 128, buffers rotate beyond L2
     dst = None

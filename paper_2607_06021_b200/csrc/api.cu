@@ -535,10 +535,11 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
         // eta (two one-CTA Jacobi SVDs) runs on the auxiliary stream while the rho contractions fill the GPU
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
-        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0));
+        cudaStream_t side = ctx->prof_on ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
+        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         {
             cudaStream_t main_stream = ctx->stream;
-            ctx->stream = ctx->aux;
+            ctx->stream = side;
             int rc_eta = LRP_OK;
             cudaError_t e1 = cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
             cudaError_t e2 = cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream);

@@ -36,7 +36,7 @@ __host__ __device__ inline int mg_kp(int k) {         // padded k: multiple of 4
 // a thread owns row PAIRS and, when the operands are 16-byte aligned with even leading dimensions (VEC), moves them
 // with 128-bit loads / stores (the output-row order of an MMA is bookkeeping only).
 template <int NJ, bool VEC>
-__global__ void __launch_bounds__(MG_THREADS)
+__global__ void __launch_bounds__(MG_THREADS, NJ == 2 ? 5 : 4)
 tall_gemm_mma_kernel(TallGemmArgs p) {
     constexpr int MG_CT = 8 * NJ;
     extern __shared__ __align__(16) double smem[];
