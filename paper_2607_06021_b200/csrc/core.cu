@@ -130,6 +130,63 @@ __device__ void cta_matmul(double* C, int ldc, int m, int n, int kk, const doubl
     __syncthreads();
 }
 
+// Least squares X Y = B by Householder QR of W = [X | B] (rows x (xn + nb), column-major, ld ldw, overwritten):
+// Y (xn x nb, ld ldy) = R^-1 (Q^T B)(0:xn, :).  Equals pinv(X) B when X has full column rank, which is how the
+// pseudo-inverse of Alg. 1 lines 5-14 is applied when X is well conditioned ("\" in the paper);
+// *cond_flag is set to 1 when min|R_cc| < 1e-8 max|R_cc| (the caller then takes the SVD pseudo-inverse instead).
+__device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb, double* Y, int ldy,
+                                   double* s_scal, int* cond_flag) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int ncol = xn + nb;
+    for (int c = 0; c < xn; ++c) {
+        double* xc = W + (size_t)c * ldw;
+        if (warp == 0) {
+            double sig = 0.0;
+            for (int r = c + 1 + lane; r < rows; r += 32) sig = fma(xc[r], xc[r], sig);
+            sig = warp_sum(sig);
+            const double alpha = xc[c];
+            double beta, tau, inv;
+            if (sig == 0.0) { beta = alpha; tau = 0.0; inv = 0.0; }
+            else {
+                beta = -copysign(sqrt(fma(alpha, alpha, sig)), alpha);
+                tau = (beta - alpha) / beta;
+                inv = 1.0 / (alpha - beta);
+            }
+            for (int r = c + 1 + lane; r < rows; r += 32) xc[r] *= inv;       // v (unit diagonal implicit)
+            if (lane == 0) { xc[c] = beta; s_scal[0] = tau; }
+        }
+        __syncthreads();
+        const double tau = s_scal[0];
+        for (int j = c + 1 + warp; j < ncol; j += nwarps) {
+            double* aj = W + (size_t)j * ldw;
+            double acc = 0.0;
+            for (int r = c + 1 + lane; r < rows; r += 32) acc = fma(xc[r], aj[r], acc);
+            acc = warp_sum(acc);
+            const double w = tau * (aj[c] + acc);
+            for (int r = c + 1 + lane; r < rows; r += 32) aj[r] = fma(-xc[r], w, aj[r]);
+            if (lane == 0) aj[c] -= w;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        double mx = 0.0, mn = INFINITY;
+        for (int c = 0; c < xn; ++c) { double d = fabs(W[c + (size_t)c * ldw]); mx = fmax(mx, d); mn = fmin(mn, d); }
+        *cond_flag = !(mn >= 1e-8 * mx && mx > 0.0);
+    }
+    __syncthreads();
+    if (*cond_flag) return;
+    for (int j = tid; j < nb; j += blockDim.x) {          // back substitution, one right-hand side per thread
+        const double* bj = W + (size_t)(xn + j) * ldw;
+        double* yj = Y + (size_t)j * ldy;
+        for (int i = xn - 1; i >= 0; --i) {
+            double acc = bj[i];
+            for (int t = i + 1; t < xn; ++t) acc = fma(-W[i + (size_t)t * ldw], yj[t], acc);
+            yj[i] = acc / W[i + (size_t)i * ldw];
+        }
+    }
+    __syncthreads();
+}
+
 // ----------------------------------------------------------------------------------------------------------
 // scross core.  QR factors: Qf (n x k) with R_C (k x k), Zf (n x l) with R_R (l x l).
 __global__ void __launch_bounds__(CORE_NT)
@@ -157,6 +214,36 @@ scross_core_kernel(CoreArgs a) {
     for (int c = tid; c < l; c += nt) a.rR[c] = fabs(a.RR[c + (size_t)c * a.ldrr]);
     __syncthreads();
     extern __shared__ __align__(16) double dyn_smem[];
+    __shared__ double s_scal[2];
+    __shared__ int s_cond;
+    // Well-conditioned X (the usual case): M = X^+ B as the Householder least-squares solution of X Y = B, with
+    // B = R_R^T (k <= l, M = Y) or B = R_C^T (k > l, M = Y^T).  Otherwise the SVD pseudo-inverse below.
+    {
+        const int ldw = xm | 1;                                       // odd leading dimension: no bank conflicts
+        const bool fits = (size_t)ldw * (xn + xm) <= (size_t)a.smem_doubles;
+        double* Wls = fits ? dyn_smem : svdw;                         // svdw has room only when core_work is sized for it
+        const double* Ro = kle ? a.RR : a.RC; const int64_t ldo = kle ? a.ldrr : a.ldrc;
+        if (fits) {
+            for (int e = tid; e < xm * xn; e += nt) Wls[(e % xm) + (size_t)(e / xm) * ldw] = X[e];
+            for (int e = tid; e < xm * xm; e += nt) {
+                int i = e % xm, j = e / xm;                            // B(i,j) = Rother(j,i)
+                Wls[i + (size_t)(xn + j) * ldw] = Ro[j + (size_t)i * ldo];
+            }
+            __syncthreads();
+            cta_ls_householder(Wls, ldw, xm, xn, xm, P, xn, s_scal, &s_cond);   // Y (xn x xm) into P's storage
+        } else {
+            if (tid == 0) s_cond = 1;
+            __syncthreads();
+        }
+    }
+    if (!s_cond) {
+        // Y = P (xn x xm).  k <= l: M = Y (k x l);  k > l: M = Y^T
+        for (int e = tid; e < k * l; e += nt) {
+            int i = e % k, j = e / k;
+            Mc[e] = kle ? P[i + (size_t)j * xn] : P[j + (size_t)i * xn];
+        }
+        __syncthreads();
+    } else {
     cta_svd(X, xm, xm, xn, Ux, xm, sx, Vx, xn, svdw, a.iwork, &s_flag, dyn_smem, a.smem_doubles);
     // P = Vx diag(1/sx) Ux^T over the kept singular values (relative cut, reading Q4)
     {
@@ -178,6 +265,7 @@ scross_core_kernel(CoreArgs a) {
     } else {
         // M = R_C (k x k) * P^T (k x l): M(i,j) = sum_t R_C(i,t) P(j,t),  P is l x k
         cta_matmul(Mc, k, k, l, k, a.RC, 1, (int)a.ldrc, P, l, 1);
+    }
     }
     const int p = k < l ? k : l;
     cta_svd(Mc, k, k, l, a.Uc, k, a.S, a.Vc, l, svdw, a.iwork, &s_flag, dyn_smem, a.smem_doubles);
@@ -303,7 +391,12 @@ static size_t jacobi_smem_bytes(const lrp_ctx* ctx, int T, int p) {
 int scross_core(lrp_ctx* ctx, const CoreArgs& a0) {
     CoreArgs a = a0;
     const int T = a.k > a.l ? a.k : a.l, p = a.k > a.l ? a.l : a.k;
-    const size_t smem = jacobi_smem_bytes(ctx, T, p);
+    size_t smem = jacobi_smem_bytes(ctx, T, p);
+    {
+        size_t ls = (size_t)(T | 1) * (size_t)(p + T) * sizeof(double);
+        size_t cap = (size_t)ctx->smem_optin > 2048 ? (size_t)ctx->smem_optin - 2048 : 0;
+        if (ls > smem && ls <= cap) smem = ls;
+    }
     a.smem_doubles = (int)(smem / sizeof(double));
     if (smem > 48 * 1024)
         LRP_CUDA(ctx, cudaFuncSetAttribute(scross_core_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
