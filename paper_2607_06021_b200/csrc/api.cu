@@ -112,7 +112,7 @@ int validate_indices(const int32_t* h, int cnt, int64_t n) {
 // ------------------------------------------------------------------------------------------------ solve workspace
 struct SolveWs {
     double *UhF, *VhF, *Cb, *Rb, *Ua, *Va, *Ub, *Vb, *scoresU, *scoresV;
-    double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *Rlev;
+    double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
     unsigned char* mask;
     void *sel_ws, *dst_ws;
@@ -134,6 +134,7 @@ struct SolveWs {
         eta_work = ar.take<double>(2 * eta_stride);
         eta_iwork = ar.take<int32_t>(2 * (size_t)Kc);
         gemmt_ws = ar.take<double>(tall_gemm_t_ws_doubles(ctx, n, Kc, Kc));
+        gemmt_ws2 = ar.take<double>(tall_gemm_t_ws_doubles(ctx, n, Kc, Kc));
         dI = ar.take<int32_t>(Kc); dJ = ar.take<int32_t>(Kc); dIpr = ar.take<int32_t>(Kc); dJpr = ar.take<int32_t>(Kc);
         dIstar = ar.take<int32_t>(2 * (size_t)Kc + 8); dJstar = ar.take<int32_t>(2 * (size_t)Kc + 8);
         mask = ar.take<unsigned char>(Kc);
@@ -155,6 +156,10 @@ struct EventPool {
     }
     static float ms(cudaEvent_t a, cudaEvent_t b) { float t = 0.f; if (a && b) cudaEventElapsedTime(&t, a, b); return t; }
 };
+
+// Run `expr` (helpers launch on ctx->stream) on another stream.
+#define LRP_ON_STREAM(ctx, strm, expr)                                          \
+    do { cudaStream_t m_ = (ctx)->stream; (ctx)->stream = (strm); int rc2_ = (expr); (ctx)->stream = m_; if (rc2_ < 0) return rc2_; } while (0)
 
 void host_union(std::vector<int32_t>& cur, const int32_t* star, int nstar, int* added) {
     *added = 0;
@@ -500,8 +505,13 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_CUDA(ctx, cudaMemcpyAsync(w.dJ, J_k.data(), sizeof(int32_t) * kk, cudaMemcpyHostToDevice, ctx->stream));
         cudaEvent_t e1 = ep.rec(ctx);
         // ---- O4: fibers  C = G(:,J) (n x kk), Rt = G(I,:)^T (n x l)
+        // the two sides of a sweep are independent until the small core: they run on the main and the auxiliary stream
+        // (every tall kernel here is latency-bound well below the HBM peak, so two in flight overlap usefully)
+        cudaStream_t side = ctx->prof_on ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ, kk, w.Cb, ld));
-        LRP_TRY(sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI, l, w.Rb, ld));
+        LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI, l, w.Rb, ld));
         cudaEvent_t e2 = ep.rec(ctx);
         // ---- O8: scross
         cudaEvent_t e3 = nullptr;
@@ -509,8 +519,10 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, w.Rb, ld, l, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
         cudaEvent_t e4 = ep.rec(ctx);
         const int p = kk < l ? kk : l;
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         LRP_TRY(rebuild(ctx, n, w.Cb, ld, kk, w.sc.Uc, kk, rank, Uk, ld, w.scoresU));
-        LRP_TRY(rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
+        LRP_ON_STREAM(ctx, side, rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
         cudaEvent_t e5 = ep.rec(ctx);
         // ---- O9: prune (Alg. 4 lines 14-23; reading Q12)
         keepI.assign(l, 1); keepJ.assign(kk, 1);
@@ -534,8 +546,8 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         tr_offI += l; tr_offJ += kk; rep_offI += l; rep_offJ += kk;
         // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
         // eta (two one-CTA Jacobi SVDs) runs on the auxiliary stream while the rho contractions fill the GPU
+        // (the auxiliary stream already holds the V-side rebuild; it additionally waits for the U-side rebuild)
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
-        cudaStream_t side = ctx->prof_on ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         {
             cudaStream_t main_stream = ctx->stream;
@@ -550,6 +562,14 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
                 ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
                 rc_eta = eta_pair(ctx, ea);
             }
+            if (rc_eta == LRP_OK && r_prev > 0) {                   // V side of rho on the auxiliary stream as well
+                rc_eta = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
+                TallGemmArgs g{};
+                g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
+                g.Cin = Vp; g.ldc = ld; g.Out = w.Rb; g.ldo = ld;       // fiber buffers are free after the rebuild
+                if (rc_eta >= 0) rc_eta = tall_gemm(ctx, g);
+                if (rc_eta >= 0) rc_eta = tall_gemm_t(ctx, n, w.Rb, ld, r_prev, w.Rb, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
+            }
             cudaError_t e3 = cudaEventRecord(ctx->ev_join, ctx->stream);
             ctx->stream = main_stream;
             if (rc_eta < 0) return rc_eta;
@@ -559,20 +579,15 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
         ra.out = w.rho_out;
         if (r_prev > 0) {
-            for (int side = 0; side < 2; ++side) {
-                const double* Xk = side == 0 ? Uk : Vk; const double* Xp = side == 0 ? Up : Vp;
-                double* Am = side == 0 ? w.Amat : w.Bmat; double* G = side == 0 ? w.GU : w.GV;
-                double* E = side == 0 ? w.Cb : w.Rb;                      // fiber buffers are free after the rebuild
-                LRP_TRY(tall_gemm_t(ctx, n, Xk, ld, rank, Xp, ld, r_prev, Am, rank, 0, w.gemmt_ws));
-                TallGemmArgs g{};
-                g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Xk; g.lda = ld; g.B = Am; g.ldb = rank;
-                g.Cin = Xp; g.ldc = ld; g.Out = E; g.ldo = ld;
-                LRP_TRY(tall_gemm(ctx, g));
-                LRP_TRY(tall_gemm_t(ctx, n, E, ld, r_prev, E, ld, r_prev, G, r_prev, 0, w.gemmt_ws));
-            }
+            LRP_TRY(tall_gemm_t(ctx, n, Uk, ld, rank, Up, ld, r_prev, w.Amat, rank, 0, w.gemmt_ws));      // U side
+            TallGemmArgs g{};
+            g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Uk; g.lda = ld; g.B = w.Amat; g.ldb = rank;
+            g.Cin = Up; g.ldc = ld; g.Out = w.Cb; g.ldo = ld;
+            LRP_TRY(tall_gemm(ctx, g));
+            LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, r_prev, w.Cb, ld, r_prev, w.GU, r_prev, 0, w.gemmt_ws));
         }
-        LRP_TRY(rho_small(ctx, ra));
         LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+        LRP_TRY(rho_small(ctx, ra));
         double h_rho[2], h_eta[2];
         LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(h_eta, w.eta, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
