@@ -37,7 +37,7 @@ template <int Q> struct SmallCfg {
     static constexpr int NT = GS * CPB;
     static constexpr int PL = L + 1;
     static constexpr int NHI = N / 64 + 1;
-    static constexpr size_t SMEM = sizeof(double2) * (64 + NHI) + sizeof(double) * ((size_t)CPB * 2 * PL + 32 * CPB);
+    static constexpr size_t SMEM = sizeof(double2) * (64 + NHI) + sizeof(double) * ((size_t)CPB * 2 * PL + 64 * CPB);
 };
 
 template <int Q>
@@ -56,7 +56,7 @@ dst1_small_kernel(int batch, const double* __restrict__ in, int64_t ld_in,
     const bool active = col < batch;
     double* re = data + (size_t)g * 2 * PL;
     double* im = re + PL;
-    double* wsum = data + (size_t)C::CPB * 2 * PL + 32 * g;
+    double* wsum = data + (size_t)C::CPB * 2 * PL + 64 * g;
     const double* x = in + (int64_t)(active ? col : 0) * ld_in;      // x_m = x[m-1]
 
     // global loads first (8 pairs in flight per thread), table build overlaps their latency
@@ -89,7 +89,7 @@ dst1_small_kernel(int batch, const double* __restrict__ in, int64_t ld_in,
         if (k == 0) {
             double a = re[0], b = im[0];
             re[0] = 0.5 * (a + b);                                   // X_1 = T_0 / 2
-            im[0] = 0.0;
+            im[0] = 0.5 * (b - a);                                   // X_{N-1} = -T_L / 2 = (Im Z_0 - Re Z_0)/2
         } else {
             int km = L - k;
             double ak = re[PADI(k)], bk = im[PADI(k)], am = re[PADI(km)], bm = im[PADI(km)];
@@ -102,16 +102,30 @@ dst1_small_kernel(int batch, const double* __restrict__ in, int64_t ld_in,
     }
     __syncthreads();
 
-    // X_{2k+1} = X_1 + sum_{m<=k} R_m : inclusive scan over re[0..L)
+    // Odd outputs P_k = X_{2k+1}: a TWO-SIDED prefix sum.  Lower half forward from P_0 = X_1 (P_k = P_{k-1} + R_k), upper
+    // half backward from the independently known P_{L-1} = X_{N-1} (P_{k-1} = P_k - R_k): every output is reached
+    // through the shorter chain, and the (small) tail of a decaying spectrum is summed from small terms only.
     {
+        constexpr int HS = GS / 2;                                   // threads per half
+        const int half = gt / HS, ht = gt % HS;
         double loc[8];
         double run = 0.0;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { run += re[PADI(gt * 8 + i)]; loc[i] = run; }
-        double incl = group_scan_incl<GS>(run, gt, wsum);
+        for (int i = 0; i < 8; ++i) {
+            const int j = ht * 8 + i;                                // position in the half's sequence
+            double v;
+            if (half == 0) v = re[PADI(j)];                          // R_j (re[0] = X_1)
+            else v = (j == 0) ? im[0] : -re[PADI(L - j)];            // u_0 = X_{N-1}, u_j = -R_{L-j}
+            run += v; loc[i] = run;
+        }
+        __syncthreads();                                             // all inputs read before any output is written
+        double incl = group_scan_incl<HS>(run, ht, wsum + 32 * half);
         double off = incl - run;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) re[PADI(gt * 8 + i)] = loc[i] + off;
+        for (int i = 0; i < 8; ++i) {
+            const int j = ht * 8 + i;
+            re[PADI(half == 0 ? j : L - 1 - j)] = loc[i] + off;      // P_j  /  P_{L-1-j}
+        }
     }
     __syncthreads();
 

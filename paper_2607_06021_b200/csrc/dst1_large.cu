@@ -134,7 +134,8 @@ __device__ __forceinline__ void untangle_pair(double2& zk, double2& zm, double2 
 
 template <int Q2, int TL>
 __global__ void __launch_bounds__(PBCfg<Q2, TL>::NT, TL <= 12 ? 2 : 1)
-dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out, double scale) {
+dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out, double scale,
+               double* __restrict__ xlast, int xstride) {
     using C = PBCfg<Q2, TL>;
     constexpr int L2 = C::L2, GS = C::GS, R2 = C::R2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
@@ -189,6 +190,7 @@ dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ ou
             if (k2 == 0) {
                 double a = re[0], b = im[0];
                 re[0] = 0.5 * (a + b); im[0] = 0.0;               // R_0 := X_1 = T_0/2
+                xlast[(int64_t)blockIdx.y * xstride] = scale * 0.5 * (b - a);   // X_{N-1} = -T_L/2, start of the backward sum
             } else if (k2 <= L2 / 2) {
                 int ia = PADI(k2), ib = PADI(L2 - k2);
                 double2 zk = make_double2(re[ia], im[ia]), zm = make_double2(re[ib], im[ib]);
@@ -218,12 +220,16 @@ dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ ou
 }
 
 // ------------------------------------------------------------------------------------------------ sweep C
-// X_{2k+1} = sum_{m <= k} R_m (R_0 = X_1): in-place inclusive scan over the even-index elements o[0], o[2], ...
+// Odd outputs P_k = X_{2k+1} from R_k = P_k - P_{k-1} (stored at o[2k], R_0 = X_1): a TWO-SIDED in-place sum over the
+// even-index elements.  Lower half of the chunks forward from P_0 = X_1, upper half backward from the independently
+// known P_{L-1} = X_{N-1} (sweep B, xlast): every output is reached through the shorter chain and the small tail of a
+// decaying spectrum is summed from small terms only.  sums: per column nchunks chunk sums + 1 slot for X_{N-1}.
 constexpr int SC_CHUNK = 4096, SC_NT = 512;       // k's per chunk
 
 __global__ void __launch_bounds__(SC_NT)
 dst1_chunksum_kernel(int log2N, const double* __restrict__ out, int64_t ld_out, double* __restrict__ sums) {
     const int64_t L = (int64_t)1 << (log2N - 1);
+    const int nch = (int)(L / SC_CHUNK);
     const double* o = out + (int64_t)blockIdx.y * ld_out + 2 * (int64_t)blockIdx.x * SC_CHUNK;
     __shared__ double ws[32];
     double acc = 0.0;
@@ -235,42 +241,63 @@ dst1_chunksum_kernel(int log2N, const double* __restrict__ out, int64_t ld_out, 
     if (threadIdx.x == 0) {
         double t = 0.0;
         for (int w = 0; w < SC_NT / 32; ++w) t += ws[w];
-        sums[(int64_t)blockIdx.y * (L / SC_CHUNK) + blockIdx.x] = t;
+        sums[(int64_t)blockIdx.y * (nch + 1) + blockIdx.x] = t;
     }
 }
 
-// exclusive scan of the chunk sums of one column (one CTA per column)
+// per column (one CTA): chunks c < nch/2 get the exclusive prefix of the chunk sums, chunks c >= nch/2 the exclusive
+// suffix (sum of the chunks above them, accumulated from the top)
 __global__ void __launch_bounds__(1024)
 dst1_scansums_kernel(int nchunks, double* __restrict__ sums) {
-    double* s = sums + (int64_t)blockIdx.x * nchunks;
+    double* s = sums + (int64_t)blockIdx.x * (nchunks + 1);
     __shared__ double wsum[32];
     __shared__ double tot;
-    double carry = 0.0;
-    for (int base = 0; base < nchunks; base += 1024) {
-        int i = base + threadIdx.x;
-        double v = i < nchunks ? s[i] : 0.0;
-        double incl = group_scan_incl<1024>(v, threadIdx.x, wsum);
-        if (i < nchunks) s[i] = carry + incl - v;
-        if (threadIdx.x == 1023) tot = incl;
-        __syncthreads();
-        carry += tot;
-        __syncthreads();
+    const int half = nchunks / 2;
+    for (int dir = 0; dir < 2; ++dir) {
+        const int cnt = dir == 0 ? half : nchunks - half;
+        double carry = 0.0;
+        for (int base = 0; base < cnt; base += 1024) {
+            const int q = base + threadIdx.x;
+            const int i = dir == 0 ? q : nchunks - 1 - q;
+            double v = q < cnt ? s[i] : 0.0;
+            double incl = group_scan_incl<1024>(v, threadIdx.x, wsum);
+            if (q < cnt) s[i] = carry + incl - v;
+            if (threadIdx.x == 1023) tot = incl;
+            __syncthreads();
+            carry += tot;
+            __syncthreads();
+        }
     }
 }
 
 __global__ void __launch_bounds__(SC_NT)
 dst1_scanapply_kernel(int log2N, double* __restrict__ out, int64_t ld_out, const double* __restrict__ sums) {
     const int64_t L = (int64_t)1 << (log2N - 1);
+    const int nch = (int)(L / SC_CHUNK);
+    const bool fwd = (int)blockIdx.x < nch / 2;
     double* o = out + (int64_t)blockIdx.y * ld_out + 2 * (int64_t)blockIdx.x * SC_CHUNK;
+    const double* sc = sums + (int64_t)blockIdx.y * (nch + 1);
     __shared__ double wsum[32];
-    constexpr int PER = SC_CHUNK / SC_NT;          // 8 consecutive k's per thread
-    double loc[PER]; double run = 0.0;
+    constexpr int PER = SC_CHUNK / SC_NT;          // 8 consecutive positions of the (possibly reversed) chunk per thread
+    double loc[PER], val[PER]; double run = 0.0;
 #pragma unroll
-    for (int i = 0; i < PER; ++i) { run += o[2 * (threadIdx.x * PER + i)]; loc[i] = run; }
+    for (int i = 0; i < PER; ++i) {
+        const int q = threadIdx.x * PER + i;
+        val[i] = o[2 * (fwd ? q : SC_CHUNK - 1 - q)];
+        run += val[i]; loc[i] = run;
+    }
     double incl = group_scan_incl<SC_NT>(run, threadIdx.x, wsum);
-    double off = incl - run + sums[(int64_t)blockIdx.y * (L / SC_CHUNK) + blockIdx.x];
+    const double off = incl - run;
+    if (fwd) {
+        const double base = sc[blockIdx.x];
 #pragma unroll
-    for (int i = 0; i < PER; ++i) o[2 * (threadIdx.x * PER + i)] = loc[i] + off;
+        for (int i = 0; i < PER; ++i) o[2 * (threadIdx.x * PER + i)] = base + off + loc[i];                    // P_k
+    } else {
+        const double xl = sc[nch], above = sc[blockIdx.x];
+#pragma unroll
+        for (int i = 0; i < PER; ++i)                                // P_k = X_{N-1} - sum_{m > k} R_m
+            o[2 * (SC_CHUNK - 1 - (threadIdx.x * PER + i))] = xl - (above + (off + loc[i] - val[i]));
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ host side
@@ -285,12 +312,13 @@ int launch_pa(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in
     return LRP_OK;
 }
 template <int Q2, int TL>
-int launch_pb(lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale) {
+int launch_pb(lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale,
+              double* xlast, int xstride) {
     using C = PBCfg<Q2, TL>;
     LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pb_kernel<Q2, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     const int L1 = 1 << (log2N - 1 - Q2);
     LRP_PROF(ctx, K_DST_P2, 16.0 * ((int64_t)1 << log2N) * cols, 0);
-    dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, out, ld_out, scale);
+    dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, out, ld_out, scale, xlast, xstride);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
@@ -309,10 +337,11 @@ int dispatch_pa(int q1, int tl, lrp_ctx* ctx, int log2N, int cols, const double*
     if (q1 == 12) return launch_pa<12, 13>(ctx, log2N, cols, in, ld_in, W);
     LRP_QL_SWITCH(q1, 13, launch_pa, ctx, log2N, cols, in, ld_in, W)
 }
-int dispatch_pb(int q2, int tl, lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale) {
-    if (tl == 12) { LRP_QL_SWITCH(q2, 12, launch_pb, ctx, log2N, cols, W, out, ld_out, scale) }
-    if (q2 == 12) return launch_pb<12, 13>(ctx, log2N, cols, W, out, ld_out, scale);
-    LRP_QL_SWITCH(q2, 13, launch_pb, ctx, log2N, cols, W, out, ld_out, scale)
+int dispatch_pb(int q2, int tl, lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale,
+                double* xlast, int xstride) {
+    if (tl == 12) { LRP_QL_SWITCH(q2, 12, launch_pb, ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride) }
+    if (q2 == 12) return launch_pb<12, 13>(ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride);
+    LRP_QL_SWITCH(q2, 13, launch_pb, ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride)
 }
 
 // tile size and split: L = 2^q = L1 * L2 with both factors <= 2^(TL-1)
@@ -340,7 +369,7 @@ int group_cols(int64_t N, int batch) {
 size_t dst1_large_ws(int64_t N, int32_t batch) {
     const int g = group_cols(N, batch);
     const int64_t L = N / 2;
-    return lrp_align_up((size_t)g * L * sizeof(double2)) + lrp_align_up((size_t)g * (L / SC_CHUNK) * sizeof(double));
+    return lrp_align_up((size_t)g * L * sizeof(double2)) + lrp_align_up((size_t)g * (L / SC_CHUNK + 1) * sizeof(double));
 }
 
 int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
@@ -351,14 +380,14 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
     const int g = group_cols(N, batch);
     lrp_arena ar(ws, ws_bytes);
     double2* W = ar.take<double2>((size_t)g * L);
-    double* sums = ar.take<double>((size_t)g * (L / SC_CHUNK));
+    double* sums = ar.take<double>((size_t)g * (L / SC_CHUNK + 1));
     if (!ar.ok()) return LRP_ERR_WORKSPACE;
     const int nchunks = (int)(L / SC_CHUNK);
     for (int c0 = 0; c0 < batch; c0 += g) {
         const int cols = (batch - c0) < g ? (batch - c0) : g;
         double* o = d_out + (int64_t)c0 * ld_out;
         LRP_TRY(dispatch_pa(q1, tl, ctx, log2N, cols, d_in + (int64_t)c0 * ld_in, ld_in, W));
-        LRP_TRY(dispatch_pb(q2, tl, ctx, log2N, cols, W, o, ld_out, scale));
+        LRP_TRY(dispatch_pb(q2, tl, ctx, log2N, cols, W, o, ld_out, scale, sums + nchunks, nchunks + 1));
         LRP_PROF(ctx, K_DST_CHUNKSUM, 8.0 * N * cols, 0);
         dst1_chunksum_kernel<<<dim3(nchunks, cols), SC_NT, 0, ctx->stream>>>(log2N, o, ld_out, sums);
         LRP_LAUNCHED(ctx);
