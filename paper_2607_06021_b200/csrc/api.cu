@@ -112,9 +112,9 @@ int validate_indices(const int32_t* h, int cnt, int64_t n) {
 // ------------------------------------------------------------------------------------------------ solve workspace
 struct SolveWs {
     double *UhF, *VhF, *Cb, *Rb, *Ua, *Va, *Ub, *Vb, *scoresU, *scoresV;
-    double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev;
+    double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev, *Rlev2;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
-    unsigned char* mask;
+    unsigned char *mask, *mask2;
     void *sel_ws, *dst_ws;
     size_t eta_stride, dst_ws_bytes;
     ScrossWs sc;
@@ -128,7 +128,7 @@ struct SolveWs {
         Sprev = ar.take<double>(Kc);
         Amat = ar.take<double>((size_t)Kc * Kc); Bmat = ar.take<double>((size_t)Kc * Kc);
         GU = ar.take<double>((size_t)Kc * Kc); GV = ar.take<double>((size_t)Kc * Kc);
-        Rlev = ar.take<double>((size_t)Kc * Kc);
+        Rlev = ar.take<double>((size_t)Kc * Kc); Rlev2 = ar.take<double>((size_t)Kc * Kc);
         rho_out = ar.take<double>(8); eta = ar.take<double>(8);
         eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
         eta_work = ar.take<double>(2 * eta_stride);
@@ -137,7 +137,7 @@ struct SolveWs {
         gemmt_ws2 = ar.take<double>(tall_gemm_t_ws_doubles(ctx, n, Kc, Kc));
         dI = ar.take<int32_t>(Kc); dJ = ar.take<int32_t>(Kc); dIpr = ar.take<int32_t>(Kc); dJpr = ar.take<int32_t>(Kc);
         dIstar = ar.take<int32_t>(2 * (size_t)Kc + 8); dJstar = ar.take<int32_t>(2 * (size_t)Kc + 8);
-        mask = ar.take<unsigned char>(Kc);
+        mask = ar.take<unsigned char>(Kc); mask2 = ar.take<unsigned char>(Kc);
         sel_ws = ar.take<char>(select_ws_bytes(ctx, n, 2 * Kc + 1));
         int dcols = rF > max_rank ? rF : max_rank;
         dst_ws_bytes = lrp_dst1_ws_impl(n, dcols);
@@ -456,8 +456,14 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         // ---- O6/O7: selection, union, safeguard
         if (!replay) {
             if (k == 0) {
-                LRP_TRY(leverage_scores_qr(ctx, n, sel_cols, selU, sel_ld, w.Cb, ld, w.Rlev, w.mask, w.sc.qr_ws, w.scoresU));
-                LRP_TRY(leverage_scores_qr(ctx, n, sel_cols, selV, sel_ld, w.Cb, ld, w.Rlev, w.mask, w.sc.qr_ws, w.scoresV));
+                // the two leverage QRs of the initial guess are independent: factored as a pair on the two streams
+                LRP_TRY(tall_copy(ctx, n, sel_cols, selU, sel_ld, w.Cb, ld));
+                LRP_TRY(tall_copy(ctx, n, sel_cols, selV, sel_ld, w.Rb, ld));
+                LRP_TRY(tall_qr_pair(ctx, n, sel_cols, w.Cb, ld, w.Rlev, sel_cols, w.sc.qr_ws, sel_cols, w.Rb, ld, w.Rlev2, sel_cols, w.sc.qr_ws2));
+                LRP_TRY(leverage_colmask(ctx, sel_cols, w.Rlev, sel_cols, LEV_COL_RCOND, w.mask));
+                LRP_TRY(tall_rownorm2(ctx, n, sel_cols, w.Cb, ld, w.mask, w.scoresU));
+                LRP_TRY(leverage_colmask(ctx, sel_cols, w.Rlev2, sel_cols, LEV_COL_RCOND, w.mask2));
+                LRP_TRY(tall_rownorm2(ctx, n, sel_cols, w.Rb, ld, w.mask2, w.scoresV));
             }
             int64_t numsel64 = (int64_t)sel_cols + p_os; if (numsel64 > n) numsel64 = n;
             if (numsel64 > 2 * (int64_t)Kc) numsel64 = 2 * (int64_t)Kc;
