@@ -197,8 +197,10 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
     c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
-    c->aux = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->pinned = nullptr;
+    c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr;
     if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->aux2, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join2, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
         cudaHostAlloc((void**)&c->pinned, 8192, cudaHostAllocDefault) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
@@ -212,6 +214,8 @@ int lrp_destroy(lrp_ctx* ctx) {
     if (!ctx) return LRP_OK;
     if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
+    if (ctx->aux2) cudaStreamDestroy(ctx->aux2);
+    if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
@@ -551,13 +555,17 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (h_trace_keepJ) memcpy(h_trace_keepJ + tr_offJ, keepJ.data(), kk);
         tr_offI += l; tr_offJ += kk; rep_offI += l; rep_offJ += kk;
         // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
-        // eta (two one-CTA Jacobi SVDs) runs on the auxiliary stream while the rho contractions fill the GPU
-        // (the auxiliary stream already holds the V-side rebuild; it additionally waits for the U-side rebuild)
+        // eta (two one-CTA Jacobi SVDs) runs on a third stream while the two rho contractions (main: U, auxiliary: V)
+        // fill the GPU
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        {
+        cudaStream_t side2 = ctx->prof_on ? ctx->stream : ctx->aux2;
+        {   // eta on the third stream: it needs both rebuilt factors (main: U, side: V)
             cudaStream_t main_stream = ctx->stream;
-            ctx->stream = side;
+            LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
+            LRP_CUDA(ctx, cudaStreamWaitEvent(side2, ctx->ev_fork, 0));
+            LRP_CUDA(ctx, cudaStreamWaitEvent(side2, ctx->ev_join, 0));
+            ctx->stream = side2;
             int rc_eta = LRP_OK;
             cudaError_t e1 = cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
             cudaError_t e2 = cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
@@ -568,7 +576,9 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
                 ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
                 rc_eta = eta_pair(ctx, ea);
             }
-            if (rc_eta == LRP_OK && r_prev > 0) {                   // V side of rho on the auxiliary stream as well
+            cudaError_t e4 = cudaEventRecord(ctx->ev_join2, ctx->stream);
+            ctx->stream = side;
+            if (rc_eta == LRP_OK && r_prev > 0) {                   // V side of rho on the auxiliary stream
                 rc_eta = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
                 TallGemmArgs g{};
                 g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
@@ -579,7 +589,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             cudaError_t e3 = cudaEventRecord(ctx->ev_join, ctx->stream);
             ctx->stream = main_stream;
             if (rc_eta < 0) return rc_eta;
-            if (e3 != cudaSuccess) { ctx->last_cuda = (int)e3; return LRP_ERR_CUDA; }
+            if (e3 != cudaSuccess || e4 != cudaSuccess) { ctx->last_cuda = (int)(e3 != cudaSuccess ? e3 : e4); return LRP_ERR_CUDA; }
         }
         RhoArgs ra{};
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
@@ -593,6 +603,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, r_prev, w.Cb, ld, r_prev, w.GU, r_prev, 0, w.gemmt_ws));
         }
         LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join2, 0));
         LRP_TRY(rho_small(ctx, ra));
         double h_rho[2], h_eta[2];
         LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));

@@ -36,7 +36,8 @@ struct lrp_ctx {
     int prof_pending;                     // kernel id whose start event is recorded, -1 if none
     lrp_prof prof[K_NUM];
     cudaStream_t aux;                     // library-owned second stream: independent sub-steps of a sweep overlap on it
-    cudaEvent_t ev_fork, ev_join;
+    cudaStream_t aux2;                    // third stream: the one-CTA eta SVDs beside the two rho contractions
+    cudaEvent_t ev_fork, ev_join, ev_join2;
     double* pinned;                       // 8 KB of pinned host memory for the small per-panel read-backs
     std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)
     std::vector<int>* ev_id;

@@ -13,6 +13,25 @@ namespace {
 constexpr int CORE_NT = 1024;
 constexpr int JACOBI_MAX_SWEEPS = 60;
 
+// 1/sqrt(x) and 1/x for normal positive x to ~1 ulp, branch free: the hardware seed (MUFU.RSQ64H / RCP64H, ~22 bits)
+// plus one cubically / two quadratically convergent correction steps.  The library routines cost ~3x the fp64
+// instructions (slow-path checks), and every lane of every warp of the Jacobi sweep executes them.
+__device__ __forceinline__ double fast_rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double r2 = y * y, e = fma(-x, r2, 1.0), t = fma(e, 0.375, 0.5), u = y * e;
+    return fma(t, u, y);
+}
+__device__ __forceinline__ double fast_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    e = fma(e, e, e);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
@@ -20,44 +39,75 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // One-sided Jacobi on A (m x n, m >= n, ld lda), accumulating the rotations into V (n x n, ld ldv, must be I on
-// entry).  Round-robin tournament ordering; one warp per column pair.  On exit A = U diag(s), columns orthogonal.
-__device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag) {
+// entry; V == nullptr: singular values only).  Round-robin tournament ordering; one warp per column pair.  On exit
+// A = U diag(s), columns orthogonal.  nrm2 (n doubles, shared or global): squared column norms, recomputed at the
+// start of every sweep and updated by the rotation formulas in between (al' = al - t ga, be' = be + t ga), with an
+// explicit recomputation whenever the update cancels (so a pair costs one dot product instead of three).
+__device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag, double* nrm2) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int np = (n + 1) & ~1;                 // players (padded to even)
     if (n < 2) return;
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
         if (tid == 0) *s_flag = 0;
+        for (int c = warp; c < n; c += nwarps) {
+            const double* ac = A + (size_t)c * lda;
+            double acc = 0.0;
+            for (int t = lane; t < m; t += 32) acc = fma(ac[t], ac[t], acc);
+            acc = warp_sum(acc);
+            if (lane == 0) nrm2[c] = acc;
+        }
         __syncthreads();
         for (int r = 0; r < np - 1; ++r) {
             for (int i = warp; i < np / 2; i += nwarps) {
                 int p, q;
                 if (i == 0) { p = np - 1; q = r; }
-                else { p = (r + i) % (np - 1); q = (r - i + (np - 1)) % (np - 1); }
+                else {
+                    p = r + i; if (p >= np - 1) p -= np - 1;
+                    q = r - i; if (q < 0) q += np - 1;
+                }
                 if (p > q) { int t = p; p = q; q = t; }
                 if (q >= n) continue;
                 double* ap = A + (size_t)p * lda;
                 double* aq = A + (size_t)q * lda;
-                double al = 0.0, be = 0.0, ga = 0.0;
+                double ga = 0.0;
+                for (int t = lane; t < m; t += 32) ga = fma(ap[t], aq[t], ga);
+                ga = warp_sum(ga);
+                const double al = nrm2[p], be = nrm2[q];
+                // converged pair: |ga| <= eps sqrt(al be)
+                if (ga == 0.0 || ga * ga <= (DBL_EPSILON * DBL_EPSILON) * (al * be)) continue;
+                // t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), zeta = (be - al) / (2 ga), without forming zeta:
+                // t = sign(d) g2 / (|d| + hypot(d, g2)), d = be - al, g2 = 2 ga;  c = 1/sqrt(1 + t^2), s = c t
+                const double dd = be - al, g2 = 2.0 * ga;
+                const double q2 = fma(dd, dd, g2 * g2);
+                const double hh = q2 * fast_rsqrt(q2);
+                const double tt = copysign(1.0, dd) * g2 * fast_rcp(fabs(dd) + hh);
+                const double c = fast_rsqrt(fma(tt, tt, 1.0)), s = c * tt;
+                double aln = fma(-tt, ga, al), ben = fma(tt, ga, be);
+                const bool redo = !(aln > 1e-4 * al) || !(ben > 1e-4 * be);      // cancellation: recompute exactly
+                double sa = 0.0, sb = 0.0;
                 for (int t = lane; t < m; t += 32) {
                     double x = ap[t], y = aq[t];
-                    al = fma(x, x, al); be = fma(y, y, be); ga = fma(x, y, ga);
+                    const double xn = c * x - s * y, yn = s * x + c * y;
+                    ap[t] = xn; aq[t] = yn;
+                    if (redo) { sa = fma(xn, xn, sa); sb = fma(yn, yn, sb); }
                 }
-                al = warp_sum(al); be = warp_sum(be); ga = warp_sum(ga);
-                if (ga == 0.0 || fabs(ga) <= DBL_EPSILON * sqrt(al * be)) continue;
-                double zeta = (be - al) / (2.0 * ga);
-                double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                double c = 1.0 / sqrt(1.0 + tt * tt), s = c * tt;
-                for (int t = lane; t < m; t += 32) {
-                    double x = ap[t], y = aq[t];
-                    ap[t] = c * x - s * y; aq[t] = s * x + c * y;
+                if (redo) {
+#pragma unroll
+                    for (int d = 16; d > 0; d >>= 1) {
+                        sa += __shfl_xor_sync(0xffffffffu, sa, d);
+                        sb += __shfl_xor_sync(0xffffffffu, sb, d);
+                    }
+                    aln = sa; ben = sb;
                 }
-                double* vp = V + (size_t)p * ldv;
-                double* vq = V + (size_t)q * ldv;
-                for (int t = lane; t < n; t += 32) {
-                    double x = vp[t], y = vq[t];
-                    vp[t] = c * x - s * y; vq[t] = s * x + c * y;
+                if (V != nullptr) {
+                    double* vp = V + (size_t)p * ldv;
+                    double* vq = V + (size_t)q * ldv;
+                    for (int t = lane; t < n; t += 32) {
+                        double x = vp[t], y = vq[t];
+                        vp[t] = c * x - s * y; vq[t] = s * x + c * y;
+                    }
                 }
-                if (lane == 0) *s_flag = 1;
+                if (lane == 0) { nrm2[p] = aln; nrm2[q] = ben; *s_flag = 1; }
             }
             __syncthreads();
         }
@@ -70,23 +120,25 @@ __device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv,
 // Thin SVD of M (m x n, ld ldm): U (m x p), s (p, descending), V (n x p), p = min(m, n).
 // work: max(m,n)*p + p*p + p doubles, iwork: p ints.  Columns of U for exactly-zero singular values are zero.
 __device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int ldu, double* s, double* V, int ldv,
-                        double* work, int* iwork, int* s_flag, double* sm = nullptr, int sm_doubles = 0) {
+                        double* work, int* iwork, int* s_flag, double* sm = nullptr, int sm_doubles = 0,
+                        bool vectors = true) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const bool tr = m < n;
     const int T = tr ? n : m, p = tr ? m : n;
     // the Jacobi working set (T x p columns + p x p rotations) lives in shared memory when it fits: every round of
     // the sweep is a dependent read-modify-write of two columns per warp, i.e. pure latency
-    const bool in_smem = sm != nullptr && (size_t)T * p + (size_t)p * p <= (size_t)sm_doubles;
+    const bool in_smem = sm != nullptr && (size_t)T * p + (size_t)p * p + (size_t)p <= (size_t)sm_doubles;
     double* A = in_smem ? sm : work;                 // T x p
     double* W = A + (size_t)T * p;                   // p x p
     double* sv = work + (size_t)T * p + (size_t)p * p; // p
+    double* nrm2 = in_smem ? W + (size_t)p * p : sv;   // p (running squared column norms of the sweep)
     for (int e = tid; e < T * p; e += nt) {
         int t = e % T, c = e / T;
         A[e] = tr ? M[c + (size_t)t * ldm] : M[t + (size_t)c * ldm];
     }
-    for (int e = tid; e < p * p; e += nt) W[e] = (e % p == e / p) ? 1.0 : 0.0;
+    if (vectors) for (int e = tid; e < p * p; e += nt) W[e] = (e % p == e / p) ? 1.0 : 0.0;
     __syncthreads();
-    cta_jacobi(A, T, T, p, W, p, s_flag);
+    cta_jacobi(A, T, T, p, vectors ? W : nullptr, p, s_flag, nrm2);
     __syncthreads();
     {   // column norms, one warp per column
         const int lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -104,6 +156,11 @@ __device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int l
         iwork[c] = rk;
     }
     __syncthreads();
+    if (!vectors) {                                              // singular values only
+        for (int c = tid; c < p; c += nt) s[iwork[c]] = sv[c];
+        __syncthreads();
+        return;
+    }
     double* Ubig = tr ? V : U; int ldbig = tr ? ldv : ldu;       // receives the normalised A columns (T rows)
     double* Usml = tr ? U : V; int ldsml = tr ? ldu : ldv;       // receives the rotation columns (p rows)
     for (int e = tid; e < T * p; e += nt) {
@@ -304,7 +361,7 @@ eta_kernel(EtaArgs a) {
     }
     __syncthreads();
     extern __shared__ __align__(16) double dyn_smem[];
-    cta_svd(X, nidx, nidx, r, Ux, nidx, sx, Vx, r, svdw, iwork, &s_flag, dyn_smem, a.smem_doubles);
+    cta_svd(X, nidx, nidx, r, Ux, nidx, sx, Vx, r, svdw, iwork, &s_flag, dyn_smem, a.smem_doubles, false);
     if (tid == 0) { double sm = sx[p - 1]; *out = sm == 0.0 ? INFINITY : 1.0 / sm; }
 }
 
@@ -383,7 +440,7 @@ size_t core_work_doubles(int k, int l) {
 }
 
 static size_t jacobi_smem_bytes(const lrp_ctx* ctx, int T, int p) {
-    size_t need = ((size_t)T * p + (size_t)p * p) * sizeof(double);
+    size_t need = ((size_t)T * p + (size_t)p * p + (size_t)p) * sizeof(double);
     size_t cap = (size_t)ctx->smem_optin > 2048 ? (size_t)ctx->smem_optin - 2048 : 0;
     return need <= cap ? need : 0;                 // 0: stay in global memory
 }
