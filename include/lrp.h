@@ -18,7 +18,8 @@
  *   - indices are 0-based int32_t (grid point i <-> 1-based frequency k = i + 1); sizes are int64_t/int32_t.
  *   - the library never allocates device memory for data: scratch comes from the workspace the caller
  *     hands to lrp_set_workspace (sized by the lrp_*_workspace_bytes functions).  Pointers must be
- *     8-byte aligned; the workspace must be 256-byte aligned.
+ *     8-byte aligned; the workspace must be 256-byte aligned.  (The ctx itself owns 780 bytes of device memory,
+ *     the arrival counters of its in-kernel reductions, and 8 KB of pinned host memory.)
  *   - every call enqueues on the ctx's stream.  lrp_dst1_batched, lrp_sample_fibers are asynchronous;
  *     lrp_leverage_select, lrp_scross and lrp_cross_deim_solve synchronise the stream internally where
  *     their control flow needs device results (documented per function) and are complete on return
@@ -64,6 +65,10 @@ int64_t lrp_launch_count(const lrp_ctx* ctx);
  * string), launch count, summed event time in ms (0 unless profiling was on), and the summed ALGORITHMIC bytes and
  * flops of those launches.  lrp_profile_reset zeroes the counters. */
 int lrp_profile_enable(lrp_ctx* ctx, int on);
+/* on = 2 records the same events WITHOUT serialising the library's streams; lrp_profile_timeline then writes one
+ * line per launch since the last reset (kernel class, start and end in ms after the first launch) to a CSV file: the
+ * timeline of the real multi-stream run (per-class ms of overlapping kernels are then not additive). */
+int lrp_profile_timeline(lrp_ctx* ctx, const char* path);
 int lrp_profile_reset(lrp_ctx* ctx);
 int lrp_profile_count(void);
 int lrp_profile_get(lrp_ctx* ctx, int i, const char** name, int64_t* count, double* ms, double* bytes, double* flops);

@@ -2,6 +2,7 @@
 // Host control flow only decides sets of a few hundred integers and a handful of scalars per sweep
 // (union / safeguard / prune / stop test); every step that touches an n-long axis is a kernel.
 #include "common.cuh"
+#include <cstdio>
 #include "tall.cuh"
 #include "qr.cuh"
 #include "core.cuh"
@@ -197,13 +198,15 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
     c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
-    c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr;
+    c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr; c->d_counters = nullptr;
     if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->aux2, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join2, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
-        cudaHostAlloc((void**)&c->pinned, 8192, cudaHostAllocDefault) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
+        cudaHostAlloc((void**)&c->pinned, 8192, cudaHostAllocDefault) != cudaSuccess ||
+        cudaMalloc((void**)&c->d_counters, 3 * 65 * sizeof(unsigned)) != cudaSuccess ||
+        cudaMemset(c->d_counters, 0, 3 * 65 * sizeof(unsigned)) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     *out = c;
@@ -213,6 +216,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
 int lrp_destroy(lrp_ctx* ctx) {
     if (!ctx) return LRP_OK;
     if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
+    if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     if (ctx->aux2) cudaStreamDestroy(ctx->aux2);
     if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);
@@ -226,7 +230,23 @@ int lrp_destroy(lrp_ctx* ctx) {
 
 int lrp_profile_enable(lrp_ctx* ctx, int on) {
     if (!ctx) return LRP_ERR_BADARG;
-    ctx->prof_on = on ? 1 : 0;
+    ctx->prof_on = on == 2 ? 2 : (on ? 1 : 0);           // 1: serial streams, clean per-kernel times; 2: timeline of the real run
+    return LRP_OK;
+}
+
+int lrp_profile_timeline(lrp_ctx* ctx, const char* path) {
+    if (!ctx || !path) return LRP_ERR_BADARG;
+    LRP_CUDA(ctx, cudaDeviceSynchronize());
+    FILE* f = fopen(path, "w");
+    if (!f) return LRP_ERR_BADARG;
+    fprintf(f, "kernel,start_ms,end_ms\n");
+    for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+        float t0 = 0.f, t1 = 0.f;
+        if (cudaEventElapsedTime(&t0, (*ctx->ev)[0], (*ctx->ev)[i]) == cudaSuccess &&
+            cudaEventElapsedTime(&t1, (*ctx->ev)[0], (*ctx->ev)[i + 1]) == cudaSuccess)
+            fprintf(f, "%s,%.4f,%.4f\n", LRP_KERNEL_NAMES[(*ctx->ev_id)[i / 2]], t0, t1);
+    }
+    fclose(f);
     return LRP_OK;
 }
 
@@ -517,7 +537,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         // ---- O4: fibers  C = G(:,J) (n x kk), Rt = G(I,:)^T (n x l)
         // the two sides of a sweep are independent until the small core: they run on the main and the auxiliary stream
         // (every tall kernel here is latency-bound well below the HBM peak, so two in flight overlap usefully)
-        cudaStream_t side = ctx->prof_on ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
+        cudaStream_t side = ctx->prof_on == 1 ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ, kk, w.Cb, ld));
@@ -559,7 +579,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         // fill the GPU
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        cudaStream_t side2 = ctx->prof_on ? ctx->stream : ctx->aux2;
+        cudaStream_t side2 = ctx->prof_on == 1 ? ctx->stream : ctx->aux2;
         {   // eta on the third stream: it needs both rebuilt factors (main: U, side: V)
             cudaStream_t main_stream = ctx->stream;
             LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));

@@ -38,6 +38,7 @@ struct lrp_ctx {
     cudaStream_t aux;                     // library-owned second stream: independent sub-steps of a sweep overlap on it
     cudaStream_t aux2;                    // third stream: the one-CTA eta SVDs beside the two rho contractions
     cudaEvent_t ev_fork, ev_join, ev_join2;
+    unsigned* d_counters;                 // 3 x 65 arrival counters (one set per stream) of the in-kernel reductions; zero between launches
     double* pinned;                       // 8 KB of pinned host memory for the small per-panel read-backs
     std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)
     std::vector<int>* ev_id;

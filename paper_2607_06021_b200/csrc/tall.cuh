@@ -21,10 +21,12 @@ struct TallGemmArgs {
 };
 
 int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p);
-// S(k x m, ld lds) (+)= A(n x k)^T B(n x m); partial_ws: tall_gemm_t_ws_doubles(ctx, n, k, m) doubles of scratch
+// S(k x m, ld lds) (+)= A(n x k)^T B(n x m); partial_ws: tall_gemm_t_ws_doubles(ctx, n, k, m) doubles of scratch.
+// Sadd (optional, ld ldadd) += the same product (the accumulated Gram-Schmidt coefficients).  One launch: the
+// reduction over row slabs happens inside the kernel.
 size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m);
 int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
-                double* S, int64_t lds, int accumulate, double* partial_ws);
+                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd = nullptr, int64_t ldadd = 0);
 int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, const unsigned char* colmask, double* out);
 int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const int32_t* idx, int nidx, double* Out, int ldo);
 int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb);

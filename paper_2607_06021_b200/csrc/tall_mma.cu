@@ -144,12 +144,16 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
 // ---- S = A^T B: 8 warps per CTA; the CTA owns ntc <= 8 tiles (16 x 16) of S and its row slab; the 8/ntc warps
 //      that share a tile split the slab's rows and are summed through shared memory in a fixed order -------------
 constexpr int MT_THREADS = 256;
+constexpr int GT_GROUP = 16;                          // row slabs per first-level reduction group
+constexpr int GT_MAXGRP = 64;                         // counters [0, 64): groups, [64]: the final level
+struct GemmTOut { double* S; int64_t lds; int accumulate; double* Sadd; int64_t ldadd; double* gpartial; unsigned* counters; };
 
 template <bool VEC>
 __global__ void __launch_bounds__(MT_THREADS)
 tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const double* __restrict__ B, int64_t ldb, int m,
-                       int64_t n, int64_t rows_per_cta, double* __restrict__ partial, int na, int nb, int ntc) {
+                       int64_t n, int64_t rows_per_cta, double* partial, int na, int nb, int ntc, GemmTOut o) {
     __shared__ double red[MT_THREADS / 32][8][32];
+    __shared__ int s_role;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, tg = lane & 3;
     const int nsub = (MT_THREADS / 32) / ntc;               // warps per tile
     const int tl = warp % ntc, sub = warp / ntc;
@@ -204,36 +208,69 @@ tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const d
 #pragma unroll
             for (int e = 0; e < 2; ++e) red[warp][(i * 2 + j) * 2 + e][lane] = acc[i][j][e];
     __syncthreads();
-    if (sub != 0 || tile >= na * nb) return;
-    double* P = partial + (int64_t)blockIdx.x * k * m;
+    if (sub == 0 && tile < na * nb) {
+        double* P = partial + (int64_t)blockIdx.x * k * m;
 #pragma unroll
-    for (int i = 0; i < 2; ++i)
+        for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
+            for (int j = 0; j < 2; ++j)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                double v = 0.0;
-                for (int s2 = 0; s2 < nsub; ++s2) v += red[tl + s2 * ntc][(i * 2 + j) * 2 + e][lane];
-                int a = a0 + 8 * i + g, b = b0 + 8 * j + 2 * tg + e;
-                if (a < k && b < m) P[a + (int64_t)b * k] = v;
-            }
-}
-
-// S(a,b) = sum_blk partial[blk](a,b) (+ S(a,b) if accumulate), fixed summation order (deterministic)
-__global__ void reduce_partials_kernel(const double* __restrict__ partial, int nblk, int k, int m,
-                                       double* __restrict__ S, int64_t lds, int accumulate) {
-    const int part = threadIdx.x & 7;                       // 8 lanes per output element, fixed order -> deterministic
-    const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;
-    const bool ok = e < k * m;
-    double s = 0.0;
-    if (ok) for (int b = part; b < nblk; b += 8) s += partial[(int64_t)b * k * m + e];
-    s += __shfl_xor_sync(0xffffffffu, s, 1);
-    s += __shfl_xor_sync(0xffffffffu, s, 2);
-    s += __shfl_xor_sync(0xffffffffu, s, 4);
-    if (!ok || part != 0) return;
-    int a = e % k, c = e / k;
-    double* o = S + a + (int64_t)c * lds;
-    *o = accumulate ? (*o + s) : s;
+                for (int e = 0; e < 2; ++e) {
+                    double v = 0.0;
+                    for (int s2 = 0; s2 < nsub; ++s2) v += red[tl + s2 * ntc][(i * 2 + j) * 2 + e][lane];
+                    int a = a0 + 8 * i + g, b = b0 + 8 * j + 2 * tg + e;
+                    if (a < k && b < m) P[a + (int64_t)b * k] = v;
+                }
+    }
+    // ---- in-kernel reduction over the row slabs, two levels, fixed summation order (deterministic): the last CTA to
+    // finish in a group of GT_GROUP slabs sums the group's partials, the last group to finish sums the groups and
+    // writes S.  No second launch: a small dependent kernel queues behind whatever the other streams have in flight.
+    // The counters return to zero, so they are initialised once per context.
+    const int km = k * m;
+    const int grp = blockIdx.x / GT_GROUP;
+    const int g_lo = grp * GT_GROUP, g_hi = min(g_lo + GT_GROUP, (int)gridDim.x);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(&o.counters[grp], 1u);
+        int role = 0;
+        if (t == (unsigned)((g_hi - g_lo) * gridDim.y) - 1u) { o.counters[grp] = 0u; role = 1; }
+        s_role = role;
+    }
+    __syncthreads();
+    if (s_role == 0) return;
+    __threadfence();
+    double* gp = o.gpartial + (int64_t)grp * km;
+    for (int e = threadIdx.x; e < km; e += MT_THREADS) {
+        double v0 = 0.0, v1 = 0.0;
+        int b = g_lo;
+        for (; b + 1 < g_hi; b += 2) { v0 += __ldcg(partial + (int64_t)b * km + e); v1 += __ldcg(partial + (int64_t)(b + 1) * km + e); }
+        if (b < g_hi) v0 += __ldcg(partial + (int64_t)b * km + e);
+        gp[e] = v0 + v1;
+    }
+    __threadfence();
+    __syncthreads();
+    const int ngrp = (gridDim.x + GT_GROUP - 1) / GT_GROUP;
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(&o.counters[GT_MAXGRP], 1u);
+        int role = 1;
+        if (t == (unsigned)ngrp - 1u) { o.counters[GT_MAXGRP] = 0u; role = 2; }
+        s_role = role;
+    }
+    __syncthreads();
+    if (s_role != 2) return;
+    __threadfence();
+    for (int e = threadIdx.x; e < km; e += MT_THREADS) {
+        double v0 = 0.0, v1 = 0.0;
+        int q = 0;
+        for (; q + 1 < ngrp; q += 2) { v0 += __ldcg(o.gpartial + (int64_t)q * km + e); v1 += __ldcg(o.gpartial + (int64_t)(q + 1) * km + e); }
+        if (q < ngrp) v0 += __ldcg(o.gpartial + (int64_t)q * km + e);
+        const double v = v0 + v1;
+        const int a = e % k, c = e / k;
+        double* dst = o.S + a + (int64_t)c * o.lds;
+        *dst = o.accumulate ? (*dst + v) : v;
+        if (o.Sadd) o.Sadd[a + (int64_t)c * o.ldadd] += v;
+    }
 }
 
 }  // namespace
@@ -274,27 +311,31 @@ static int tall_gemm_t_nblk(int64_t n, int k, int m) {
 
 size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m) {
     (void)ctx;
-    return (size_t)tall_gemm_t_nblk(n, k, m) * k * m;
+    return ((size_t)tall_gemm_t_nblk(n, k, m) + GT_MAXGRP) * k * m;      // slab partials + group partials
 }
 
 int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
-                double* S, int64_t lds, int accumulate, double* partial_ws) {
+                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd, int64_t ldadd) {
     if (k <= 0 || m <= 0) return LRP_OK;
     int nblk = tall_gemm_t_nblk(n, k, m);
+    const int nblk_max = nblk;
     const int ntc = tall_gemm_t_ntc(k, m);
     int64_t rows_per = (n + nblk - 1) / nblk;
     rows_per = (rows_per + 15) / 16 * 16;
     nblk = (int)((n + rows_per - 1) / rows_per);
     const int na = (k + 15) / 16, nb = (m + 15) / 16;
     dim3 grid(nblk, (na * nb + ntc - 1) / ntc);
+    if ((nblk + GT_GROUP - 1) / GT_GROUP > GT_MAXGRP) return LRP_ERR_BADARG;
+    GemmTOut o{};
+    o.S = S; o.lds = lds; o.accumulate = accumulate; o.Sadd = Sadd; o.ldadd = ldadd;
+    o.gpartial = partial_ws + (size_t)nblk_max * k * m;
+    // one counter set per library stream: launches on a stream are ordered, the counters are back at zero when a launch ends
+    const int slot = ctx->stream == ctx->aux ? 1 : (ctx->stream == ctx->aux2 ? 2 : 0);
+    o.counters = ctx->d_counters + slot * (GT_MAXGRP + 1);
     LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
     const bool vec = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) & 15u) == 0;
-    if (vec) tall_gemm_t_mma_kernel<true><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
-    else tall_gemm_t_mma_kernel<false><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc);
-    LRP_LAUNCHED(ctx);
-    int tot = k * m;
-    LRP_PROF(ctx, K_REDUCE, 8.0 * nblk * k * m, 0);
-    reduce_partials_kernel<<<(tot * 8 + 127) / 128, 128, 0, ctx->stream>>>(partial_ws, nblk, k, m, S, lds, accumulate);
+    if (vec) tall_gemm_t_mma_kernel<true><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);
+    else tall_gemm_t_mma_kernel<false><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }

@@ -25,7 +25,8 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_workspace_bytes", "lrp_dst1_workspace_bytes", "lrp_leverage_workspace_bytes",
            "lrp_scross_workspace_bytes", "lrp_set_workspace", "lrp_dst1_batched", "lrp_sample_fibers",
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
-           "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get"]
+           "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
+           "lrp_profile_timeline"]
 
 
 class SolveOpts(C.Structure):
@@ -85,6 +86,7 @@ def load_library():
     lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_lowrank_entries.restype = C.c_int
     lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
+    lib.lrp_profile_timeline.argtypes = [vp, C.c_char_p]; lib.lrp_profile_timeline.restype = C.c_int
     lib.lrp_profile_reset.argtypes = [vp]; lib.lrp_profile_reset.restype = C.c_int
     lib.lrp_profile_count.argtypes = []; lib.lrp_profile_count.restype = C.c_int
     lib.lrp_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(dbl),
@@ -168,8 +170,12 @@ class Context:
     def launch_count(self) -> int:
         return int(self.lib.lrp_launch_count(self.h))
 
-    def profile_enable(self, on: bool):
+    def profile_enable(self, on):
+        """on = True/1: per-kernel times with the library's streams serialised; on = 2: timeline mode (real overlap)."""
         self._check(self.lib.lrp_profile_enable(self.h, int(on)), "lrp_profile_enable")
+
+    def profile_timeline(self, path: str):
+        self._check(self.lib.lrp_profile_timeline(self.h, path.encode()), "lrp_profile_timeline")
 
     def profile_reset(self):
         self._check(self.lib.lrp_profile_reset(self.h), "lrp_profile_reset")
