@@ -549,11 +549,6 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, w.Rb, ld, l, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
         cudaEvent_t e4 = ep.rec(ctx);
         const int p = kk < l ? kk : l;
-        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
-        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        LRP_TRY(rebuild(ctx, n, w.Cb, ld, kk, w.sc.Uc, kk, rank, Uk, ld, w.scoresU));
-        LRP_ON_STREAM(ctx, side, rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
-        cudaEvent_t e5 = ep.rec(ctx);
         // ---- O9: prune (Alg. 4 lines 14-23; reading Q12)
         keepI.assign(l, 1); keepJ.assign(kk, 1);
         if (replay && opts->h_replay_keepI && opts->h_replay_keepJ) {
@@ -574,17 +569,14 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (h_trace_keepI) memcpy(h_trace_keepI + tr_offI, keepI.data(), l);
         if (h_trace_keepJ) memcpy(h_trace_keepJ + tr_offJ, keepJ.data(), kk);
         tr_offI += l; tr_offJ += kk; rep_offI += l; rep_offJ += kk;
-        // ---- O10: rho (factored, reading Q13), eta (reading Q14), indicator
-        // eta (two one-CTA Jacobi SVDs) runs on a third stream while the two rho contractions (main: U, auxiliary: V)
-        // fill the GPU
+        // ---- eta (reading Q14) from the factored form U(I,:) = Q(I,:) Uc: two one-CTA Jacobi SVDs on the third stream,
+        // started before the rebuild so that they hide behind it (and behind the rho contractions of later sweeps)
+        cudaStream_t side2 = ctx->prof_on == 1 ? ctx->stream : ctx->aux2;
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        cudaStream_t side2 = ctx->prof_on == 1 ? ctx->stream : ctx->aux2;
-        {   // eta on the third stream: it needs both rebuilt factors (main: U, side: V)
+        LRP_CUDA(ctx, cudaStreamWaitEvent(side2, ctx->ev_fork, 0));
+        {
             cudaStream_t main_stream = ctx->stream;
-            LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
-            LRP_CUDA(ctx, cudaStreamWaitEvent(side2, ctx->ev_fork, 0));
-            LRP_CUDA(ctx, cudaStreamWaitEvent(side2, ctx->ev_join, 0));
             ctx->stream = side2;
             int rc_eta = LRP_OK;
             cudaError_t e1 = cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
@@ -592,30 +584,42 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             if (e1 != cudaSuccess || e2 != cudaSuccess) { ctx->last_cuda = (int)(e1 != cudaSuccess ? e1 : e2); rc_eta = LRP_ERR_CUDA; }
             if (rc_eta == LRP_OK) {
                 EtaArgs ea{};
-                ea.r = rank; ea.U = Uk; ea.ldu = ld; ea.I = w.dIpr; ea.nI = (int)I_pr.size(); ea.V = Vk; ea.ldv = ld; ea.J = w.dJpr; ea.nJ = (int)J_pr.size();
+                ea.r = rank; ea.U = w.Cb; ea.ldu = ld; ea.I = w.dIpr; ea.nI = (int)I_pr.size(); ea.V = w.Rb; ea.ldv = ld; ea.J = w.dJpr; ea.nJ = (int)J_pr.size();
+                ea.CU = w.sc.Uc; ea.kU = kk; ea.ldcu = kk; ea.CV = w.sc.Vc; ea.kV = l; ea.ldcv = l;
                 ea.eta = w.eta; ea.work = w.eta_work; ea.work_stride = w.eta_stride; ea.iwork = w.eta_iwork; ea.iwork_stride = Kc;
                 rc_eta = eta_pair(ctx, ea);
             }
             cudaError_t e4 = cudaEventRecord(ctx->ev_join2, ctx->stream);
-            ctx->stream = side;
-            if (rc_eta == LRP_OK && r_prev > 0) {                   // V side of rho on the auxiliary stream
-                rc_eta = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
-                TallGemmArgs g{};
-                g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
-                g.Cin = Vp; g.ldc = ld; g.Out = w.Rb; g.ldo = ld;       // fiber buffers are free after the rebuild
-                if (rc_eta >= 0) rc_eta = tall_gemm(ctx, g);
-                if (rc_eta >= 0) rc_eta = tall_gemm_t(ctx, n, w.Rb, ld, r_prev, w.Rb, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
-            }
-            cudaError_t e3 = cudaEventRecord(ctx->ev_join, ctx->stream);
             ctx->stream = main_stream;
             if (rc_eta < 0) return rc_eta;
-            if (e3 != cudaSuccess || e4 != cudaSuccess) { ctx->last_cuda = (int)(e3 != cudaSuccess ? e3 : e4); return LRP_ERR_CUDA; }
+            if (e4 != cudaSuccess) { ctx->last_cuda = (int)e4; return LRP_ERR_CUDA; }
         }
+        LRP_TRY(rebuild(ctx, n, w.Cb, ld, kk, w.sc.Uc, kk, rank, Uk, ld, w.scoresU));
+        LRP_ON_STREAM(ctx, side, rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
+        cudaEvent_t e5 = ep.rec(ctx);
+        // ---- O10: rho (factored, reading Q13), indicator.  The two sides run on the main and the auxiliary stream; their
+        // update kernels overwrite the fiber buffers (free after the rebuild), which eta still reads: they wait for it.
+        if (r_prev > 0) {
+            cudaStream_t main_stream = ctx->stream;
+            ctx->stream = side;
+            int rc_v = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
+            cudaError_t ew = cudaStreamWaitEvent(side, ctx->ev_join2, 0);
+            TallGemmArgs g{};
+            g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
+            g.Cin = Vp; g.ldc = ld; g.Out = w.Rb; g.ldo = ld;
+            if (rc_v >= 0 && ew == cudaSuccess) rc_v = tall_gemm(ctx, g);
+            if (rc_v >= 0 && ew == cudaSuccess) rc_v = tall_gemm_t(ctx, n, w.Rb, ld, r_prev, w.Rb, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
+            ctx->stream = main_stream;
+            if (rc_v < 0) return rc_v;
+            if (ew != cudaSuccess) { ctx->last_cuda = (int)ew; return LRP_ERR_CUDA; }
+        }
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
         RhoArgs ra{};
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
         ra.out = w.rho_out;
         if (r_prev > 0) {
             LRP_TRY(tall_gemm_t(ctx, n, Uk, ld, rank, Up, ld, r_prev, w.Amat, rank, 0, w.gemmt_ws));      // U side
+            LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join2, 0));
             TallGemmArgs g{};
             g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Uk; g.lda = ld; g.B = w.Amat; g.ldb = rank;
             g.Cin = Up; g.ldc = ld; g.Out = w.Cb; g.ldo = ld;

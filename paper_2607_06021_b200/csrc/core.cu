@@ -344,6 +344,7 @@ eta_kernel(EtaArgs a) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const double* F = side == 0 ? a.U : a.V; const int64_t ldf = side == 0 ? a.ldu : a.ldv;
     const int32_t* idx = side == 0 ? a.I : a.J; const int nidx = side == 0 ? a.nI : a.nJ;
+    const double* Cf = side == 0 ? a.CU : a.CV; const int kf = side == 0 ? a.kU : a.kV; const int64_t ldcf = side == 0 ? a.ldcu : a.ldcv;
     const int r = a.r;
     double* out = a.eta + side;
     if (nidx == 0 || r == 0) { if (tid == 0) *out = INFINITY; return; }
@@ -357,7 +358,12 @@ eta_kernel(EtaArgs a) {
     double* svdw = Vx + (size_t)r * p;
     for (int e = tid; e < nidx * r; e += nt) {
         int i = e % nidx, c = e / nidx;
-        X[e] = F[(int64_t)idx[i] + (int64_t)c * ldf];
+        if (Cf == nullptr) X[e] = F[(int64_t)idx[i] + (int64_t)c * ldf];
+        else {                                           // row idx[i] of (QF CF)(:, c)
+            double acc = 0.0;
+            for (int t = 0; t < kf; ++t) acc = fma(F[(int64_t)idx[i] + (int64_t)t * ldf], Cf[t + (int64_t)c * ldcf], acc);
+            X[e] = acc;
+        }
     }
     __syncthreads();
     extern __shared__ __align__(16) double dyn_smem[];

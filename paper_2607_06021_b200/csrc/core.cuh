@@ -23,6 +23,9 @@ struct EtaArgs {
     int r;
     const double* U; int64_t ldu; const int32_t* I; int nI;
     const double* V; int64_t ldv; const int32_t* J; int nJ;
+    // optional factored form: U = QU CU (QU n x kU passed as U/ldu, CU kU x r), likewise V -- eta can then start from
+    // the core's output, before the tall rebuild products exist
+    const double* CU; int kU; int64_t ldcu; const double* CV; int kV; int64_t ldcv;
     double* eta;                                // [2] device: eta1, eta2
     double* work; size_t work_stride; int32_t* iwork; size_t iwork_stride;
     int smem_doubles;
