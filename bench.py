@@ -133,6 +133,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--timeline", default="", help="also write the per-launch timeline (CSV) of one real multi-stream solve here")
     ap.add_argument("--dst-p", type=int, default=20, help="log2(n+1) of the batched DST-I side measurement")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -206,6 +207,12 @@ def main():
     R.barrier(dist)
     agg_e2e = R.throughput(dist, e2e_ms, float(n) ** 2 * steps, dev)
 
+    if args.timeline and rank == 0:                 # start/end of every launch of one solve, streams NOT serialised
+        ctx.profile_reset(); ctx.profile_enable(2)
+        step()
+        ctx.profile_timeline(args.timeline)
+        ctx.profile_enable(False); ctx.profile_reset()
+
     # ---- per-kernel profile (separate pass: events around every launch), roofline of the dominant kernel
     ctx.profile_reset(); ctx.profile_enable(True)
     nprof = 2
@@ -235,7 +242,7 @@ def main():
     # measured DRAM traffic of that kernel class from the committed ncu capture (ratio to its algorithmic bytes), per launch
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r01b_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r01c_traffic.csv")) as fh:
             for row in csv.DictReader(fh):
                 if row["kernel"] == top["kernel"]:
                     ratio = float(row["dram_bytes_per_launch"]) / float(row["alg_bytes_per_launch"])
