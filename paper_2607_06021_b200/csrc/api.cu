@@ -116,7 +116,7 @@ struct SolveWs {
     double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev, *Rlev2;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
     unsigned char *mask, *mask2;
-    void *sel_ws, *dst_ws;
+    void *sel_ws, *dst_ws, *dst_ws2;
     size_t eta_stride, dst_ws_bytes;
     ScrossWs sc;
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank) {
@@ -143,6 +143,7 @@ struct SolveWs {
         int dcols = rF > max_rank ? rF : max_rank;
         dst_ws_bytes = lrp_dst1_ws_impl(n, dcols);
         dst_ws = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
+        dst_ws2 = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
         bool ok = sc.carve(ar, ctx, n, Kc, Kc);
         return ok && ar.ok();
     }
@@ -457,8 +458,15 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     cudaEvent_t e_start = ep.rec(ctx);
 
     // O3: spectral RHS factors
-    LRP_TRY(lrp_dst1_impl(ctx, n, rF, d_UF, ldu, w.UhF, ld, scale, w.dst_ws, w.dst_ws_bytes));
-    LRP_TRY(lrp_dst1_impl(ctx, n, rF, d_VF, ldv, w.VhF, ld, scale, w.dst_ws, w.dst_ws_bytes));
+    {   // the two batched transforms are independent: main and auxiliary stream
+        cudaStream_t dside = ctx->prof_on == 1 ? ctx->stream : ctx->aux;
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(dside, ctx->ev_fork, 0));
+        LRP_TRY(lrp_dst1_impl(ctx, n, rF, d_UF, ldu, w.UhF, ld, scale, w.dst_ws, w.dst_ws_bytes));
+        LRP_ON_STREAM(ctx, dside, lrp_dst1_impl(ctx, n, rF, d_VF, ldv, w.VhF, ld, scale, w.dst_ws2, w.dst_ws_bytes));
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, dside));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    }
     cudaEvent_t e_dst = ep.rec(ctx);
     info->ms_dst_fwd = 0.f;
 
@@ -657,8 +665,15 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     if (r > r_prev) r = r_prev;
     if (r > max_rank) r = max_rank;
     cudaEvent_t e_inv0 = ep.rec(ctx);
-    LRP_TRY(lrp_dst1_impl(ctx, n, r, Up, ld, d_UW, lduw, scale, w.dst_ws, w.dst_ws_bytes));      // O12
-    LRP_TRY(lrp_dst1_impl(ctx, n, r, Vp, ld, d_VW, ldvw, scale, w.dst_ws, w.dst_ws_bytes));
+    {   // O12
+        cudaStream_t dside = ctx->prof_on == 1 ? ctx->stream : ctx->aux;
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(dside, ctx->ev_fork, 0));
+        LRP_TRY(lrp_dst1_impl(ctx, n, r, Up, ld, d_UW, lduw, scale, w.dst_ws, w.dst_ws_bytes));
+        LRP_ON_STREAM(ctx, dside, lrp_dst1_impl(ctx, n, r, Vp, ld, d_VW, ldvw, scale, w.dst_ws2, w.dst_ws_bytes));
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, dside));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    }
     LRP_CUDA(ctx, cudaMemcpyAsync(d_SW, w.Sprev, sizeof(double) * r, cudaMemcpyDeviceToDevice, ctx->stream));
     if (d_Uhat && d_Vhat && d_Shat && ld_hat >= n) {
         LRP_TRY(tall_copy(ctx, n, r_prev, Up, ld, d_Uhat, ld_hat));
