@@ -32,3 +32,8 @@ int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const in
 int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb);
 int tall_lowrank_entries(lrp_ctx* ctx, int r, const double* U, int64_t ldu, const double* S, const double* V, int64_t ldv,
                          const int64_t* rows, const int64_t* cols, int64_t count, double* out);
+
+// G (m x m) = E^T E with E = Cin - A B formed on the fly (never written).  Returns 1 (nothing launched) when the shape
+// is outside the fused kernel's range; partial_ws as for tall_gemm_t(n, m, m).
+int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb,
+                    const double* Cin, int64_t ldc, int m, double* G, int64_t ldg, double* partial_ws);

@@ -148,6 +148,59 @@ constexpr int GT_GROUP = 16;                          // row slabs per first-lev
 constexpr int GT_MAXGRP = 64;                         // counters [0, 64): groups, [64]: the final level
 struct GemmTOut { double* S; int64_t lds; int accumulate; double* Sadd; int64_t ldadd; double* gpartial; unsigned* counters; };
 
+// ---- in-kernel reduction over the row slabs, two levels, fixed summation order (deterministic): the last CTA to
+// finish in a group of GT_GROUP slabs sums the group's partials, the last group to finish sums the groups and writes
+// S.  No second launch: a small dependent kernel queues behind whatever the other streams have in flight.  The
+// counters return to zero, so they are initialised once per context.  Every thread of every CTA of the grid calls it
+// (gridDim.x slabs, gridDim.y CTAs per slab) after its slab's partial entries are written.
+__device__ __forceinline__ void slab_reduce_tail(double* partial, int k, int m, const GemmTOut& o, int* s_role) {
+    const int km = k * m, nthr = blockDim.x;
+    const int grp = blockIdx.x / GT_GROUP;
+    const int g_lo = grp * GT_GROUP, g_hi = min(g_lo + GT_GROUP, (int)gridDim.x);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(&o.counters[grp], 1u);
+        int role = 0;
+        if (t == (unsigned)((g_hi - g_lo) * gridDim.y) - 1u) { o.counters[grp] = 0u; role = 1; }
+        *s_role = role;
+    }
+    __syncthreads();
+    if (*s_role == 0) return;
+    __threadfence();
+    double* gp = o.gpartial + (int64_t)grp * km;
+    for (int e = threadIdx.x; e < km; e += nthr) {
+        double v0 = 0.0, v1 = 0.0;
+        int b = g_lo;
+        for (; b + 1 < g_hi; b += 2) { v0 += __ldcg(partial + (int64_t)b * km + e); v1 += __ldcg(partial + (int64_t)(b + 1) * km + e); }
+        if (b < g_hi) v0 += __ldcg(partial + (int64_t)b * km + e);
+        gp[e] = v0 + v1;
+    }
+    __threadfence();
+    __syncthreads();
+    const int ngrp = (gridDim.x + GT_GROUP - 1) / GT_GROUP;
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(&o.counters[GT_MAXGRP], 1u);
+        int role = 1;
+        if (t == (unsigned)ngrp - 1u) { o.counters[GT_MAXGRP] = 0u; role = 2; }
+        *s_role = role;
+    }
+    __syncthreads();
+    if (*s_role != 2) return;
+    __threadfence();
+    for (int e = threadIdx.x; e < km; e += nthr) {
+        double v0 = 0.0, v1 = 0.0;
+        int q = 0;
+        for (; q + 1 < ngrp; q += 2) { v0 += __ldcg(o.gpartial + (int64_t)q * km + e); v1 += __ldcg(o.gpartial + (int64_t)(q + 1) * km + e); }
+        if (q < ngrp) v0 += __ldcg(o.gpartial + (int64_t)q * km + e);
+        const double v = v0 + v1;
+        const int a = e % k, c = e / k;
+        double* dst = o.S + a + (int64_t)c * o.lds;
+        *dst = o.accumulate ? (*dst + v) : v;
+        if (o.Sadd) o.Sadd[a + (int64_t)c * o.ldadd] += v;
+    }
+}
+
 template <bool VEC>
 __global__ void __launch_bounds__(MT_THREADS)
 tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const double* __restrict__ B, int64_t ldb, int m,
@@ -222,55 +275,121 @@ tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const d
                     if (a < k && b < m) P[a + (int64_t)b * k] = v;
                 }
     }
-    // ---- in-kernel reduction over the row slabs, two levels, fixed summation order (deterministic): the last CTA to
-    // finish in a group of GT_GROUP slabs sums the group's partials, the last group to finish sums the groups and
-    // writes S.  No second launch: a small dependent kernel queues behind whatever the other streams have in flight.
-    // The counters return to zero, so they are initialised once per context.
-    const int km = k * m;
-    const int grp = blockIdx.x / GT_GROUP;
-    const int g_lo = grp * GT_GROUP, g_hi = min(g_lo + GT_GROUP, (int)gridDim.x);
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned t = atomicAdd(&o.counters[grp], 1u);
-        int role = 0;
-        if (t == (unsigned)((g_hi - g_lo) * gridDim.y) - 1u) { o.counters[grp] = 0u; role = 1; }
-        s_role = role;
+    slab_reduce_tail(partial, k, m, o, &s_role);
+}
+
+// ---- G = E^T E with E = Cin - A B (n x m) formed on the fly and never written: the rho update of the stop test
+//      (Alg. 4 line 24 in the factored form of DESIGN.md: E_U = U_{k-1} - U_k (U_k^T U_{k-1})).  One pass over A and Cin
+//      instead of an update sweep (read A, Cin, write E) plus a Gram sweep (read E).  Per warp and 32-row slab: E in the
+//      DMMA accumulators as in tall_gemm, through shared memory into fragment layout (the same registers serve as the
+//      A and the B operand of E^T E), upper-triangular 8 x 8 tiles of G accumulated over the CTA's slabs; per-CTA
+//      partials are reduced inside the kernel like those of tall_gemm_t.
+constexpr int RG_THREADS = 128;
+__host__ __device__ inline int rg_lde(int m8) { return m8 + (((4 - m8 % 16) + 16) % 16); }      // == 4 (mod 16): conflict-free fragments
+
+template <int NJ>
+__global__ void __launch_bounds__(RG_THREADS, NJ <= 5 ? 3 : 2)
+tall_resid_gram_kernel(int64_t n, const double* __restrict__ A, int64_t lda, int k, const double* __restrict__ B, int64_t ldb,
+                       const double* __restrict__ Cin, int64_t ldc, int m, double* partial, GemmTOut o) {
+    constexpr int NT2 = NJ * (NJ + 1) / 2;
+    extern __shared__ __align__(16) double smem[];
+    __shared__ int s_role;
+    const int kp = mg_kp(k), k4 = (k + 3) & ~3, lde = rg_lde(8 * NJ);
+    double* Bs = smem;                                            // [8 NJ][kp]
+    double* Es_all = smem + (size_t)8 * NJ * kp;                  // [4 warps][32][lde]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, tg = lane & 3;
+    double* Es = Es_all + (size_t)warp * 32 * lde;
+    for (int e = tid; e < 8 * NJ * k4; e += RG_THREADS) {
+        const int t = e % k4, c = e / k4;
+        Bs[c * kp + t] = (t < k && c < m) ? B[(int64_t)t + (int64_t)c * ldb] : 0.0;
     }
     __syncthreads();
-    if (s_role == 0) return;
-    __threadfence();
-    double* gp = o.gpartial + (int64_t)grp * km;
-    for (int e = threadIdx.x; e < km; e += MT_THREADS) {
-        double v0 = 0.0, v1 = 0.0;
-        int b = g_lo;
-        for (; b + 1 < g_hi; b += 2) { v0 += __ldcg(partial + (int64_t)b * km + e); v1 += __ldcg(partial + (int64_t)(b + 1) * km + e); }
-        if (b < g_hi) v0 += __ldcg(partial + (int64_t)b * km + e);
-        gp[e] = v0 + v1;
+    double gacc[NT2][2];
+#pragma unroll
+    for (int t = 0; t < NT2; ++t) { gacc[t][0] = 0.0; gacc[t][1] = 0.0; }
+    const int64_t nslab = (n + RG_THREADS - 1) / RG_THREADS;
+    for (int64_t slab = blockIdx.x; slab < nslab; slab += gridDim.x) {
+        const int64_t R0 = slab * RG_THREADS + warp * 32;
+        int64_t rows[4]; bool valid[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { rows[i] = R0 + 16 * (i >> 1) + 2 * g + (i & 1); valid[i] = rows[i] < n; }
+        double acc[4][NJ][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+#pragma unroll 4
+        for (int t0 = 0; t0 < k4; t0 += 4) {
+            const int t = t0 + tg;
+            double a[4], b[NJ];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                double2 v = make_double2(0.0, 0.0);
+                if (valid[2 * h] && t < k) v = *reinterpret_cast<const double2*>(A + rows[2 * h] + (int64_t)t * lda);
+                a[2 * h] = v.x; a[2 * h + 1] = valid[2 * h + 1] ? v.y : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) b[j] = Bs[(8 * j + g) * kp + t];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < NJ; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        // E = Cin - A B into the warp's shared-memory tile (rows local 16 (i>>1) + 2 g + (i&1)); invalid rows / columns are zero
+        __syncwarp();
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int col = 8 * j + 2 * tg + e;
+                    double2 cin = make_double2(0.0, 0.0);
+                    if (valid[2 * h] && col < m) cin = *reinterpret_cast<const double2*>(Cin + rows[2 * h] + (int64_t)col * ldc);
+                    const int rl = 16 * h + 2 * g;
+                    Es[rl * lde + col] = (valid[2 * h] && col < m) ? cin.x - acc[2 * h][j][e] : 0.0;
+                    Es[(rl + 1) * lde + col] = (valid[2 * h + 1] && col < m) ? cin.y - acc[2 * h + 1][j][e] : 0.0;
+                }
+        __syncwarp();
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            double f[NJ];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) f[j] = Es[(4 * ks + tg) * lde + 8 * j + g];
+            int t = 0;
+#pragma unroll
+            for (int mt = 0; mt < NJ; ++mt)
+#pragma unroll
+                for (int nt = mt; nt < NJ; ++nt, ++t) dmma(gacc[t][0], gacc[t][1], f[mt], f[nt]);
+        }
     }
-    __threadfence();
+    // CTA partial: warps summed in a fixed order through shared memory, both triangles written
     __syncthreads();
-    const int ngrp = (gridDim.x + GT_GROUP - 1) / GT_GROUP;
-    if (threadIdx.x == 0) {
-        const unsigned t = atomicAdd(&o.counters[GT_MAXGRP], 1u);
-        int role = 1;
-        if (t == (unsigned)ngrp - 1u) { o.counters[GT_MAXGRP] = 0u; role = 2; }
-        s_role = role;
+    double* red = Es_all;                                         // [4][NT2 * 2][32]
+    {
+#pragma unroll
+        for (int t = 0; t < NT2; ++t) { red[((size_t)warp * NT2 * 2 + 2 * t) * 32 + lane] = gacc[t][0]; red[((size_t)warp * NT2 * 2 + 2 * t + 1) * 32 + lane] = gacc[t][1]; }
     }
     __syncthreads();
-    if (s_role != 2) return;
-    __threadfence();
-    for (int e = threadIdx.x; e < km; e += MT_THREADS) {
-        double v0 = 0.0, v1 = 0.0;
-        int q = 0;
-        for (; q + 1 < ngrp; q += 2) { v0 += __ldcg(o.gpartial + (int64_t)q * km + e); v1 += __ldcg(o.gpartial + (int64_t)(q + 1) * km + e); }
-        if (q < ngrp) v0 += __ldcg(o.gpartial + (int64_t)q * km + e);
-        const double v = v0 + v1;
-        const int a = e % k, c = e / k;
-        double* dst = o.S + a + (int64_t)c * o.lds;
-        *dst = o.accumulate ? (*dst + v) : v;
-        if (o.Sadd) o.Sadd[a + (int64_t)c * o.ldadd] += v;
+    if (warp == 0) {
+        double* P = partial + (int64_t)blockIdx.x * m * m;
+        int t = 0;
+#pragma unroll
+        for (int mt = 0; mt < NJ; ++mt)
+#pragma unroll
+            for (int nt = mt; nt < NJ; ++nt, ++t)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    double v = 0.0;
+                    for (int w2 = 0; w2 < RG_THREADS / 32; ++w2) v += red[((size_t)w2 * NT2 * 2 + 2 * t + e) * 32 + lane];
+                    const int a = 8 * mt + g, b = 8 * nt + 2 * tg + e;
+                    if (a < m && b < m) {
+                        if (mt != nt || a <= b) P[a + (int64_t)b * m] = v;
+                        if (mt != nt || a < b) P[b + (int64_t)a * m] = v;
+                    }
+                }
     }
+    slab_reduce_tail(partial, m, m, o, &s_role);
 }
 
 }  // namespace
@@ -336,6 +455,41 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
     const bool vec = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) & 15u) == 0;
     if (vec) tall_gemm_t_mma_kernel<true><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);
     else tall_gemm_t_mma_kernel<false><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+
+// G (m x m, ld ldg) = E^T E, E = Cin - A B (B: k x m device, ld ldb), without writing E.  Returns 1 when the shape or
+// the alignment is outside the fused kernel's range (m > 64, odd leading dimensions): the caller then takes the
+// update + Gram sweeps.  partial_ws: tall_gemm_t_ws_doubles(ctx, n, m, m) doubles.
+int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb,
+                    const double* Cin, int64_t ldc, int m, double* G, int64_t ldg, double* partial_ws) {
+    if (k <= 0 || m <= 0) return 1;
+    const int NJ = (m + 7) / 8;
+    const bool vec = (lda % 2 == 0) && (ldc % 2 == 0) && ((((uintptr_t)A) | ((uintptr_t)Cin)) & 15u) == 0;
+    if (NJ > 8 || !vec) return 1;
+    int nblk = tall_gemm_t_nblk(n, m, m);                          // same partial geometry as tall_gemm_t
+    const int nblk_max = nblk;
+    const int64_t nslab = (n + RG_THREADS - 1) / RG_THREADS;
+    if (nblk > nslab) nblk = (int)nslab;
+    const size_t es = (size_t)4 * 32 * rg_lde(8 * NJ), rd = (size_t)4 * NJ * (NJ + 1) * 32;
+    const size_t smem = sizeof(double) * ((size_t)8 * NJ * mg_kp(k) + (es > rd ? es : rd));
+    if (smem > (size_t)ctx->smem_optin) return 1;
+    GemmTOut o{};
+    o.S = G; o.lds = ldg; o.accumulate = 0; o.Sadd = nullptr; o.ldadd = 0;
+    o.gpartial = partial_ws + (size_t)nblk_max * m * m;
+    const int slot = ctx->stream == ctx->aux ? 1 : (ctx->stream == ctx->aux2 ? 2 : 0);
+    o.counters = ctx->d_counters + slot * (GT_MAXGRP + 1);
+    void (*kern)(int64_t, const double*, int64_t, int, const double*, int64_t, const double*, int64_t, int, double*, GemmTOut) = nullptr;
+    switch (NJ) {
+        case 1: kern = tall_resid_gram_kernel<1>; break; case 2: kern = tall_resid_gram_kernel<2>; break;
+        case 3: kern = tall_resid_gram_kernel<3>; break; case 4: kern = tall_resid_gram_kernel<4>; break;
+        case 5: kern = tall_resid_gram_kernel<5>; break; case 6: kern = tall_resid_gram_kernel<6>; break;
+        case 7: kern = tall_resid_gram_kernel<7>; break; default: kern = tall_resid_gram_kernel<8>; break;
+    }
+    if (smem > 48 * 1024) LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LRP_PROF(ctx, K_GEMM_SUBTRACT, 8.0 * n * (k + m), 2.0 * n * m * (k + m));
+    kern<<<nblk, RG_THREADS, smem, ctx->stream>>>(n, A, lda, k, B, ldb, Cin, ldc, m, partial_ws, o);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
