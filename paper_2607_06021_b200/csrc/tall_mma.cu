@@ -8,6 +8,7 @@
 #include "common.cuh"
 #include "tall.cuh"
 #include <math.h>
+#include <stdlib.h>
 
 namespace {
 
@@ -408,7 +409,8 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
         LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
-    if (grid > 148 * 8) grid = 148 * 8;            // persistent over row slabs: B is staged once per column tile per CTA
+    const int64_t resident = 148 * (nj == 2 ? 5 : 4);   // persistent over row slabs (B staged once per column tile per CTA):
+    if (grid > resident) grid = resident;            // exactly one resident wave, so that the slabs are balanced
     LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
              8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
     kern<<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
@@ -422,7 +424,7 @@ static int tall_gemm_t_ntc(int k, int m) {       // tiles per CTA: 1, 2, 4 or 8 
 }
 static int tall_gemm_t_nblk(int64_t n, int k, int m) {
     (void)k; (void)m;
-    int64_t want = 148 * 4;                            // B200: 148 SMs; fixed so that workspace sizes need no device query
+    int64_t want = 148 * 3;                            // B200: 148 SMs x 3 resident CTAs (one wave); fixed: workspace sizes need no device query
     int64_t by_rows = (n + 511) / 512;
     int64_t nb = want < by_rows ? want : by_rows;
     return (int)(nb < 1 ? 1 : nb);
@@ -465,11 +467,13 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
 int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb,
                     const double* Cin, int64_t ldc, int m, double* G, int64_t ldg, double* partial_ws) {
     if (k <= 0 || m <= 0) return 1;
+    if (getenv("LRP_NO_FUSED_RHO")) return 1;                      // test hook: force the two-sweep path
     const int NJ = (m + 7) / 8;
     const bool vec = (lda % 2 == 0) && (ldc % 2 == 0) && ((((uintptr_t)A) | ((uintptr_t)Cin)) & 15u) == 0;
     if (NJ > 8 || !vec) return 1;
     int nblk = tall_gemm_t_nblk(n, m, m);                          // same partial geometry as tall_gemm_t
     const int nblk_max = nblk;
+    if (nblk > 148 * (NJ <= 5 ? 3 : 2)) nblk = 148 * (NJ <= 5 ? 3 : 2);   // one resident wave of the persistent CTAs
     const int64_t nslab = (n + RG_THREADS - 1) / RG_THREADS;
     if (nblk > nslab) nblk = (int)nslab;
     const size_t es = (size_t)4 * 32 * rg_lde(8 * NJ), rd = (size_t)4 * NJ * (NJ + 1) * 32;
@@ -488,7 +492,7 @@ int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k
         case 7: kern = tall_resid_gram_kernel<7>; break; default: kern = tall_resid_gram_kernel<8>; break;
     }
     if (smem > 48 * 1024) LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    LRP_PROF(ctx, K_GEMM_SUBTRACT, 8.0 * n * (k + m), 2.0 * n * m * (k + m));
+    LRP_PROF(ctx, K_RESID_GRAM, 8.0 * n * (k + m), 2.0 * n * m * (k + m));
     kern<<<nblk, RG_THREADS, smem, ctx->stream>>>(n, A, lda, k, B, ldb, Cin, ldc, m, partial_ws, o);
     LRP_LAUNCHED(ctx);
     return LRP_OK;

@@ -97,3 +97,20 @@ def test_set_cap_truncation_and_gpu_trace_replay(ctx):
     again = _solve(ctx, w, replay=rep, want_spectral=True)
     assert again["sweeps"] == res["sweeps"] and again["rank"] == res["rank"]
     assert torch.equal(again["Shat"], res["Shat"])
+
+
+def test_fused_and_two_sweep_stop_test_agree(ctx, monkeypatch):
+    """rho (Alg. 4 line 24) through the fused residual-Gram kernel (E = U_{k-1} - U_k A never written)
+    and through the update sweep + Gram sweep it replaces (shapes outside the fused kernel's range take that path):
+    the same sweeps, ranks and index decisions, rho equal to rounding of a sum of squares."""
+    w = W.make("C2", 3)
+    a = _solve(ctx, w)
+    monkeypatch.setenv("LRP_NO_FUSED_RHO", "1")
+    b = _solve(ctx, w)
+    monkeypatch.delenv("LRP_NO_FUSED_RHO")
+    assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
+    ia, ib = a["info"], b["info"]
+    for k in range(a["sweeps"]):
+        ra, rb = ia.rho_per_sweep[k], ib.rho_per_sweep[k]
+        assert abs(ra - rb) <= 1e-9 * max(abs(ra), abs(rb)) + 1e-13 * ia.snorm
+        assert ia.rank_per_sweep[k] == ib.rank_per_sweep[k] and ia.nI[k] == ib.nI[k] and ia.nJ[k] == ib.nJ[k]
