@@ -205,9 +205,11 @@ __device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb,
             double beta, tau, inv;
             if (sig == 0.0) { beta = alpha; tau = 0.0; inv = 0.0; }
             else {
-                beta = -copysign(sqrt(fma(alpha, alpha, sig)), alpha);
-                tau = (beta - alpha) / beta;
-                inv = 1.0 / (alpha - beta);
+                const double nrm2 = fma(alpha, alpha, sig), aa = fabs(alpha);
+                const double rs = fast_rsqrt(nrm2), mu = nrm2 * rs;          // |beta|
+                beta = -copysign(mu, alpha);
+                tau = fma(aa, rs, 1.0);                                      // (beta - alpha) / beta
+                inv = copysign(fast_rcp(aa + mu), alpha);                    // 1 / (alpha - beta)
             }
             for (int r = c + 1 + lane; r < rows; r += 32) xc[r] *= inv;       // v (unit diagonal implicit)
             if (lane == 0) { xc[c] = beta; s_scal[0] = tau; }
@@ -232,14 +234,22 @@ __device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb,
     }
     __syncthreads();
     if (*cond_flag) return;
-    for (int j = tid; j < nb; j += blockDim.x) {          // back substitution, one right-hand side per thread
-        const double* bj = W + (size_t)(xn + j) * ldw;
-        double* yj = Y + (size_t)j * ldy;
-        for (int i = xn - 1; i >= 0; --i) {
-            double acc = bj[i];
-            for (int t = i + 1; t < xn; ++t) acc = fma(-W[i + (size_t)t * ldw], yj[t], acc);
-            yj[i] = acc / W[i + (size_t)i * ldw];
+    // back substitution R Y = (Q^T B)(0:xn, :), column oriented and in place in W: step i fixes row i of Y for all
+    // right-hand sides, then removes its contribution from the rows above (xn steps of i * nb independent updates)
+    for (int i = xn - 1; i >= 0; --i) {
+        const double rii = W[i + (size_t)i * ldw];
+        for (int j = tid; j < nb; j += blockDim.x) W[i + (size_t)(xn + j) * ldw] /= rii;
+        __syncthreads();
+        for (int e = tid; e < i * nb; e += blockDim.x) {
+            const int t = e % i, j = e / i;
+            double* bj = W + (size_t)(xn + j) * ldw;
+            bj[t] = fma(-W[t + (size_t)i * ldw], bj[i], bj[t]);
         }
+        __syncthreads();
+    }
+    for (int e = tid; e < xn * nb; e += blockDim.x) {
+        const int i = e % xn, j = e / xn;
+        Y[i + (size_t)j * ldy] = W[i + (size_t)(xn + j) * ldw];
     }
     __syncthreads();
 }
