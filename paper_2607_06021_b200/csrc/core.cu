@@ -12,7 +12,6 @@ namespace {
 
 constexpr int CORE_NT = 1024;
 constexpr int JACOBI_MAX_SWEEPS = 60;
-constexpr int JR = 4;                        // rows per lane of the register path of the Jacobi sweep (m <= 128)
 
 // 1/sqrt(x) and 1/x for normal positive x to ~1 ulp, branch free: the hardware seed (MUFU.RSQ64H / RCP64H, ~22 bits)
 // plus one cubically / two quadratically convergent correction steps.  The library routines cost ~3x the fp64
@@ -37,6 +36,60 @@ __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
     return v;
+}
+
+// One pair (p, q) of the sweep with the two columns in registers (JR rows per lane: m <= 32 JR) from the dot product to
+// the rotated store -- one shared-memory read and one write per element.  Returns false when the pair is converged.
+template <int JR>
+__device__ __forceinline__ bool jacobi_pair_regs(double* ap, double* aq, int m, double* V, int ldv, int n, int p, int q,
+                                             double al, double be, int lane, double& aln_out, double& ben_out) {
+    double x[JR], y[JR];
+    double ga = 0.0;
+#pragma unroll
+    for (int u = 0; u < JR; ++u) {
+        const int t = lane + 32 * u;
+        x[u] = t < m ? ap[t] : 0.0; y[u] = t < m ? aq[t] : 0.0;
+        ga = fma(x[u], y[u], ga);
+    }
+    ga = warp_sum(ga);
+    if (ga == 0.0 || ga * ga <= (DBL_EPSILON * DBL_EPSILON) * (al * be)) return false;
+    const double dd = be - al, g2 = 2.0 * ga;
+    const double q2 = fma(dd, dd, g2 * g2);
+    const double hh = q2 * fast_rsqrt(q2);
+    const double tt = copysign(1.0, dd) * g2 * fast_rcp(fabs(dd) + hh);
+    const double c = fast_rsqrt(fma(tt, tt, 1.0)), s = c * tt;
+    double aln = fma(-tt, ga, al), ben = fma(tt, ga, be);
+    const bool redo = !(aln > 1e-4 * al) || !(ben > 1e-4 * be);  // cancellation: recompute exactly
+    double sa = 0.0, sb = 0.0;
+#pragma unroll
+    for (int u = 0; u < JR; ++u) {
+        const int t = lane + 32 * u;
+        const double xn = c * x[u] - s * y[u], yn = s * x[u] + c * y[u];
+        if (t < m) { ap[t] = xn; aq[t] = yn; }
+        sa = fma(xn, xn, sa); sb = fma(yn, yn, sb);
+    }
+    if (redo) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            sa += __shfl_xor_sync(0xffffffffu, sa, d);
+            sb += __shfl_xor_sync(0xffffffffu, sb, d);
+        }
+        aln = sa; ben = sb;
+    }
+    if (V != nullptr) {
+        double* vp = V + (size_t)p * ldv;
+        double* vq = V + (size_t)q * ldv;
+#pragma unroll
+        for (int u = 0; u < JR; ++u) {
+            const int t = lane + 32 * u;
+            if (t < n) {
+                const double xv = vp[t], yv = vq[t];
+                vp[t] = c * xv - s * yv; vq[t] = s * xv + c * yv;
+            }
+        }
+    }
+    aln_out = aln; ben_out = ben;
+    return true;
 }
 
 // One-sided Jacobi on A (m x n, m >= n, ld lda), accumulating the rotations into V (n x n, ld ldv, must be I on
@@ -71,54 +124,11 @@ __device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv,
                 double* ap = A + (size_t)p * lda;
                 double* aq = A + (size_t)q * lda;
                 const double al = nrm2[p], be = nrm2[q];
-                if (m <= 32 * JR) {
-                    // the usual case (K <= 128): the pair's two columns live in registers from the dot product to the
-                    // rotated store -- one shared-memory read and one write per element
-                    double x[JR], y[JR];
-                    double ga = 0.0;
-#pragma unroll
-                    for (int u = 0; u < JR; ++u) {
-                        const int t = lane + 32 * u;
-                        x[u] = t < m ? ap[t] : 0.0; y[u] = t < m ? aq[t] : 0.0;
-                        ga = fma(x[u], y[u], ga);
-                    }
-                    ga = warp_sum(ga);
-                    if (ga == 0.0 || ga * ga <= (DBL_EPSILON * DBL_EPSILON) * (al * be)) continue;
-                    const double dd = be - al, g2 = 2.0 * ga;
-                    const double q2 = fma(dd, dd, g2 * g2);
-                    const double hh = q2 * fast_rsqrt(q2);
-                    const double tt = copysign(1.0, dd) * g2 * fast_rcp(fabs(dd) + hh);
-                    const double c = fast_rsqrt(fma(tt, tt, 1.0)), s = c * tt;
-                    double aln = fma(-tt, ga, al), ben = fma(tt, ga, be);
-                    const bool redo = !(aln > 1e-4 * al) || !(ben > 1e-4 * be);  // cancellation: recompute exactly
-                    double sa = 0.0, sb = 0.0;
-#pragma unroll
-                    for (int u = 0; u < JR; ++u) {
-                        const int t = lane + 32 * u;
-                        const double xn = c * x[u] - s * y[u], yn = s * x[u] + c * y[u];
-                        if (t < m) { ap[t] = xn; aq[t] = yn; }
-                        sa = fma(xn, xn, sa); sb = fma(yn, yn, sb);
-                    }
-                    if (redo) {
-#pragma unroll
-                        for (int d = 16; d > 0; d >>= 1) {
-                            sa += __shfl_xor_sync(0xffffffffu, sa, d);
-                            sb += __shfl_xor_sync(0xffffffffu, sb, d);
-                        }
-                        aln = sa; ben = sb;
-                    }
-                    if (V != nullptr) {
-                        double* vp = V + (size_t)p * ldv;
-                        double* vq = V + (size_t)q * ldv;
-#pragma unroll
-                        for (int u = 0; u < JR; ++u) {
-                            const int t = lane + 32 * u;
-                            if (t < n) {
-                                const double xv = vp[t], yv = vq[t];
-                                vp[t] = c * xv - s * yv; vq[t] = s * xv + c * yv;
-                            }
-                        }
-                    }
+                if (m <= 128) {
+                    double aln, ben;
+                    const bool rot = m <= 64 ? jacobi_pair_regs<2>(ap, aq, m, V, ldv, n, p, q, al, be, lane, aln, ben)
+                                             : jacobi_pair_regs<4>(ap, aq, m, V, ldv, n, p, q, al, be, lane, aln, ben);
+                    if (!rot) continue;
                     if (lane == 0) { nrm2[p] = aln; nrm2[q] = ben; *s_flag = 1; }
                     continue;
                 }
