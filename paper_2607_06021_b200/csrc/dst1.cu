@@ -82,7 +82,7 @@ dst1_small_kernel(int batch, const double* __restrict__ in, int64_t ld_in,
     if (gt == 0) ((L & 1) ? im : re)[PADI(L >> 1)] = 2.0 * xmid;     // t_L = 2 x_L
     __syncthreads();
 
-    fft_smem<Q>(re, im, gt, lo, hi, 4);                              // exp(-2 pi i mm/L) = tw(4 mm)
+    fft_smem<Q, C::CPB>(re, im, gt, g, lo, hi, 4);                              // exp(-2 pi i mm/L) = tw(4 mm)
 
     // untangle: pairs (k, L-k), k = 0 .. L/2
     for (int k = gt; k <= L / 2; k += GS) {

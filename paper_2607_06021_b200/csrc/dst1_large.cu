@@ -6,16 +6,20 @@
 //            so each element is fetched from HBM once), length-L1 FFTs over the strided index j1, four-step twiddle,
 //            W[k1*L2 + j2] (complex, 8N bytes per column);
 //   sweep B: the CTA owns T rows k1 and their mirror rows L1 - k1: length-L2 FFTs, real-FFT untangle of the pairs
-//            (k, L-k) in shared memory, writes X_{2k} (final) and R_k = X_{2k+1} - X_{2k-1} in natural order;
-//   sweep C: in-place prefix sum over the odd outputs (chunk sums, scan of the chunk sums, apply).
-// Columns are processed in groups whose W + output footprint stays L2-resident, so that ideally only the read of x
-// and the final write of the output reach HBM.
+//            (k, L-k) in shared memory; (R_k, X_{2k}) with R_k = X_{2k+1} - X_{2k-1} go back IN PLACE into the rows of W
+//            (fully coalesced), and the CTA's partial sums of R over every 4096-wide chunk of k go to a small table;
+//   sweep C: one CTA per chunk of 4096 consecutive k: gathers its (R, X_even) from the [k1][k2] layout of W (runs of
+//            4096/L1 entries), transposes through shared memory, two-sided prefix sum of R from the scanned chunk sums,
+//            writes the natural-order output contiguously.
+// L1 is kept small (256 where the row of L2 still fits a CTA) so that sweep A reads x and writes W in >= 128-byte runs.
 #include "common.cuh"
 #include "fft_smem.cuh"
 #include <math.h>
 #include <stdlib.h>
 
 namespace {
+
+constexpr int SC_CHUNK = 4096, SC_NT = 512;       // sweep C: k's per chunk, threads per chunk
 
 constexpr int row_stride(int Lrow, int nrows) {            // padded row length with (stride mod 16) == max(1, 16/nrows)
     int want = (16 / nrows) > 0 ? (16 / nrows) : 1;
@@ -99,8 +103,9 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
     __syncthreads();
     {
         const int g = tid / GS, gt = tid % GS;
-        fft_smem<Q1>(re + g * RS, im + g * RS, gt, lo, hi, 2);
+        fft_smem<Q1, NT / GS>(re + g * RS, im + g * RS, gt, g, lo, hi, 2);
     }
+    __syncthreads();                                  // the sub-FFTs synchronise per group; the store below reads across groups
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         int e = tid + i * NT;
@@ -134,8 +139,8 @@ __device__ __forceinline__ void untangle_pair(double2& zk, double2& zm, double2 
 
 template <int Q2, int TL>
 __global__ void __launch_bounds__(PBCfg<Q2, TL>::NT, TL <= 12 ? 2 : 1)
-dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out, double scale,
-               double* __restrict__ xlast, int xstride) {
+dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restrict__ xlast, int xstride,
+               double* __restrict__ part) {
     using C = PBCfg<Q2, TL>;
     constexpr int L2 = C::L2, GS = C::GS, R2 = C::R2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
@@ -148,8 +153,7 @@ dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ ou
     double* im = re + C::IMOFF;
     const int tid = threadIdx.x;
     const int c = blockIdx.x;
-    const double2* Wc = W + (int64_t)blockIdx.y * L;
-    double* o = out + (int64_t)blockIdx.y * ld_out;
+    double2* Wc = W + (int64_t)blockIdx.y * L;
     auto row_of = [&](int slot) {
         int rho = c * T + (slot < T ? slot : slot - T);
         return slot < T ? rho : (rho == 0 ? L1 / 2 : L1 - rho);
@@ -173,8 +177,9 @@ dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ ou
     __syncthreads();
     {
         const int g = tid / GS, gt = tid % GS;
-        fft_smem<Q2>(re + g * RS, im + g * RS, gt, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
+        fft_smem<Q2, NT / GS>(re + g * RS, im + g * RS, gt, g, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
     }
+    __syncthreads();                                  // per-group barriers inside; the untangle pairs rows of different groups
     // untangle: thread owns the pair {(slot r, k2), its mirror}; k = row + L1*k2
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -207,51 +212,48 @@ dst1_pb_kernel(int log2N, const double2* __restrict__ W, double* __restrict__ ou
         }
     }
     __syncthreads();
-    // natural-order output: X_{2k} at o[2k-1], R_k at o[2k]; for fixed k2 the T rows of a tile are 2T consecutive doubles
+    // (R_k, X_{2k}) back into the CTA's own rows of W
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         int e = tid + i * NT;
-        int slot = e % R2, k2 = e / R2;
-        int64_t k = (int64_t)row_of(slot) + (int64_t)L1 * k2;
+        int slot = e / L2, k2 = e % L2;
         int ia = slot * RS + PADI(k2);
-        o[2 * k] = scale * re[ia];
-        if (k >= 1) o[2 * k - 1] = scale * im[ia];
+        Wc[(int64_t)row_of(slot) * L2 + k2] = make_double2(scale * re[ia], scale * im[ia]);
+    }
+    // partial chunk sums of R: chunk of k = row + L1*k2 is k2 / CW (L1 <= SC_CHUNK), fixed order -> deterministic
+    {
+        const int CW = SC_CHUNK / L1 > 0 ? SC_CHUNK / L1 : 1;
+        const int nch = L2 / CW;
+        double* pc = part + ((int64_t)blockIdx.y * gridDim.x + c) * nch;
+        for (int ch = tid; ch < nch; ch += NT) {
+            double acc = 0.0;
+            for (int slot = 0; slot < R2; ++slot)
+                for (int j = 0; j < CW; ++j) acc += re[slot * RS + PADI(ch * CW + j)];
+            pc[ch] = scale * acc;
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------ sweep C
-// Odd outputs P_k = X_{2k+1} from R_k = P_k - P_{k-1} (stored at o[2k], R_0 = X_1): a TWO-SIDED in-place sum over the
-// even-index elements.  Lower half of the chunks forward from P_0 = X_1, upper half backward from the independently
-// known P_{L-1} = X_{N-1} (sweep B, xlast): every output is reached through the shorter chain and the small tail of a
-// decaying spectrum is summed from small terms only.  sums: per column nchunks chunk sums + 1 slot for X_{N-1}.
-constexpr int SC_CHUNK = 4096, SC_NT = 512;       // k's per chunk
+// Odd outputs P_k = X_{2k+1} from R_k = P_k - P_{k-1} (R_0 = X_1): a TWO-SIDED sum.  Lower half of the chunks forward
+// from P_0 = X_1, upper half backward from the independently known P_{L-1} = X_{N-1} (sweep B, xlast): every output is
+// reached through the shorter chain and the small tail of a decaying spectrum is summed from small terms only.
+// sums: per column nchunks chunk sums + 1 slot for X_{N-1}; part: per column [nB][nchunks] partial sums of sweep B.
 
-__global__ void __launch_bounds__(SC_NT)
-dst1_chunksum_kernel(int log2N, const double* __restrict__ out, int64_t ld_out, double* __restrict__ sums) {
-    const int64_t L = (int64_t)1 << (log2N - 1);
-    const int nch = (int)(L / SC_CHUNK);
-    const double* o = out + (int64_t)blockIdx.y * ld_out + 2 * (int64_t)blockIdx.x * SC_CHUNK;
-    __shared__ double ws[32];
-    double acc = 0.0;
-#pragma unroll
-    for (int i = 0; i < SC_CHUNK / SC_NT; ++i) acc += o[2 * (threadIdx.x + i * SC_NT)];
-    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int w = 0; w < SC_NT / 32; ++w) t += ws[w];
-        sums[(int64_t)blockIdx.y * (nch + 1) + blockIdx.x] = t;
-    }
-}
-
-// per column (one CTA): chunks c < nch/2 get the exclusive prefix of the chunk sums, chunks c >= nch/2 the exclusive
-// suffix (sum of the chunks above them, accumulated from the top)
+// per column (one CTA): chunk sums from sweep B's partials, then chunks c < nch/2 get the exclusive prefix of the chunk
+// sums, chunks c >= nch/2 the exclusive suffix (sum of the chunks above them, accumulated from the top)
 __global__ void __launch_bounds__(1024)
-dst1_scansums_kernel(int nchunks, double* __restrict__ sums) {
+dst1_scansums_kernel(int nchunks, int nB, const double* __restrict__ part, double* __restrict__ sums) {
     double* s = sums + (int64_t)blockIdx.x * (nchunks + 1);
+    const double* pc = part + (int64_t)blockIdx.x * nB * nchunks;
     __shared__ double wsum[32];
     __shared__ double tot;
+    for (int ch = threadIdx.x; ch < nchunks; ch += 1024) {
+        double acc = 0.0;
+        for (int b = 0; b < nB; ++b) acc += pc[(int64_t)b * nchunks + ch];
+        s[ch] = acc;
+    }
+    __syncthreads();
     const int half = nchunks / 2;
     for (int dir = 0; dir < 2; ++dir) {
         const int cnt = dir == 0 ? half : nchunks - half;
@@ -270,33 +272,79 @@ dst1_scansums_kernel(int nchunks, double* __restrict__ sums) {
     }
 }
 
+// shared-memory index of local k (0..4095): +1 per 8 (blocked scan reads: thread t owns k = 8t..8t+7), +PM per row of
+// K1C (transposed stores: a half-warp holds consecutive k2 of one k1, i.e. k's that are K1C apart)
+__device__ __forceinline__ int sc_pad(int k, int log2K1C, int PM) { return k + (k >> 3) + (k >> log2K1C) * PM; }
+constexpr int SC_ARR = SC_CHUNK + SC_CHUNK / 8 + 32 * 16 + 8;       // doubles per array
+static_assert(SC_ARR % 16 == 8, "R and X_even banks interleave in the output loop");
+
 __global__ void __launch_bounds__(SC_NT)
-dst1_scanapply_kernel(int log2N, double* __restrict__ out, int64_t ld_out, const double* __restrict__ sums) {
+dst1_scanapply_kernel(int log2N, int log2L1, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out,
+                      const double* __restrict__ sums) {
     const int64_t L = (int64_t)1 << (log2N - 1);
     const int nch = (int)(L / SC_CHUNK);
-    const bool fwd = (int)blockIdx.x < nch / 2;
-    double* o = out + (int64_t)blockIdx.y * ld_out + 2 * (int64_t)blockIdx.x * SC_CHUNK;
+    const int L1 = 1 << log2L1;
+    const int64_t L2 = L >> log2L1;
+    const int CW = L1 >= SC_CHUNK ? 1 : SC_CHUNK / L1;                // k2's per chunk
+    const int log2K1C = L1 >= SC_CHUNK ? 12 : log2L1;                 // k1's per chunk K1C = min(L1, 4096)
+    const int K1C = 1 << log2K1C;
+    const int PM = CW >= 16 ? 1 : 16 / CW;
+    const int c = blockIdx.x;
+    const bool fwd = c < nch / 2;
+    const double2* Wc = W + (int64_t)blockIdx.y * L;
+    double* o = out + (int64_t)blockIdx.y * ld_out;
     const double* sc = sums + (int64_t)blockIdx.y * (nch + 1);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* sR = (double*)smem_raw;
+    double* sX = sR + SC_ARR;
     __shared__ double wsum[32];
-    constexpr int PER = SC_CHUNK / SC_NT;          // 8 consecutive positions of the (possibly reversed) chunk per thread
+    // chunk c holds k = k1 + L1*k2: (L1 <= 4096) all k1, k2 in [c*CW, (c+1)*CW); (L1 > 4096) one k2 and a range of k1
+    const int64_t k2base = L1 >= SC_CHUNK ? ((int64_t)c * SC_CHUNK) / L1 : (int64_t)c * CW;
+    const int k1base = L1 >= SC_CHUNK ? (int)(((int64_t)c * SC_CHUNK) % L1) : 0;
+    constexpr int PER = SC_CHUNK / SC_NT;
+    double2 v[PER];
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int e = threadIdx.x + i * SC_NT;
+        const int k2o = e % CW, k1 = e / CW;
+        v[i] = Wc[(int64_t)(k1base + k1) * L2 + k2base + k2o];
+    }
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int e = threadIdx.x + i * SC_NT;
+        const int k2o = e % CW, k1 = e / CW;
+        const int ix = sc_pad(k1 + K1C * k2o, log2K1C, PM);
+        sR[ix] = v[i].x; sX[ix] = v[i].y;
+    }
+    __syncthreads();
     double loc[PER], val[PER]; double run = 0.0;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
         const int q = threadIdx.x * PER + i;
-        val[i] = o[2 * (fwd ? q : SC_CHUNK - 1 - q)];
+        val[i] = sR[sc_pad(fwd ? q : SC_CHUNK - 1 - q, log2K1C, PM)];
         run += val[i]; loc[i] = run;
     }
     double incl = group_scan_incl<SC_NT>(run, threadIdx.x, wsum);
     const double off = incl - run;
     if (fwd) {
-        const double base = sc[blockIdx.x];
+        const double base = sc[c];
 #pragma unroll
-        for (int i = 0; i < PER; ++i) o[2 * (threadIdx.x * PER + i)] = base + off + loc[i];                    // P_k
+        for (int i = 0; i < PER; ++i) sR[sc_pad(threadIdx.x * PER + i, log2K1C, PM)] = base + off + loc[i];     // P_k
     } else {
-        const double xl = sc[nch], above = sc[blockIdx.x];
+        const double xl = sc[nch], above = sc[c];
 #pragma unroll
         for (int i = 0; i < PER; ++i)                                // P_k = X_{N-1} - sum_{m > k} R_m
-            o[2 * (SC_CHUNK - 1 - (threadIdx.x * PER + i))] = xl - (above + (off + loc[i] - val[i]));
+            sR[sc_pad(SC_CHUNK - 1 - (threadIdx.x * PER + i), log2K1C, PM)] = xl - (above + (off + loc[i] - val[i]));
+    }
+    __syncthreads();
+    // natural order: X_{2k} at o[2k-1], P_k = X_{2k+1} at o[2k]; the chunk's 8192 outputs are contiguous from o[2 k0 - 1]
+    const int64_t obase = 2 * (int64_t)c * SC_CHUNK - 1;
+#pragma unroll
+    for (int i = 0; i < 2 * PER; ++i) {
+        const int j = threadIdx.x + i * SC_NT;
+        const int ix = sc_pad(j >> 1, log2K1C, PM);
+        const double val2 = (j & 1) ? sR[ix] : sX[ix];
+        if (obase + j >= 0) o[obase + j] = val2;
     }
 }
 
@@ -312,13 +360,12 @@ int launch_pa(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in
     return LRP_OK;
 }
 template <int Q2, int TL>
-int launch_pb(lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale,
-              double* xlast, int xstride) {
+int launch_pb(lrp_ctx* ctx, int log2N, int cols, double2* W, double scale, double* xlast, int xstride, double* part) {
     using C = PBCfg<Q2, TL>;
     LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pb_kernel<Q2, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     const int L1 = 1 << (log2N - 1 - Q2);
     LRP_PROF(ctx, K_DST_P2, 16.0 * ((int64_t)1 << log2N) * cols, 0);
-    dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, out, ld_out, scale, xlast, xstride);
+    dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, scale, xlast, xstride, part);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
@@ -337,25 +384,36 @@ int dispatch_pa(int q1, int tl, lrp_ctx* ctx, int log2N, int cols, const double*
     if (q1 == 12) return launch_pa<12, 13>(ctx, log2N, cols, in, ld_in, W);
     LRP_QL_SWITCH(q1, 13, launch_pa, ctx, log2N, cols, in, ld_in, W)
 }
-int dispatch_pb(int q2, int tl, lrp_ctx* ctx, int log2N, int cols, const double2* W, double* out, int64_t ld_out, double scale,
-                double* xlast, int xstride) {
-    if (tl == 12) { LRP_QL_SWITCH(q2, 12, launch_pb, ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride) }
-    if (q2 == 12) return launch_pb<12, 13>(ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride);
-    LRP_QL_SWITCH(q2, 13, launch_pb, ctx, log2N, cols, W, out, ld_out, scale, xlast, xstride)
+int dispatch_pb(int q2, int tl, lrp_ctx* ctx, int log2N, int cols, double2* W, double scale, double* xlast, int xstride,
+                double* part) {
+    if (tl == 12) { LRP_QL_SWITCH(q2, 12, launch_pb, ctx, log2N, cols, W, scale, xlast, xstride, part) }
+    if (q2 == 12) return launch_pb<12, 13>(ctx, log2N, cols, W, scale, xlast, xstride, part);
+    LRP_QL_SWITCH(q2, 13, launch_pb, ctx, log2N, cols, W, scale, xlast, xstride, part)
 }
 
-// tile size and split: L = 2^q = L1 * L2 with both factors <= 2^(TL-1)
-void plan(int log2N, int* tl, int* q1, int* q2) {
+// split L = 2^q = L1 * L2 and the tile sizes (2^tl points per CTA) of the two sweeps.  L1 = 256 wherever a pair of
+// rows of L2 still fits a CTA (sweep A then moves x and W in 128-byte runs and its sub-FFTs are one warp each).
+struct Plan { int q1, q2, tla, tlb, nB, nch; };
+int tile_rows(int tl, int q) { return 1 << (tl - q); }
+Plan plan(int log2N) {
     const int q = log2N - 1;
-    *tl = q <= 22 ? 12 : 13;
-    *q2 = q / 2; *q1 = q - *q2;
-    if (const char* e = getenv("LRP_DST_TL")) { int v = atoi(e); if (v == 13 && q >= 14) *tl = 13; }
-    if (const char* e = getenv("LRP_DST_Q1")) { int v = atoi(e); if (v >= 7 && v <= *tl - 1 && q - v >= 7 && q - v <= *tl - 1) { *q1 = v; *q2 = q - v; } }
+    Plan p;
+    p.q1 = q <= 14 ? 7 : 8;
+    if (q - p.q1 > 12) p.q1 = q - 12;
+    if (const char* e = getenv("LRP_DST_Q1")) { int v = atoi(e); if (v >= 7 && v <= 12 && q - v >= 7 && q - v <= 12) p.q1 = v; }
+    p.q2 = q - p.q1;
+    p.tla = p.q1 >= 9 ? 13 : 12;
+    if (const char* e = getenv("LRP_DST_TLA")) { int v = atoi(e); if ((v == 12 && p.q1 <= 11) || v == 13) p.tla = v; }
+    p.tlb = p.q2 >= 12 ? 13 : 12;
+    if (const char* e = getenv("LRP_DST_TLB")) { int v = atoi(e); if ((v == 12 && p.q2 <= 11) || v == 13) p.tlb = v; }
+    p.nB = (1 << p.q1) / tile_rows(p.tlb, p.q2);
+    p.nch = (int)(((int64_t)1 << q) / SC_CHUNK);
+    return p;
 }
 
-// columns per group: W + output of one group should stay L2-resident between the sweeps
+// columns per group (workspace bound: W of one group)
 int group_cols(int64_t N, int batch) {
-    int64_t per_col = N * 16;
+    int64_t per_col = N * 8;
     static int64_t budget_mb = 0;
     if (budget_mb == 0) { const char* e = getenv("LRP_DST_GROUP_MB"); budget_mb = e ? atoll(e) : 4096; if (budget_mb < 1) budget_mb = 4096; }
     int g = (int)((budget_mb << 20) / per_col);
@@ -369,33 +427,34 @@ int group_cols(int64_t N, int batch) {
 size_t dst1_large_ws(int64_t N, int32_t batch) {
     const int g = group_cols(N, batch);
     const int64_t L = N / 2;
-    return lrp_align_up((size_t)g * L * sizeof(double2)) + lrp_align_up((size_t)g * (L / SC_CHUNK + 1) * sizeof(double));
+    const Plan p = plan(lrp_ilog2(N));
+    return lrp_align_up((size_t)g * L * sizeof(double2)) + lrp_align_up((size_t)g * (p.nch + 1) * sizeof(double)) +
+           lrp_align_up((size_t)g * p.nB * p.nch * sizeof(double));
 }
 
 int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
                double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes) {
     const int64_t N = (int64_t)1 << log2N, L = N / 2;
     if (log2N > 25) return LRP_ERR_UNSUPPORTED_N;
-    int tl, q1, q2; plan(log2N, &tl, &q1, &q2);
+    const Plan p = plan(log2N);
     const int g = group_cols(N, batch);
     lrp_arena ar(ws, ws_bytes);
     double2* W = ar.take<double2>((size_t)g * L);
-    double* sums = ar.take<double>((size_t)g * (L / SC_CHUNK + 1));
+    double* sums = ar.take<double>((size_t)g * (p.nch + 1));
+    double* part = ar.take<double>((size_t)g * p.nB * p.nch);
     if (!ar.ok()) return LRP_ERR_WORKSPACE;
-    const int nchunks = (int)(L / SC_CHUNK);
+    constexpr int SC_SMEM = 2 * SC_ARR * (int)sizeof(double);
+    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_scanapply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SC_SMEM));
     for (int c0 = 0; c0 < batch; c0 += g) {
         const int cols = (batch - c0) < g ? (batch - c0) : g;
         double* o = d_out + (int64_t)c0 * ld_out;
-        LRP_TRY(dispatch_pa(q1, tl, ctx, log2N, cols, d_in + (int64_t)c0 * ld_in, ld_in, W));
-        LRP_TRY(dispatch_pb(q2, tl, ctx, log2N, cols, W, o, ld_out, scale, sums + nchunks, nchunks + 1));
-        LRP_PROF(ctx, K_DST_CHUNKSUM, 8.0 * N * cols, 0);
-        dst1_chunksum_kernel<<<dim3(nchunks, cols), SC_NT, 0, ctx->stream>>>(log2N, o, ld_out, sums);
-        LRP_LAUNCHED(ctx);
+        LRP_TRY(dispatch_pa(p.q1, p.tla, ctx, log2N, cols, d_in + (int64_t)c0 * ld_in, ld_in, W));
+        LRP_TRY(dispatch_pb(p.q2, p.tlb, ctx, log2N, cols, W, scale, sums + p.nch, p.nch + 1, part));
         LRP_PROF(ctx, K_DST_SCANSUMS, 0, 0);
-        dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(nchunks, sums);
+        dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(p.nch, p.nB, part, sums);
         LRP_LAUNCHED(ctx);
         LRP_PROF(ctx, K_DST_FINISH, 16.0 * N * cols, 0);
-        dst1_scanapply_kernel<<<dim3(nchunks, cols), SC_NT, 0, ctx->stream>>>(log2N, o, ld_out, sums);
+        dst1_scanapply_kernel<<<dim3(p.nch, cols), SC_NT, SC_SMEM, ctx->stream>>>(log2N, p.q1, W, o, ld_out, sums);
         LRP_LAUNCHED(ctx);
     }
     return LRP_OK;

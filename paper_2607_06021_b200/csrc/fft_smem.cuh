@@ -70,11 +70,20 @@ template <> struct Bfly<8> {
     }
 };
 
+// barrier over the GS threads of group g (of NG groups per CTA): the sub-FFTs of a CTA are independent, so a pass never
+// needs to wait for the other groups.  One warp or less: __syncwarp; else a named barrier (ids 1..15) per group.
+template <int GS, int NG>
+__device__ __forceinline__ void group_bar(int g) {
+    if constexpr (GS <= 32) __syncwarp();
+    else if constexpr (NG == 1 || NG > 15) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(GS) : "memory");
+}
+
 // One Stockham pass of radix R over a length-2^Q complex sequence held in (re, im) (padded with PADI),
 // executed by the GS = 2^Q/8 threads of a group (gt = thread in group); every thread keeps its 8 complex
 // values in registers across the barrier, so the pass is in place.  Twiddle exp(-2 pi i mm / L) = tw(tw_mul*mm).
-template <int Q, int R, bool FIRST>
-__device__ __forceinline__ void fft_pass(double* re, double* im, int gt, int log2Ns,
+template <int Q, int R, bool FIRST, int NG>
+__device__ __forceinline__ void fft_pass(double* re, double* im, int gt, int g, int log2Ns,
                                          const double2* lo, const double2* hi, int tw_mul) {
     constexpr int L = 1 << Q, GS = L / 8, ITEMS = 8 / R, STRIDE = L / R;
     double2 v[ITEMS][R];
@@ -85,7 +94,7 @@ __device__ __forceinline__ void fft_pass(double* re, double* im, int gt, int log
             int idx = PADI(gt + it * GS + r * STRIDE);
             v[it][r] = make_double2(re[idx], im[idx]);
         }
-    __syncthreads();
+    group_bar<GS, NG>(g);
     const int Ns = 1 << log2Ns;
 #pragma unroll
     for (int it = 0; it < ITEMS; ++it) {
@@ -115,19 +124,20 @@ __device__ __forceinline__ void fft_pass(double* re, double* im, int gt, int log
             re[idx] = v[it][r].x; im[idx] = v[it][r].y;
         }
     }
-    __syncthreads();
+    group_bar<GS, NG>(g);
 }
 
 // forward complex FFT of length 2^Q in shared memory, natural order in and out (Stockham autosort).
-template <int Q>
-__device__ __forceinline__ void fft_smem(double* re, double* im, int gt,
+// g = index of the calling thread's group among the NG groups (of 2^Q/8 threads each) of the CTA.
+template <int Q, int NG>
+__device__ __forceinline__ void fft_smem(double* re, double* im, int gt, int g,
                                          const double2* lo, const double2* hi, int tw_mul) {
     constexpr int A = Q / 3, B = Q % 3;
-    fft_pass<Q, 8, true>(re, im, gt, 0, lo, hi, tw_mul);
+    fft_pass<Q, 8, true, NG>(re, im, gt, g, 0, lo, hi, tw_mul);
 #pragma unroll
-    for (int p = 1; p < A; ++p) fft_pass<Q, 8, false>(re, im, gt, 3 * p, lo, hi, tw_mul);
-    if (B == 1) fft_pass<Q, 2, false>(re, im, gt, 3 * A, lo, hi, tw_mul);
-    if (B == 2) fft_pass<Q, 4, false>(re, im, gt, 3 * A, lo, hi, tw_mul);
+    for (int p = 1; p < A; ++p) fft_pass<Q, 8, false, NG>(re, im, gt, g, 3 * p, lo, hi, tw_mul);
+    if (B == 1) fft_pass<Q, 2, false, NG>(re, im, gt, g, 3 * A, lo, hi, tw_mul);
+    if (B == 2) fft_pass<Q, 4, false, NG>(re, im, gt, g, 3 * A, lo, hi, tw_mul);
 }
 
 // inclusive scan of one value per thread over the GS (power of two) threads of a group; wsum: >= 32 doubles
