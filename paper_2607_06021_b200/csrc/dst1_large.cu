@@ -36,8 +36,9 @@ template <int Q1, int TL> struct PACfg {
     static constexpr int IMOFF = T2 * RS + 8;
     static constexpr int NHI = (2 * L1) / 64 + 1;
     static constexpr int TW_LO = 32, TW_HI = (L1 + 31) / 32;
+    static constexpr int SLO = 33, SHI = TW_HI | 1;        // odd row strides: the T2 rows are read side by side
     static constexpr int CH = 4;                  // loads in flight per thread (register budget)
-    static constexpr size_t SMEM = sizeof(double2) * (64 + NHI + 2 * T2 + (size_t)T2 * (TW_LO + TW_HI)) +
+    static constexpr size_t SMEM = sizeof(double2) * (64 + NHI + 2 * T2 + (size_t)T2 * (SLO + SHI)) +
                                    sizeof(double) * ((size_t)2 * IMOFF);
 };
 
@@ -53,8 +54,8 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
     double2* hi = lo + 64;
     double2* tB = hi + C::NHI;                       // [T2][2]   exp(-i pi (2 j2 + b)/N)
     double2* t4lo = tB + 2 * T2;                     // [T2][32]  exp(-2 pi i j2 l / L)
-    double2* t4hi = t4lo + T2 * C::TW_LO;            // [T2][L1/32] exp(-2 pi i j2 (32 h) / L)
-    double* re = (double*)(t4hi + T2 * C::TW_HI);
+    double2* t4hi = t4lo + T2 * C::SLO;            // [T2][L1/32] exp(-2 pi i j2 (32 h) / L)
+    double* re = (double*)(t4hi + T2 * C::SHI);
     double* im = re + C::IMOFF;
     const int tid = threadIdx.x;
     const int c = blockIdx.x;
@@ -68,8 +69,8 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
     }
     for (int i = tid; i < T2 * (C::TW_LO + C::TW_HI); i += NT) {
         int s, kk; double2* dst;
-        if (i < T2 * C::TW_LO) { s = i / C::TW_LO; kk = i % C::TW_LO; dst = t4lo + i; }
-        else { int q = i - T2 * C::TW_LO; s = q / C::TW_HI; kk = (q % C::TW_HI) * 32; dst = t4hi + q; }
+        if (i < T2 * C::TW_LO) { s = i / C::TW_LO; kk = i % C::TW_LO; dst = t4lo + s * C::SLO + kk; }
+        else { int q = i - T2 * C::TW_LO; s = q / C::TW_HI; kk = (q % C::TW_HI) * 32; dst = t4hi + s * C::SHI + (q % C::TW_HI); }
         int64_t prod = ((int64_t)j2_of(s) * kk) & (L - 1);
         double sn, cs; sincospi(-2.0 * (double)prod / (double)L, &sn, &cs); *dst = make_double2(cs, sn);
     }
@@ -111,7 +112,7 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
         int e = tid + i * NT;
         int s = e % T2, k1 = e / T2;
         double2 v = make_double2(re[s * RS + PADI(k1)], im[s * RS + PADI(k1)]);
-        double2 w = cmul(t4hi[s * C::TW_HI + (k1 >> 5)], t4lo[s * C::TW_LO + (k1 & 31)]);
+        double2 w = cmul(t4hi[s * C::SHI + (k1 >> 5)], t4lo[s * C::SLO + (k1 & 31)]);
         Wc[(int64_t)k1 * L2 + j2_of(s)] = cmul(v, w);
     }
 }
@@ -158,27 +159,18 @@ dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restr
         int rho = c * T + (slot < T ? slot : slot - T);
         return slot < T ? rho : (rho == 0 ? L1 / 2 : L1 - rho);
     };
+    const int g = tid / GS, gt = tid % GS;           // group g transforms row slot g; v[r] = row[gt + r*GS]: first-pass operands
     double2 v[8];
+    {
+        const double2* row = Wc + (int64_t)row_of(g) * L2;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int e = tid + i * NT;
-        v[i] = Wc[(int64_t)row_of(e / L2) * L2 + (e % L2)];
+        for (int r = 0; r < 8; ++r) v[r] = row[gt + r * GS];
     }
     tw_build(lo, hi, 2 * L2, C::NHI, tid, NT);        // exp(-2 pi i u/(2 L2)) = exp(-2 pi i (L1 u)/N)
     for (int i = tid; i < R2; i += NT) {
         double sn, cs; sincospi(-2.0 * (double)row_of(i) / (double)N, &sn, &cs); rowtw[i] = make_double2(cs, sn);
     }
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int e = tid + i * NT;
-        int slot = e / L2, j2 = e % L2;
-        re[slot * RS + PADI(j2)] = v[i].x; im[slot * RS + PADI(j2)] = v[i].y;
-    }
-    __syncthreads();
-    {
-        const int g = tid / GS, gt = tid % GS;
-        fft_smem<Q2, NT / GS>(re + g * RS, im + g * RS, gt, g, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
-    }
+    fft_smem_from_regs<Q2, NT / GS>(v, re + g * RS, im + g * RS, gt, g, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
     __syncthreads();                                  // per-group barriers inside; the untangle pairs rows of different groups
     // untangle: thread owns the pair {(slot r, k2), its mirror}; k = row + L1*k2
 #pragma unroll

@@ -140,6 +140,26 @@ __device__ __forceinline__ void fft_smem(double* re, double* im, int gt, int g,
     if (B == 2) fft_pass<Q, 4, false, NG>(re, im, gt, g, 3 * A, lo, hi, tw_mul);
 }
 
+// Same transform with the first radix-8 pass fed from registers: v[r] = x[gt + r * 2^Q/8] (what a coalesced global load of
+// the row delivers), so the sequence is never stored and re-read before the first butterfly.  The CTA-wide barrier
+// after the first pass also publishes twiddle tables built since the last barrier.
+template <int Q, int NG>
+__device__ __forceinline__ void fft_smem_from_regs(double2 (&v)[8], double* re, double* im, int gt, int g,
+                                                   const double2* lo, const double2* hi, int tw_mul) {
+    constexpr int A = Q / 3, B = Q % 3;
+    Bfly<8>::run(v);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        int idx = PADI(gt * 8 + r);
+        re[idx] = v[r].x; im[idx] = v[r].y;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int p = 1; p < A; ++p) fft_pass<Q, 8, false, NG>(re, im, gt, g, 3 * p, lo, hi, tw_mul);
+    if (B == 1) fft_pass<Q, 2, false, NG>(re, im, gt, g, 3 * A, lo, hi, tw_mul);
+    if (B == 2) fft_pass<Q, 4, false, NG>(re, im, gt, g, 3 * A, lo, hi, tw_mul);
+}
+
 // inclusive scan of one value per thread over the GS (power of two) threads of a group; wsum: >= 32 doubles
 // of shared memory per group (used when GS > 32).  Contains barriers: call from all threads.
 template <int GS>
