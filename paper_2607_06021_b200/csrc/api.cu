@@ -35,8 +35,10 @@ int check_n(int64_t n) {
 struct ScrossWs {
     double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws, *qr_ws2;
     int32_t *scal_i, *iwork;
+    int ldrc, ldrr;               // leading dimensions of RC / RR: fixed (kmax / lmax), so that a factor survives a change of k
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int kmax, int lmax) {
         int K = kmax > lmax ? kmax : lmax;
+        ldrc = kmax; ldrr = lmax;
         RC = ar.take<double>((size_t)kmax * kmax); RR = ar.take<double>((size_t)lmax * lmax);
         Uc = ar.take<double>((size_t)K * K); S = ar.take<double>(K); Vc = ar.take<double>((size_t)K * K);
         rC = ar.take<double>(kmax); rR = ar.take<double>(lmax);
@@ -50,14 +52,16 @@ struct ScrossWs {
 
 // QR of both fiber blocks (in place), the small core, and the host copies the driver needs.
 // On return (stream synchronised): Qb = Q, Zb = Z, ws.Uc/S/Vc hold the core SVD, h_S (p), h_rC (k), h_rR (l) filled.
-int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, double* Zb, int64_t ldz, int l,
+// k0 / l0: leading columns of Qb / Zb that already hold the Q factor of the same fibers (with their block of RC / RR
+// in place) from the previous call: the fibers of surviving indices do not change between sweeps.
+int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, int k0, double* Zb, int64_t ldz, int l, int l0,
                   const int32_t* dI, const int32_t* dJ, ScrossWs& w,
                   double* h_S, double* h_rC, double* h_rR, int* h_rank, double* h_smin,
                   cudaEvent_t ev_qr_done) {
-    LRP_TRY(tall_qr_pair(ctx, n, k, Qb, ldq, w.RC, k, w.qr_ws, l, Zb, ldz, w.RR, l, w.qr_ws2));
+    LRP_TRY(tall_qr_pair_from(ctx, n, k, k0, Qb, ldq, w.RC, w.ldrc, w.qr_ws, l, l0, Zb, ldz, w.RR, w.ldrr, w.qr_ws2));
     if (ev_qr_done) LRP_CUDA(ctx, cudaEventRecord(ev_qr_done, ctx->stream));
     CoreArgs a{};
-    a.k = k; a.l = l; a.Q = Qb; a.ldq = ldq; a.Z = Zb; a.ldz = ldz; a.RC = w.RC; a.ldrc = k; a.RR = w.RR; a.ldrr = l;
+    a.k = k; a.l = l; a.Q = Qb; a.ldq = ldq; a.Z = Zb; a.ldz = ldz; a.RC = w.RC; a.ldrc = w.ldrc; a.RR = w.RR; a.ldrr = w.ldrr;
     a.I = dI; a.J = dJ; a.pinv_rcond = PINV_RCOND; a.rank_rcond = RANK_RCOND;
     a.Uc = w.Uc; a.S = w.S; a.Vc = w.Vc; a.rC = w.rC; a.rR = w.rR; a.scal_i = w.scal_i; a.scal_d = w.scal_d;
     a.work = w.core_work; a.iwork = w.iwork;
@@ -407,7 +411,7 @@ int lrp_scross(lrp_ctx* ctx, int64_t n, const double* d_C, int64_t ldc, int32_t 
     const int p = k < l ? k : l;
     std::vector<double> hS(p), hrC(k), hrR(l);
     int rank = 0; double smin = 0.0;
-    LRP_TRY(scross_factor(ctx, n, Qb, n, k, Zb, n, l, d_I, d_J, w, hS.data(), hrC.data(), hrR.data(), &rank, &smin, nullptr));
+    LRP_TRY(scross_factor(ctx, n, Qb, n, k, 0, Zb, n, l, 0, d_I, d_J, w, hS.data(), hrC.data(), hrR.data(), &rank, &smin, nullptr));
     LRP_TRY(rebuild(ctx, n, Qb, n, k, w.Uc, k, rank, d_U, ldu, nullptr));
     LRP_TRY(rebuild(ctx, n, Zb, n, l, w.Vc, l, rank, d_V, ldv, nullptr));
     LRP_CUDA(ctx, cudaMemcpyAsync(d_S, w.S, sizeof(double) * p, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -475,6 +479,11 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     const double* selU = U0 ? U0 : w.UhF; const double* selV = U0 ? V0 : w.VhF;
     int64_t sel_ld = U0 ? ld0 : ld; int sel_cols = U0 ? r0 : rF;
     std::vector<int32_t> I_prev, J_prev, I_k, J_k, hstar(2 * (size_t)Kc + 8);
+    // Fibers of an index are the same in every sweep, and the QR of a column prefix is the prefix of the QR: the leading
+    // columns of this sweep's fiber block that repeat last sweep's block in the same order keep their Q columns (still in
+    // Cb / Rb) and their block of R; only the columns after the common prefix are sampled and factored.
+    std::vector<int32_t> I_fact, J_fact;          // index lists whose Q factors Rb / Cb hold (empty: none)
+    const bool reuse_qr = getenv("LRP_NO_QR_REUSE") == nullptr;
     std::vector<double> hS(Kc), hrC(Kc), hrR(Kc), hS_last;
     std::vector<uint8_t> keepI, keepJ;
     int rank = 0; double smin = 0.0;
@@ -548,13 +557,19 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         cudaStream_t side = ctx->prof_on == 1 ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ, kk, w.Cb, ld));
-        LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI, l, w.Rb, ld));
+        int k0 = 0, l0 = 0;
+        if (reuse_qr) {
+            while (k0 < kk && k0 < (int)J_fact.size() && J_fact[k0] == J_k[k0]) ++k0;
+            while (l0 < l && l0 < (int)I_fact.size() && I_fact[l0] == I_k[l0]) ++l0;
+        }
+        if (kk > k0) LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ + k0, kk - k0, w.Cb + (int64_t)k0 * ld, ld));
+        if (l > l0) LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
         cudaEvent_t e2 = ep.rec(ctx);
         // ---- O8: scross
         cudaEvent_t e3 = nullptr;
         { cudaEvent_t tmp; if (cudaEventCreate(&tmp) == cudaSuccess) { ep.ev.push_back(tmp); e3 = tmp; } }
-        LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, w.Rb, ld, l, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
+        LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, k0, w.Rb, ld, l, l0, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
+        J_fact = J_k; I_fact = I_k;
         cudaEvent_t e4 = ep.rec(ctx);
         const int p = kk < l ? kk : l;
         // ---- O9: prune (Alg. 4 lines 14-23; reading Q12)
@@ -618,6 +633,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
                 TallGemmArgs g{};
                 g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
                 g.Cin = Vp; g.ldc = ld; g.Out = w.Rb; g.ldo = ld;
+                I_fact.clear();                              // Rb no longer holds the Q factor
                 rc_v = tall_gemm(ctx, g);
                 if (rc_v >= 0) rc_v = tall_gemm_t(ctx, n, w.Rb, ld, r_prev, w.Rb, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
             }
@@ -638,6 +654,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
                 TallGemmArgs g{};
                 g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Uk; g.lda = ld; g.B = w.Amat; g.ldb = rank;
                 g.Cin = Up; g.ldc = ld; g.Out = w.Cb; g.ldo = ld;
+                J_fact.clear();                              // Cb no longer holds the Q factor
                 LRP_TRY(tall_gemm(ctx, g));
                 LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, r_prev, w.Cb, ld, r_prev, w.GU, r_prev, 0, w.gemmt_ws));
             }

@@ -9,7 +9,14 @@ int tall_qr(lrp_ctx* ctx, int64_t n, int K, double* A, int64_t lda, double* R, i
 int tall_qr_pair(lrp_ctx* ctx, int64_t n, int K1, double* A1, int64_t lda1, double* R1, int64_t ldr1, double* ws1,
                  int K2, double* A2, int64_t lda2, double* R2, int64_t ldr2, double* ws2);
 
+// Same, extending existing factorizations: the leading k01 (k02) columns of A1 (A2) already hold orthonormal Q columns
+// and the leading k0 x k0 block of R their triangular factor (QR of a column prefix is the prefix of the QR); only
+// the columns from k0 on are projected and factored.  k0 = 0: the whole block.
+int tall_qr_pair_from(lrp_ctx* ctx, int64_t n, int K1, int k01, double* A1, int64_t lda1, double* R1, int64_t ldr1, double* ws1,
+                      int K2, int k02, double* A2, int64_t lda2, double* R2, int64_t ldr2, double* ws2);
+
 struct QrJob {
+    int k0;                                       // leading columns already factored (0: none)
     int64_t n; int K; double* A; int64_t lda; double* R; int64_t ldr; double* ws; cudaStream_t stream;
     double* hR;                                   // pinned host scratch, 256 doubles
     double *stack, *partial, *Stmp, *d_runmax;    // carved from ws by tall_qr_begin

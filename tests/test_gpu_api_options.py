@@ -104,13 +104,40 @@ def test_fused_and_two_sweep_stop_test_agree(ctx, monkeypatch):
     and through the update sweep + Gram sweep it replaces (shapes outside the fused kernel's range take that path):
     the same sweeps, ranks and index decisions, rho equal to rounding of a sum of squares."""
     w = W.make("C2", 3)
+    # the two-sweep path borrows the fiber buffers, which ends the reuse of their Q factors: both runs factor every
+    # fiber block from scratch, so that only the stop test differs
+    monkeypatch.setenv("LRP_NO_QR_REUSE", "1")
     a = _solve(ctx, w)
     monkeypatch.setenv("LRP_NO_FUSED_RHO", "1")
     b = _solve(ctx, w)
     monkeypatch.delenv("LRP_NO_FUSED_RHO")
+    monkeypatch.delenv("LRP_NO_QR_REUSE")
     assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
     ia, ib = a["info"], b["info"]
     for k in range(a["sweeps"]):
         ra, rb = ia.rho_per_sweep[k], ib.rho_per_sweep[k]
         assert abs(ra - rb) <= 1e-9 * max(abs(ra), abs(rb)) + 1e-13 * ia.snorm
         assert ia.rank_per_sweep[k] == ib.rank_per_sweep[k] and ia.nI[k] == ib.nI[k] and ia.nJ[k] == ib.nJ[k]
+
+
+@pytest.mark.parametrize("cfg,seed,nred", [("C2", 0, None), ("C2", 3, None), ("C3", 0, 16383), ("C4", 0, 32767)])
+def test_qr_prefix_reuse_matches_full_factorization(ctx, monkeypatch, cfg, seed, nred):
+    """Fibers of surviving indices do not change between sweeps (G-hat is fixed, eq. (4)) and the QR of a
+    column prefix is the prefix of the QR, so the driver keeps the Q columns of the common prefix of consecutive index
+    lists and factors only the new fibers.  Against factoring every block from scratch (LRP_NO_QR_REUSE): the same
+    index decisions in the first sweeps, the same rank, and reconstructed entries equal to the parity tolerance."""
+    from paper_2607_06021_b200 import lrp
+    w = W.make(cfg, seed) if nred is None else W.make(cfg, seed, nred)
+    a = _solve(ctx, w)
+    monkeypatch.setenv("LRP_NO_QR_REUSE", "1")
+    b = _solve(ctx, w)
+    monkeypatch.delenv("LRP_NO_QR_REUSE")
+    assert abs(a["sweeps"] - b["sweeps"]) <= 1 and a["rank"] == b["rank"]
+    for ta, tb in list(zip(a["trace"], b["trace"]))[:2]:
+        assert list(ta["I"]) == list(tb["I"]) and list(ta["J"]) == list(tb["J"])
+    rows, cols = W.sample_pairs(w.n, 4096, seed=5)
+    ea = _entries(lrp.tall_to_numpy(a["UW"]), a["SW"].cpu().numpy(), lrp.tall_to_numpy(a["VW"]), rows, cols)
+    eb = _entries(lrp.tall_to_numpy(b["UW"]), b["SW"].cpu().numpy(), lrp.tall_to_numpy(b["VW"]), rows, cols)
+    tol = 1e-10 if (a["converged"] and b["converged"]) else 2 * max(a["info"].rho, b["info"].rho) / a["info"].snorm + 1e-10
+    assert np.abs(ea - eb).max() <= tol * np.abs(eb).max()
+    assert a["info"].launches < b["info"].launches
