@@ -625,21 +625,19 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             cudaStream_t main_stream = ctx->stream;
             ctx->stream = side;
             int rc_v = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
-            cudaError_t ew = cudaSuccess;
             // E_V = V_{k-1} - V_k B and its Gram matrix in one pass (E never written); outside the fused kernel's range:
-            // update sweep into the fiber buffer (free after the rebuild, but eta still reads it: wait) + Gram sweep
+            // update sweep IN PLACE over V_{k-1} (dead after this test: its buffer is the next sweep's rebuild target)
+            // + Gram sweep.  The fiber buffers keep their Q factors for the next sweep.
             if (rc_v >= 0) rc_v = tall_resid_gram(ctx, n, Vk, ld, rank, w.Bmat, rank, Vp, ld, r_prev, w.GV, r_prev, w.gemmt_ws2);
-            if (rc_v == 1 && (ew = cudaStreamWaitEvent(side, ctx->ev_join2, 0)) == cudaSuccess) {
+            if (rc_v == 1) {
                 TallGemmArgs g{};
                 g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Vk; g.lda = ld; g.B = w.Bmat; g.ldb = rank;
-                g.Cin = Vp; g.ldc = ld; g.Out = w.Rb; g.ldo = ld;
-                I_fact.clear();                              // Rb no longer holds the Q factor
+                g.Cin = Vp; g.ldc = ld; g.Out = Vp; g.ldo = ld;
                 rc_v = tall_gemm(ctx, g);
-                if (rc_v >= 0) rc_v = tall_gemm_t(ctx, n, w.Rb, ld, r_prev, w.Rb, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
+                if (rc_v >= 0) rc_v = tall_gemm_t(ctx, n, Vp, ld, r_prev, Vp, ld, r_prev, w.GV, r_prev, 0, w.gemmt_ws2);
             }
             ctx->stream = main_stream;
             if (rc_v < 0) return rc_v;
-            if (ew != cudaSuccess) { ctx->last_cuda = (int)ew; return LRP_ERR_CUDA; }
         }
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
         RhoArgs ra{};
@@ -650,13 +648,11 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
             int rc_u = tall_resid_gram(ctx, n, Uk, ld, rank, w.Amat, rank, Up, ld, r_prev, w.GU, r_prev, w.gemmt_ws);
             if (rc_u < 0) return rc_u;
             if (rc_u == 1) {
-                LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join2, 0));
                 TallGemmArgs g{};
                 g.n = n; g.k = rank; g.m = r_prev; g.mode = TG_SUBTRACT; g.A = Uk; g.lda = ld; g.B = w.Amat; g.ldb = rank;
-                g.Cin = Up; g.ldc = ld; g.Out = w.Cb; g.ldo = ld;
-                J_fact.clear();                              // Cb no longer holds the Q factor
+                g.Cin = Up; g.ldc = ld; g.Out = Up; g.ldo = ld;
                 LRP_TRY(tall_gemm(ctx, g));
-                LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, r_prev, w.Cb, ld, r_prev, w.GU, r_prev, 0, w.gemmt_ws));
+                LRP_TRY(tall_gemm_t(ctx, n, Up, ld, r_prev, Up, ld, r_prev, w.GU, r_prev, 0, w.gemmt_ws));
             }
         }
         LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));

@@ -104,14 +104,10 @@ def test_fused_and_two_sweep_stop_test_agree(ctx, monkeypatch):
     and through the update sweep + Gram sweep it replaces (shapes outside the fused kernel's range take that path):
     the same sweeps, ranks and index decisions, rho equal to rounding of a sum of squares."""
     w = W.make("C2", 3)
-    # the two-sweep path borrows the fiber buffers, which ends the reuse of their Q factors: both runs factor every
-    # fiber block from scratch, so that only the stop test differs
-    monkeypatch.setenv("LRP_NO_QR_REUSE", "1")
     a = _solve(ctx, w)
     monkeypatch.setenv("LRP_NO_FUSED_RHO", "1")
     b = _solve(ctx, w)
     monkeypatch.delenv("LRP_NO_FUSED_RHO")
-    monkeypatch.delenv("LRP_NO_QR_REUSE")
     assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
     ia, ib = a["info"], b["info"]
     for k in range(a["sweeps"]):
