@@ -117,6 +117,7 @@ int validate_indices(const int32_t* h, int cnt, int64_t n) {
 // ------------------------------------------------------------------------------------------------ solve workspace
 struct SolveWs {
     double *UhF, *VhF, *Cb, *Rb, *Ua, *Va, *Ub, *Vb, *scoresU, *scoresV;
+    double *UcPrev, *VcPrev, *nestU, *nestV;      // previous core factors and scratch of the nested stop test
     double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev, *Rlev2;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
     unsigned char *mask, *mask2;
@@ -134,6 +135,8 @@ struct SolveWs {
         Amat = ar.take<double>((size_t)Kc * Kc); Bmat = ar.take<double>((size_t)Kc * Kc);
         GU = ar.take<double>((size_t)Kc * Kc); GV = ar.take<double>((size_t)Kc * Kc);
         Rlev = ar.take<double>((size_t)Kc * Kc); Rlev2 = ar.take<double>((size_t)Kc * Kc);
+        UcPrev = ar.take<double>((size_t)Kc * Kc); VcPrev = ar.take<double>((size_t)Kc * Kc);
+        nestU = ar.take<double>((size_t)Kc * Kc); nestV = ar.take<double>((size_t)Kc * Kc);
         rho_out = ar.take<double>(8); eta = ar.take<double>(8);
         eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
         eta_work = ar.take<double>(2 * eta_stride);
@@ -484,6 +487,8 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     // Cb / Rb) and their block of R; only the columns after the common prefix are sampled and factored.
     std::vector<int32_t> I_fact, J_fact;          // index lists whose Q factors Rb / Cb hold (empty: none)
     const bool reuse_qr = getenv("LRP_NO_QR_REUSE") == nullptr;
+    const bool nested_rho = reuse_qr && getenv("LRP_NO_NESTED_RHO") == nullptr;
+    int kk_prev = 0, l_prev = 0;                  // sizes of the previous sweep's index lists (rows of UcPrev / VcPrev)
     std::vector<double> hS(Kc), hrC(Kc), hrR(Kc), hS_last;
     std::vector<uint8_t> keepI, keepJ;
     int rank = 0; double smin = 0.0;
@@ -620,8 +625,20 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_TRY(rebuild(ctx, n, w.Cb, ld, kk, w.sc.Uc, kk, rank, Uk, ld, w.scoresU));
         LRP_ON_STREAM(ctx, side, rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
         cudaEvent_t e5 = ep.rec(ctx);
-        // ---- O10: rho (factored, reading Q13), indicator.  The two sides run on the main and the auxiliary stream.
-        if (r_prev > 0) {
+        // ---- O10: rho (factored, reading Q13), indicator.
+        // Nested case: last sweep's lists are prefixes of this sweep's and their Q columns were kept, so U_{k-1}, V_{k-1}
+        // lie in the spans of Q_k, Z_k and rho needs the small core factors only (no pass over the tall iterates).
+        const bool nested = nested_rho && r_prev > 0 && k0 == kk_prev && l0 == l_prev && kk_prev > 0 && l_prev > 0;
+        if (nested) {
+            RhoNestedSide su{}, sv{};
+            su.kk = kk; su.kkp = kk_prev; su.Uc = w.sc.Uc; su.ldc = kk; su.Ucp = w.UcPrev; su.ldcp = kk_prev;
+            su.A = w.Amat; su.G = w.GU; su.scratch = w.nestU;
+            sv.kk = l; sv.kkp = l_prev; sv.Uc = w.sc.Vc; sv.ldc = l; sv.Ucp = w.VcPrev; sv.ldcp = l_prev;
+            sv.A = w.Bmat; sv.G = w.GV; sv.scratch = w.nestV;
+            LRP_TRY(rho_nested_prep(ctx, rank, r_prev, su, sv));
+        }
+        // General case: the two sides run on the main and the auxiliary stream.
+        if (r_prev > 0 && !nested) {
             cudaStream_t main_stream = ctx->stream;
             ctx->stream = side;
             int rc_v = tall_gemm_t(ctx, n, Vk, ld, rank, Vp, ld, r_prev, w.Bmat, rank, 0, w.gemmt_ws2);
@@ -643,7 +660,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         RhoArgs ra{};
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
         ra.out = w.rho_out;
-        if (r_prev > 0) {
+        if (r_prev > 0 && !nested) {
             LRP_TRY(tall_gemm_t(ctx, n, Uk, ld, rank, Up, ld, r_prev, w.Amat, rank, 0, w.gemmt_ws));      // U side
             int rc_u = tall_resid_gram(ctx, n, Uk, ld, rank, w.Amat, rank, Up, ld, r_prev, w.GU, r_prev, w.gemmt_ws);
             if (rc_u < 0) return rc_u;
@@ -662,6 +679,9 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(h_eta, w.eta, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.Sprev, w.sc.S, sizeof(double) * rank, cudaMemcpyDeviceToDevice, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.UcPrev, w.sc.Uc, sizeof(double) * (size_t)kk * rank, cudaMemcpyDeviceToDevice, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(w.VcPrev, w.sc.Vc, sizeof(double) * (size_t)l * rank, cudaMemcpyDeviceToDevice, ctx->stream));
+        kk_prev = kk; l_prev = l;
         LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         cudaEvent_t e6 = ep.rec(ctx);
         const double rho = h_rho[0], snorm = h_rho[1], eta1 = h_eta[0], eta2 = h_eta[1];

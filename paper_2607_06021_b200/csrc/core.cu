@@ -488,6 +488,34 @@ rho_kernel(RhoArgs a) {
     }
 }
 
+struct RhoNestedArgs { int r, rp; RhoNestedSide side[2]; };
+
+__global__ void __launch_bounds__(CORE_NT)
+rho_nested_kernel(RhoNestedArgs a) {
+    const RhoNestedSide s = a.side[blockIdx.x];
+    const int tid = threadIdx.x, nt = blockDim.x, r = a.r, rp = a.rp;
+    for (int e = tid; e < r * rp; e += nt) {                     // A = Uc^T [Ucp; 0]
+        int i = e % r, t = e / r;
+        double acc = 0.0;
+        for (int c = 0; c < s.kkp; ++c) acc = fma(s.Uc[c + (size_t)i * s.ldc], s.Ucp[c + (size_t)t * s.ldcp], acc);
+        s.A[e] = acc;
+    }
+    __syncthreads();
+    for (int e = tid; e < s.kk * rp; e += nt) {                  // M = [Ucp; 0] - Uc A
+        int c = e % s.kk, t = e / s.kk;
+        double acc = c < s.kkp ? s.Ucp[c + (size_t)t * s.ldcp] : 0.0;
+        for (int i = 0; i < r; ++i) acc = fma(-s.Uc[c + (size_t)i * s.ldc], s.A[i + (size_t)t * r], acc);
+        s.scratch[e] = acc;
+    }
+    __syncthreads();
+    for (int e = tid; e < rp * rp; e += nt) {                    // G = M^T M
+        int t = e % rp, u = e / rp;
+        double acc = 0.0;
+        for (int c = 0; c < s.kk; ++c) acc = fma(s.scratch[c + (size_t)t * s.kk], s.scratch[c + (size_t)u * s.kk], acc);
+        s.G[e] = acc;
+    }
+}
+
 __global__ void snorm_kernel(int r, const double* S, double* out) {
     if (threadIdx.x == 0) {
         double sn = 0.0;
@@ -564,6 +592,15 @@ int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
     LRP_PROF(ctx, K_RHO, 0, 0);
     if (a.rp == 0) snorm_kernel<<<1, 32, 0, ctx->stream>>>(a.r, a.Sk, a.out);
     else rho_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+
+int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const RhoNestedSide& v) {
+    RhoNestedArgs a{};
+    a.r = r; a.rp = rp; a.side[0] = u; a.side[1] = v;
+    LRP_PROF(ctx, K_RHO, 0, 0);
+    rho_nested_kernel<<<2, CORE_NT, 0, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }

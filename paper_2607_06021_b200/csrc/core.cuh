@@ -42,6 +42,18 @@ struct RhoArgs {
 };
 int rho_small(lrp_ctx* ctx, const RhoArgs& a);
 
+// Nested case of the stop test: when last sweep's index list is a prefix of this sweep's, Q_{k-1} is the leading block of
+// Q_k (the driver keeps those columns), so U_{k-1} = Q_k [Uc_{k-1}; 0] and the operands of rho come from the small core
+// factors alone:  A = Uc_k^T [Uc_{k-1}; 0],  E_U = Q_k M with M = [Uc_{k-1}; 0] - Uc_k A,  GU = M^T M  (Q_k orthonormal).
+// One CTA per side (side 0: U, side 1: V).  scratch: kk * rp doubles per side.
+struct RhoNestedSide {
+    int kk, kkp;                                // rows of Uc_k, rows of Uc_{k-1} (kkp <= kk)
+    const double* Uc; int ldc;                  // kk x r
+    const double* Ucp; int ldcp;                // kkp x rp
+    double* A; double* G; double* scratch;      // r x rp (ld r), rp x rp (ld rp)
+};
+int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const RhoNestedSide& v);
+
 int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double rcond, unsigned char* mask);
 
 // top-`num` of scores[0..n) ordered by (score desc, index asc) -> idx_out (device).  ws: select_ws_bytes(ctx, n, num).
