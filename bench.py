@@ -242,7 +242,7 @@ def main():
     # measured DRAM traffic of that kernel class from the committed ncu capture (ratio to its algorithmic bytes), per launch
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r01c_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r01d_traffic.csv")) as fh:
             for row in csv.DictReader(fh):
                 if row["kernel"] == top["kernel"]:
                     ratio = float(row["dram_bytes_per_launch"]) / float(row["alg_bytes_per_launch"])

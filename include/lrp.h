@@ -171,6 +171,10 @@ typedef struct lrp_solve_info {
  * prune masks; the per-sweep counts are info->nI / nJ.
  * Optional spectral outputs (DEVICE, may be NULL): d_Uhat / d_Vhat (n x K_cap, ld = ld_hat) and d_Shat
  * (K_cap) receive the last spectral iterate before the final truncation (info->rank_per_sweep[sweeps-1] columns).
+ * Between sweeps the fibers of surviving indices are not resampled: the leading columns of a fiber block that repeat
+ * the previous block keep their Q and R factors, and when the previous index lists are prefixes of the current ones
+ * rho (Alg. 4 line 24) is evaluated from the small core factors (readings R4, R5; the
+ * environment variables LRP_NO_QR_REUSE / LRP_NO_NESTED_RHO, read per call, switch either off for comparison).
  * Synchronous: complete on return.  Returns LRP_WARN_NOCONV when the stop test never passed. */
 int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
                          const double* d_UF, int64_t ldu, const double* d_SF, const double* d_VF, int64_t ldv,

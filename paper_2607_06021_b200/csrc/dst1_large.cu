@@ -232,20 +232,30 @@ dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restr
 // reached through the shorter chain and the small tail of a decaying spectrum is summed from small terms only.
 // sums: per column nchunks chunk sums + 1 slot for X_{N-1}; part: per column [nB][nchunks] partial sums of sweep B.
 
-// per column (one CTA): chunk sums from sweep B's partials, then chunks c < nch/2 get the exclusive prefix of the chunk
-// sums, chunks c >= nch/2 the exclusive suffix (sum of the chunks above them, accumulated from the top)
+// chunk sums from sweep B's partials: one thread per chunk, fixed order over the nB contributing CTAs (deterministic)
+__global__ void __launch_bounds__(128)
+dst1_chunkreduce_kernel(int nchunks, int nB, const double* __restrict__ part, double* __restrict__ sums) {
+    const int ch = blockIdx.x * 128 + threadIdx.x;
+    if (ch >= nchunks) return;
+    const double* pc = part + (int64_t)blockIdx.y * nB * nchunks + ch;
+    double acc = 0.0;
+    int b = 0;
+    for (; b + 4 <= nB; b += 4) {
+        double v0 = pc[(int64_t)b * nchunks], v1 = pc[(int64_t)(b + 1) * nchunks];
+        double v2 = pc[(int64_t)(b + 2) * nchunks], v3 = pc[(int64_t)(b + 3) * nchunks];
+        acc += v0; acc += v1; acc += v2; acc += v3;
+    }
+    for (; b < nB; ++b) acc += pc[(int64_t)b * nchunks];
+    sums[(int64_t)blockIdx.y * (nchunks + 1) + ch] = acc;
+}
+
+// per column (one CTA): chunks c < nch/2 get the exclusive prefix of the chunk sums, chunks c >= nch/2 the exclusive
+// suffix (sum of the chunks above them, accumulated from the top)
 __global__ void __launch_bounds__(1024)
-dst1_scansums_kernel(int nchunks, int nB, const double* __restrict__ part, double* __restrict__ sums) {
+dst1_scansums_kernel(int nchunks, double* __restrict__ sums) {
     double* s = sums + (int64_t)blockIdx.x * (nchunks + 1);
-    const double* pc = part + (int64_t)blockIdx.x * nB * nchunks;
     __shared__ double wsum[32];
     __shared__ double tot;
-    for (int ch = threadIdx.x; ch < nchunks; ch += 1024) {
-        double acc = 0.0;
-        for (int b = 0; b < nB; ++b) acc += pc[(int64_t)b * nchunks + ch];
-        s[ch] = acc;
-    }
-    __syncthreads();
     const int half = nchunks / 2;
     for (int dir = 0; dir < 2; ++dir) {
         const int cnt = dir == 0 ? half : nchunks - half;
@@ -442,8 +452,11 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
         double* o = d_out + (int64_t)c0 * ld_out;
         LRP_TRY(dispatch_pa(p.q1, p.tla, ctx, log2N, cols, d_in + (int64_t)c0 * ld_in, ld_in, W));
         LRP_TRY(dispatch_pb(p.q2, p.tlb, ctx, log2N, cols, W, scale, sums + p.nch, p.nch + 1, part));
+        LRP_PROF(ctx, K_DST_CHUNKSUM, 8.0 * p.nB * p.nch * cols, 0);
+        dst1_chunkreduce_kernel<<<dim3((p.nch + 127) / 128, cols), 128, 0, ctx->stream>>>(p.nch, p.nB, part, sums);
+        LRP_LAUNCHED(ctx);
         LRP_PROF(ctx, K_DST_SCANSUMS, 0, 0);
-        dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(p.nch, p.nB, part, sums);
+        dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(p.nch, sums);
         LRP_LAUNCHED(ctx);
         LRP_PROF(ctx, K_DST_FINISH, 16.0 * N * cols, 0);
         dst1_scanapply_kernel<<<dim3(p.nch, cols), SC_NT, SC_SMEM, ctx->stream>>>(log2N, p.q1, W, o, ld_out, sums);

@@ -264,9 +264,10 @@ class Context:
         dev = UF.device
         Kc = max(2 * (max_rank + oversample), rF + oversample + 1)
         self.ensure_workspace(self.lib.lrp_workspace_bytes(n, rF, max_rank, oversample))
-        UW = torch.zeros((max_rank, n), dtype=torch.float64, device=dev)
-        VW = torch.zeros((max_rank, n), dtype=torch.float64, device=dev)
-        SW = torch.zeros(max_rank, dtype=torch.float64, device=dev)
+        # outputs: only the first info.rank columns are defined (and returned); no fill kernels on the solve's path
+        UW = torch.empty((max_rank, n), dtype=torch.float64, device=dev)
+        VW = torch.empty((max_rank, n), dtype=torch.float64, device=dev)
+        SW = torch.empty(max_rank, dtype=torch.float64, device=dev)
         o = SolveOpts()
         o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
         keep = []
@@ -295,9 +296,9 @@ class Context:
         tkI = np.zeros(MAX_SWEEPS_INFO * Kc, dtype=np.uint8); tkJ = np.zeros_like(tkI)
         Uhat = Vhat = Shat = None
         if want_spectral:
-            Uhat = torch.zeros((Kc, n), dtype=torch.float64, device=dev)
-            Vhat = torch.zeros((Kc, n), dtype=torch.float64, device=dev)
-            Shat = torch.zeros(Kc, dtype=torch.float64, device=dev)
+            Uhat = torch.empty((Kc, n), dtype=torch.float64, device=dev)
+            Vhat = torch.empty((Kc, n), dtype=torch.float64, device=dev)
+            Shat = torch.empty(Kc, dtype=torch.float64, device=dev)
         rc = self._check(self.lib.lrp_cross_deim_solve(
             self.h, n, rF, _ptr(UF), ldu, _ptr(SF), _ptr(VF), ldv, C.byref(o), _ptr(UW), n, _ptr(SW), _ptr(VW), n,
             C.byref(info), trI.ctypes.data, trJ.ctypes.data, tkI.ctypes.data, tkJ.ctypes.data,
