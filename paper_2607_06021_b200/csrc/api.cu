@@ -115,9 +115,11 @@ int validate_indices(const int32_t* h, int cnt, int64_t n) {
 }
 
 // ------------------------------------------------------------------------------------------------ solve workspace
+constexpr int NREST_MAX = 16;      // dropped trailing Q columns of the previous fiber block kept aside for the nested stop test
 struct SolveWs {
     double *UhF, *VhF, *Cb, *Rb, *Ua, *Va, *Ub, *Vb, *scoresU, *scoresV;
     double *UcPrev, *VcPrev, *nestU, *nestV;      // previous core factors and scratch of the nested stop test
+    double *QrestU, *QrestV, *TU, *TV, *GpU, *GpV;   // dropped trailing Q columns (n x NREST_MAX), T = Q^T Q_rest, P^T P
     double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev, *Rlev2;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
     unsigned char *mask, *mask2;
@@ -136,7 +138,10 @@ struct SolveWs {
         GU = ar.take<double>((size_t)Kc * Kc); GV = ar.take<double>((size_t)Kc * Kc);
         Rlev = ar.take<double>((size_t)Kc * Kc); Rlev2 = ar.take<double>((size_t)Kc * Kc);
         UcPrev = ar.take<double>((size_t)Kc * Kc); VcPrev = ar.take<double>((size_t)Kc * Kc);
-        nestU = ar.take<double>((size_t)Kc * Kc); nestV = ar.take<double>((size_t)Kc * Kc);
+        nestU = ar.take<double>(2 * (size_t)Kc * Kc); nestV = ar.take<double>(2 * (size_t)Kc * Kc);
+        QrestU = ar.take<double>(ld * NREST_MAX); QrestV = ar.take<double>(ld * NREST_MAX);
+        TU = ar.take<double>((size_t)Kc * NREST_MAX); TV = ar.take<double>((size_t)Kc * NREST_MAX);
+        GpU = ar.take<double>(NREST_MAX * NREST_MAX); GpV = ar.take<double>(NREST_MAX * NREST_MAX);
         rho_out = ar.take<double>(8); eta = ar.take<double>(8);
         eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
         eta_work = ar.take<double>(2 * eta_stride);
@@ -560,13 +565,20 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         // the two sides of a sweep are independent until the small core: they run on the main and the auxiliary stream
         // (every tall kernel here is latency-bound well below the HBM peak, so two in flight overlap usefully)
         cudaStream_t side = ctx->prof_on == 1 ? ctx->stream : ctx->aux;      // profiling: serial, clean per-kernel event times
-        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
-        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         int k0 = 0, l0 = 0;
         if (reuse_qr) {
             while (k0 < kk && k0 < (int)J_fact.size() && J_fact[k0] == J_k[k0]) ++k0;
             while (l0 < l && l0 < (int)I_fact.size() && I_fact[l0] == I_k[l0]) ++l0;
         }
+        // nested stop test (reading R5): the previous block's Q columns after the common prefix are about to be
+        // overwritten; up to NREST_MAX of them are set aside (they carry part of U_{k-1})
+        const int nrJ = (int)J_fact.size() - k0, nrI = (int)I_fact.size() - l0;
+        const bool nested = nested_rho && r_prev > 0 && k0 > 0 && l0 > 0 && (int)J_fact.size() == kk_prev &&
+                            (int)I_fact.size() == l_prev && nrJ <= NREST_MAX && nrI <= NREST_MAX;
+        if (nested && nrJ > 0) LRP_TRY(tall_copy(ctx, n, nrJ, w.Cb + (int64_t)k0 * ld, ld, w.QrestU, ld));
+        if (nested && nrI > 0) LRP_TRY(tall_copy(ctx, n, nrI, w.Rb + (int64_t)l0 * ld, ld, w.QrestV, ld));
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
         if (kk > k0) LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ + k0, kk - k0, w.Cb + (int64_t)k0 * ld, ld));
         if (l > l0) LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
         cudaEvent_t e2 = ep.rec(ctx);
@@ -626,15 +638,39 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         LRP_ON_STREAM(ctx, side, rebuild(ctx, n, w.Rb, ld, l, w.sc.Vc, l, rank, Vk, ld, w.scoresV));
         cudaEvent_t e5 = ep.rec(ctx);
         // ---- O10: rho (factored, reading Q13), indicator.
-        // Nested case: last sweep's lists are prefixes of this sweep's and their Q columns were kept, so U_{k-1}, V_{k-1}
-        // lie in the spans of Q_k, Z_k and rho needs the small core factors only (no pass over the tall iterates).
-        const bool nested = nested_rho && r_prev > 0 && k0 == kk_prev && l0 == l_prev && kk_prev > 0 && l_prev > 0;
+        // Nested case: last sweep's lists are (up to a few dropped trailing entries) prefixes of this sweep's and the Q
+        // columns of the common prefix were kept: rho needs the small core factors and, for the dropped columns, three
+        // narrow passes (T = Q_k^T Q_rest, P = Q_rest - Q_k T, P^T P) instead of the contractions over the tall iterates.
         if (nested) {
+            if (nrI > 0) {
+                cudaStream_t main_stream = ctx->stream;
+                ctx->stream = side;
+                int rc_v = tall_gemm_t(ctx, n, w.Rb, ld, l, w.QrestV, ld, nrI, w.TV, l, 0, w.gemmt_ws2);
+                if (rc_v >= 0) {
+                    TallGemmArgs g{};
+                    g.n = n; g.k = l; g.m = nrI; g.mode = TG_SUBTRACT; g.A = w.Rb; g.lda = ld; g.B = w.TV; g.ldb = l;
+                    g.Cin = w.QrestV; g.ldc = ld; g.Out = w.QrestV; g.ldo = ld;
+                    rc_v = tall_gemm(ctx, g);
+                }
+                if (rc_v >= 0) rc_v = tall_gemm_t(ctx, n, w.QrestV, ld, nrI, w.QrestV, ld, nrI, w.GpV, nrI, 0, w.gemmt_ws2);
+                ctx->stream = main_stream;
+                if (rc_v < 0) return rc_v;
+            }
+            LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
+            if (nrJ > 0) {
+                LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, kk, w.QrestU, ld, nrJ, w.TU, kk, 0, w.gemmt_ws));
+                TallGemmArgs g{};
+                g.n = n; g.k = kk; g.m = nrJ; g.mode = TG_SUBTRACT; g.A = w.Cb; g.lda = ld; g.B = w.TU; g.ldb = kk;
+                g.Cin = w.QrestU; g.ldc = ld; g.Out = w.QrestU; g.ldo = ld;
+                LRP_TRY(tall_gemm(ctx, g));
+                LRP_TRY(tall_gemm_t(ctx, n, w.QrestU, ld, nrJ, w.QrestU, ld, nrJ, w.GpU, nrJ, 0, w.gemmt_ws));
+            }
+            LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
             RhoNestedSide su{}, sv{};
-            su.kk = kk; su.kkp = kk_prev; su.Uc = w.sc.Uc; su.ldc = kk; su.Ucp = w.UcPrev; su.ldcp = kk_prev;
-            su.A = w.Amat; su.G = w.GU; su.scratch = w.nestU;
-            sv.kk = l; sv.kkp = l_prev; sv.Uc = w.sc.Vc; sv.ldc = l; sv.Ucp = w.VcPrev; sv.ldcp = l_prev;
-            sv.A = w.Bmat; sv.G = w.GV; sv.scratch = w.nestV;
+            su.kk = kk; su.kkp = kk_prev; su.k0 = k0; su.Uc = w.sc.Uc; su.ldc = kk; su.Ucp = w.UcPrev; su.ldcp = kk_prev;
+            su.T = w.TU; su.Gp = w.GpU; su.A = w.Amat; su.G = w.GU; su.scratch = w.nestU;
+            sv.kk = l; sv.kkp = l_prev; sv.k0 = l0; sv.Uc = w.sc.Vc; sv.ldc = l; sv.Ucp = w.VcPrev; sv.ldcp = l_prev;
+            sv.T = w.TV; sv.Gp = w.GpV; sv.A = w.Bmat; sv.G = w.GV; sv.scratch = w.nestV;
             LRP_TRY(rho_nested_prep(ctx, rank, r_prev, su, sv));
         }
         // General case: the two sides run on the main and the auxiliary stream.

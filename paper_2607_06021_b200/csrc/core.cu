@@ -494,24 +494,39 @@ __global__ void __launch_bounds__(CORE_NT)
 rho_nested_kernel(RhoNestedArgs a) {
     const RhoNestedSide s = a.side[blockIdx.x];
     const int tid = threadIdx.x, nt = blockDim.x, r = a.r, rp = a.rp;
-    for (int e = tid; e < r * rp; e += nt) {                     // A = Uc^T [Ucp; 0]
+    const int nrest = s.kkp - s.k0;
+    double* Y = s.scratch; double* M = s.scratch + (size_t)s.kk * rp;
+    const double* Ucr = s.Ucp + s.k0;                            // Uc_rest(q, t) = Ucr[q + t * ldcp]
+    for (int e = tid; e < s.kk * rp; e += nt) {                  // Y = [Uc_pref; 0] + T Uc_rest
+        int c = e % s.kk, t = e / s.kk;
+        double acc = c < s.k0 ? s.Ucp[c + (size_t)t * s.ldcp] : 0.0;
+        for (int q = 0; q < nrest; ++q) acc = fma(s.T[c + (size_t)q * s.kk], Ucr[q + (size_t)t * s.ldcp], acc);
+        Y[e] = acc;
+    }
+    __syncthreads();
+    for (int e = tid; e < r * rp; e += nt) {                     // A = Uc^T Y
         int i = e % r, t = e / r;
         double acc = 0.0;
-        for (int c = 0; c < s.kkp; ++c) acc = fma(s.Uc[c + (size_t)i * s.ldc], s.Ucp[c + (size_t)t * s.ldcp], acc);
+        for (int c = 0; c < s.kk; ++c) acc = fma(s.Uc[c + (size_t)i * s.ldc], Y[c + (size_t)t * s.kk], acc);
         s.A[e] = acc;
     }
     __syncthreads();
-    for (int e = tid; e < s.kk * rp; e += nt) {                  // M = [Ucp; 0] - Uc A
+    for (int e = tid; e < s.kk * rp; e += nt) {                  // M = Y - Uc A
         int c = e % s.kk, t = e / s.kk;
-        double acc = c < s.kkp ? s.Ucp[c + (size_t)t * s.ldcp] : 0.0;
+        double acc = Y[e];
         for (int i = 0; i < r; ++i) acc = fma(-s.Uc[c + (size_t)i * s.ldc], s.A[i + (size_t)t * r], acc);
-        s.scratch[e] = acc;
+        M[e] = acc;
     }
     __syncthreads();
-    for (int e = tid; e < rp * rp; e += nt) {                    // G = M^T M
+    for (int e = tid; e < rp * rp; e += nt) {                    // G = M^T M + Uc_rest^T (P^T P) Uc_rest
         int t = e % rp, u = e / rp;
         double acc = 0.0;
-        for (int c = 0; c < s.kk; ++c) acc = fma(s.scratch[c + (size_t)t * s.kk], s.scratch[c + (size_t)u * s.kk], acc);
+        for (int c = 0; c < s.kk; ++c) acc = fma(M[c + (size_t)t * s.kk], M[c + (size_t)u * s.kk], acc);
+        for (int q = 0; q < nrest; ++q) {
+            double w = 0.0;
+            for (int q2 = 0; q2 < nrest; ++q2) w = fma(s.Gp[q + (size_t)q2 * nrest], Ucr[q2 + (size_t)u * s.ldcp], w);
+            acc = fma(Ucr[q + (size_t)t * s.ldcp], w, acc);
+        }
         s.G[e] = acc;
     }
 }

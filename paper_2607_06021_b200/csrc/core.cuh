@@ -42,14 +42,20 @@ struct RhoArgs {
 };
 int rho_small(lrp_ctx* ctx, const RhoArgs& a);
 
-// Nested case of the stop test: when last sweep's index list is a prefix of this sweep's, Q_{k-1} is the leading block of
-// Q_k (the driver keeps those columns), so U_{k-1} = Q_k [Uc_{k-1}; 0] and the operands of rho come from the small core
-// factors alone:  A = Uc_k^T [Uc_{k-1}; 0],  E_U = Q_k M with M = [Uc_{k-1}; 0] - Uc_k A,  GU = M^T M  (Q_k orthonormal).
-// One CTA per side (side 0: U, side 1: V).  scratch: kk * rp doubles per side.
+// Nested case of the stop test: last sweep's index list is, up to `nrest` = kkp - k0 dropped trailing entries, a prefix
+// of this sweep's, and the driver kept the Q columns of the common prefix (k0 columns), so
+//   U_{k-1} = Q_k Y + P Uc_rest,   Y = [Uc_pref; 0] + T Uc_rest,   T = Q_k^T Q_rest,   P = Q_rest - Q_k T  (P _|_ Q_k),
+// with Uc_pref / Uc_rest the first k0 / last nrest rows of Uc_{k-1} and Q_rest the dropped Q columns (set aside by the
+// driver).  The operands of rho then come from small matrices:
+//   A = U_k^T U_{k-1} = Uc_k^T Y,   E_U = Q_k M + P Uc_rest with M = Y - Uc_k A,   GU = M^T M + Uc_rest^T (P^T P) Uc_rest.
+// nrest = 0 (nothing dropped): Y = [Uc_{k-1}; 0], no T, no P.  One CTA per side (side 0: U, side 1: V).
+// scratch: 2 * kk * rp doubles per side.
 struct RhoNestedSide {
-    int kk, kkp;                                // rows of Uc_k, rows of Uc_{k-1} (kkp <= kk)
+    int kk, kkp, k0;                            // rows of Uc_k, rows of Uc_{k-1}, common prefix (k0 <= kkp, k0 <= kk)
     const double* Uc; int ldc;                  // kk x r
     const double* Ucp; int ldcp;                // kkp x rp
+    const double* T;                            // kk x nrest (ld kk), unused when nrest = 0
+    const double* Gp;                           // nrest x nrest (ld nrest) = P^T P
     double* A; double* G; double* scratch;      // r x rp (ld r), rp x rp (ld rp)
 };
 int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const RhoNestedSide& v);
