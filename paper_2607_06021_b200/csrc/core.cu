@@ -456,19 +456,19 @@ rho_kernel(RhoArgs a) {
     for (int e = tid; e < r * r; e += nt) {
         int i = e % r, j = e / r;
         double v = (i == j) ? a.Sk[i] : 0.0;
+#pragma unroll 4
         for (int t = 0; t < rp; ++t) v = fma(-a.A[i + (size_t)t * r] * a.Sp[t], a.B[j + (size_t)t * r], v);
         acc = fma(v, v, acc);
     }
-    // term2: ||A S' E_V^T||_F^2 = sum_i sum_{t,u} A(i,t) Sp(t) GV(t,u) Sp(u) A(i,u);  term3 likewise with B, GU
-    for (int e = tid; e < 2 * r; e += nt) {
-        int i = e % r; const double* Mx = e < r ? a.A : a.B; const double* G = e < r ? a.GV : a.GU;
-        double s = 0.0;
-        for (int t = 0; t < rp; ++t) {
-            double w = 0.0;
-            for (int u = 0; u < rp; ++u) w = fma(G[t + (size_t)u * rp], a.Sp[u] * Mx[i + (size_t)u * r], w);
-            s = fma(Mx[i + (size_t)t * r] * a.Sp[t], w, s);
-        }
-        acc += s > 0.0 ? s : 0.0;
+    // term2: ||A S' E_V^T||_F^2 = sum_i sum_{t,u} A(i,t) Sp(t) GV(t,u) Sp(u) A(i,u);  term3 likewise with B, GU.
+    // One (side, i, t) per thread step; the total is non-negative up to rounding (clamped with the sum below).
+    for (int e = tid; e < 2 * r * rp; e += nt) {
+        const int side = e / (r * rp), rem = e % (r * rp), i = rem % r, t = rem / r;
+        const double* Mx = side == 0 ? a.A : a.B; const double* G = side == 0 ? a.GV : a.GU;
+        double w = 0.0;
+#pragma unroll 4
+        for (int u = 0; u < rp; ++u) w = fma(G[t + (size_t)u * rp], a.Sp[u] * Mx[i + (size_t)u * r], w);
+        acc = fma(Mx[i + (size_t)t * r] * a.Sp[t], w, acc);
     }
     // term4: ||E_U S' E_V^T||_F^2 = sum_{t,u} GU(t,u) Sp(t) Sp(u) GV(t,u)
     for (int e = tid; e < rp * rp; e += nt) {
@@ -488,44 +488,72 @@ rho_kernel(RhoArgs a) {
     }
 }
 
-struct RhoNestedArgs { int r, rp; RhoNestedSide side[2]; };
+struct RhoNestedArgs { int r, rp, use_smem; RhoNestedSide s0, s1; };
 
+// use_smem: Y, M, A and compact copies of Uc, Ucp live in dynamic shared memory (small cores); otherwise Y, M in the
+// global scratch and the factors are read in place.
+// dot product with four independent partial sums (the single chain is latency-bound: one DFMA per ~8 cycles)
+template <typename FA, typename FB>
+__device__ __forceinline__ double dot4(int len, FA fa, FB fb) {
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int c = 0;
+    for (; c + 4 <= len; c += 4) {
+        a0 = fma(fa(c), fb(c), a0); a1 = fma(fa(c + 1), fb(c + 1), a1);
+        a2 = fma(fa(c + 2), fb(c + 2), a2); a3 = fma(fa(c + 3), fb(c + 3), a3);
+    }
+    for (; c < len; ++c) a0 = fma(fa(c), fb(c), a0);
+    return (a0 + a1) + (a2 + a3);
+}
+
+template <bool USE_SMEM>
 __global__ void __launch_bounds__(CORE_NT)
 rho_nested_kernel(RhoNestedArgs a) {
-    const RhoNestedSide s = a.side[blockIdx.x];
+    extern __shared__ __align__(16) double dyn_smem[];
+    // field-wise select (a dynamically indexed parameter array would live in local memory)
+    const RhoNestedSide s = blockIdx.x == 0 ? a.s0 : a.s1;
     const int tid = threadIdx.x, nt = blockDim.x, r = a.r, rp = a.rp;
     const int nrest = s.kkp - s.k0;
     double* Y = s.scratch; double* M = s.scratch + (size_t)s.kk * rp;
-    const double* Ucr = s.Ucp + s.k0;                            // Uc_rest(q, t) = Ucr[q + t * ldcp]
+    double* Aw = s.A;
+    const double* Uc = s.Uc; int ldc = s.ldc;
+    const double* Ucp = s.Ucp; int ldcp = s.ldcp;
+    if (USE_SMEM) {
+        Y = dyn_smem; M = Y + (size_t)s.kk * rp; Aw = M + (size_t)s.kk * rp;
+        double* uc = Aw + (size_t)r * rp; double* ucp = uc + (size_t)s.kk * r;
+        for (int e = tid; e < s.kk * r; e += nt) uc[e] = s.Uc[(e % s.kk) + (size_t)(e / s.kk) * s.ldc];
+        for (int e = tid; e < s.kkp * rp; e += nt) ucp[e] = s.Ucp[(e % s.kkp) + (size_t)(e / s.kkp) * s.ldcp];
+        Uc = uc; ldc = s.kk; Ucp = ucp; ldcp = s.kkp;
+        __syncthreads();
+    }
+    const double* Ucr = Ucp + s.k0;                              // Uc_rest(q, t) = Ucr[q + t * ldcp]
     for (int e = tid; e < s.kk * rp; e += nt) {                  // Y = [Uc_pref; 0] + T Uc_rest
         int c = e % s.kk, t = e / s.kk;
-        double acc = c < s.k0 ? s.Ucp[c + (size_t)t * s.ldcp] : 0.0;
-        for (int q = 0; q < nrest; ++q) acc = fma(s.T[c + (size_t)q * s.kk], Ucr[q + (size_t)t * s.ldcp], acc);
+        double acc = c < s.k0 ? Ucp[c + (size_t)t * ldcp] : 0.0;
+        for (int q = 0; q < nrest; ++q) acc = fma(s.T[c + (size_t)q * s.kk], Ucr[q + (size_t)t * ldcp], acc);
         Y[e] = acc;
     }
     __syncthreads();
     for (int e = tid; e < r * rp; e += nt) {                     // A = Uc^T Y
         int i = e % r, t = e / r;
-        double acc = 0.0;
-        for (int c = 0; c < s.kk; ++c) acc = fma(s.Uc[c + (size_t)i * s.ldc], Y[c + (size_t)t * s.kk], acc);
-        s.A[e] = acc;
+        const double* ua = Uc + (size_t)i * ldc; const double* ya = Y + (size_t)t * s.kk;
+        Aw[e] = dot4(s.kk, [&](int c) { return ua[c]; }, [&](int c) { return ya[c]; });
     }
     __syncthreads();
     for (int e = tid; e < s.kk * rp; e += nt) {                  // M = Y - Uc A
         int c = e % s.kk, t = e / s.kk;
-        double acc = Y[e];
-        for (int i = 0; i < r; ++i) acc = fma(-s.Uc[c + (size_t)i * s.ldc], s.A[i + (size_t)t * r], acc);
-        M[e] = acc;
+        const double* ua = Uc + c; const double* aa = Aw + (size_t)t * r;
+        M[e] = Y[e] - dot4(r, [&](int i) { return ua[(size_t)i * ldc]; }, [&](int i) { return aa[i]; });
     }
+    if (USE_SMEM) for (int e = tid; e < r * rp; e += nt) s.A[e] = Aw[e];
     __syncthreads();
     for (int e = tid; e < rp * rp; e += nt) {                    // G = M^T M + Uc_rest^T (P^T P) Uc_rest
         int t = e % rp, u = e / rp;
-        double acc = 0.0;
-        for (int c = 0; c < s.kk; ++c) acc = fma(M[c + (size_t)t * s.kk], M[c + (size_t)u * s.kk], acc);
+        const double* mt = M + (size_t)t * s.kk; const double* mu = M + (size_t)u * s.kk;
+        double acc = dot4(s.kk, [&](int c) { return mt[c]; }, [&](int c) { return mu[c]; });
         for (int q = 0; q < nrest; ++q) {
             double w = 0.0;
-            for (int q2 = 0; q2 < nrest; ++q2) w = fma(s.Gp[q + (size_t)q2 * nrest], Ucr[q2 + (size_t)u * s.ldcp], w);
-            acc = fma(Ucr[q + (size_t)t * s.ldcp], w, acc);
+            for (int q2 = 0; q2 < nrest; ++q2) w = fma(s.Gp[q + (size_t)q2 * nrest], Ucr[q2 + (size_t)u * ldcp], w);
+            acc = fma(Ucr[q + (size_t)t * ldcp], w, acc);
         }
         s.G[e] = acc;
     }
@@ -613,9 +641,16 @@ int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
 
 int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const RhoNestedSide& v) {
     RhoNestedArgs a{};
-    a.r = r; a.rp = rp; a.side[0] = u; a.side[1] = v;
+    a.r = r; a.rp = rp; a.s0 = u; a.s1 = v;
+    auto need = [&](const RhoNestedSide& s) { return sizeof(double) * ((size_t)2 * s.kk * rp + (size_t)r * rp + (size_t)s.kk * r + (size_t)s.kkp * rp); };
+    size_t smem = need(u) > need(v) ? need(u) : need(v);
+    a.use_smem = smem <= (size_t)200 * 1024 ? 1 : 0;
+    if (!a.use_smem) smem = 0;
+    if (smem > 48 * 1024)
+        LRP_CUDA(ctx, cudaFuncSetAttribute(rho_nested_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_RHO, 0, 0);
-    rho_nested_kernel<<<2, CORE_NT, 0, ctx->stream>>>(a);
+    if (a.use_smem) rho_nested_kernel<true><<<2, CORE_NT, smem, ctx->stream>>>(a);
+    else rho_nested_kernel<false><<<2, CORE_NT, 0, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
