@@ -37,7 +37,7 @@ __host__ __device__ inline int mg_kp(int k) {         // padded k: multiple of 4
 // a thread owns row PAIRS and, when the operands are 16-byte aligned with even leading dimensions (VEC), moves them
 // with 128-bit loads / stores (the output-row order of an MMA is bookkeeping only).
 template <int NJ, bool VEC>
-__global__ void __launch_bounds__(MG_THREADS, NJ == 2 ? 5 : 4)
+__global__ void __launch_bounds__(MG_THREADS, NJ == 2 ? 5 : (NJ <= 4 ? 4 : 3))
 tall_gemm_mma_kernel(TallGemmArgs p) {
     constexpr int MG_CT = 8 * NJ;
     extern __shared__ __align__(16) double smem[];
@@ -397,19 +397,24 @@ tall_resid_gram_kernel(int64_t n, const double* __restrict__ A, int64_t lda, int
 
 int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
     if (p.n <= 0 || p.m <= 0) return LRP_OK;
-    const int nj = p.m <= 16 ? 2 : 4;
+    // column tiles of 8 nj: every tile pass re-reads A, so 33..48 columns (the rebuild U = Q Uc, the first sweep's
+    // fibers) go in ONE pass of nj = 5 / 6 instead of two of nj = 4
+    const int tiles = (p.m + 7) / 8;
+    const int nj = p.m <= 16 ? 2 : (tiles == 5 ? 5 : (tiles == 6 ? 6 : 4));
     size_t smem = sizeof(double) * ((size_t)(8 * nj) * mg_kp(p.k > 0 ? p.k : 1) + 8 * nj);
     auto al16 = [](const void* q) { return ((uintptr_t)q & 15u) == 0; };
     const bool vec = (p.lda % 2 == 0) && (p.ldo % 2 == 0) && al16(p.A) && al16(p.Out) &&
                      (p.mode != TG_SUBTRACT || ((p.ldc % 2 == 0) && al16(p.Cin)));
     void (*kern)(TallGemmArgs) = nj == 2 ? (vec ? tall_gemm_mma_kernel<2, true> : tall_gemm_mma_kernel<2, false>)
+                               : nj == 5 ? (vec ? tall_gemm_mma_kernel<5, true> : tall_gemm_mma_kernel<5, false>)
+                               : nj == 6 ? (vec ? tall_gemm_mma_kernel<6, true> : tall_gemm_mma_kernel<6, false>)
                                          : (vec ? tall_gemm_mma_kernel<4, true> : tall_gemm_mma_kernel<4, false>);
     if (smem > 48 * 1024) {
         if (smem > (size_t)ctx->smem_optin) return LRP_ERR_BADARG;
         LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
-    const int64_t resident = 148 * (nj == 2 ? 5 : 4);   // persistent over row slabs (B staged once per column tile per CTA):
+    const int64_t resident = 148 * (nj == 2 ? 5 : (nj <= 4 ? 4 : 3));   // persistent over row slabs (B staged once per column tile per CTA):
     if (grid > resident) grid = resident;            // exactly one resident wave, so that the slabs are balanced
     LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
              8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
