@@ -151,7 +151,13 @@ typedef struct lrp_solve_opts {
     const uint8_t* h_replay_keepI;  /* concatenated prune masks (1 = survives), may be NULL -> decide */
     const uint8_t* h_replay_keepJ;
     int32_t replay_final_rank;      /* > 0: use this final rank */
+    int32_t flags;                  /* bit mask of LRP_FLAG_* below; 0 = default path */
 } lrp_solve_opts;
+
+/* lrp_solve_opts.flags: switch one of the driver's shortcuts off (comparison runs of the tests; results agree to rounding) */
+#define LRP_FLAG_NO_QR_REUSE    1   /* factor every fiber block from scratch (reading R4 off) */
+#define LRP_FLAG_NO_NESTED_RHO  2   /* rho always from the tall iterates (reading R5 off) */
+#define LRP_FLAG_NO_FUSED_RHO   4   /* rho's residual Gram matrix by an update sweep + a Gram sweep instead of the fused kernel */
 
 typedef struct lrp_solve_info {
     int32_t rank, sweeps, converged;
@@ -173,8 +179,8 @@ typedef struct lrp_solve_info {
  * (K_cap) receive the last spectral iterate before the final truncation (info->rank_per_sweep[sweeps-1] columns).
  * Between sweeps the fibers of surviving indices are not resampled: the leading columns of a fiber block that repeat
  * the previous block keep their Q and R factors, and when the previous index lists are prefixes of the current ones
- * rho (Alg. 4 line 24) is evaluated from the small core factors (readings R4, R5; the
- * environment variables LRP_NO_QR_REUSE / LRP_NO_NESTED_RHO, read per call, switch either off for comparison).
+ * rho (Alg. 4 line 24) is evaluated from the small core factors (readings R4, R5;
+ * opts->flags LRP_FLAG_NO_QR_REUSE / LRP_FLAG_NO_NESTED_RHO switch either off for comparison).
  * Synchronous: complete on return.  Returns LRP_WARN_NOCONV when the stop test never passed. */
 int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
                          const double* d_UF, int64_t ldu, const double* d_SF, const double* d_VF, int64_t ldv,

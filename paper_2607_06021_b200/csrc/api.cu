@@ -8,7 +8,6 @@
 #include "core.cuh"
 #include <math.h>
 #include <string.h>
-#include <stdlib.h>
 #include <vector>
 #include <algorithm>
 #include <new>
@@ -161,14 +160,25 @@ struct SolveWs {
     }
 };
 
+// timing events of a solve: owned by the ctx and created once (the first solves grow the pool, later ones reuse it)
 struct EventPool {
-    std::vector<cudaEvent_t> ev;
-    ~EventPool() { for (auto e : ev) cudaEventDestroy(e); }
-    cudaEvent_t rec(lrp_ctx* ctx) {
-        cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
-        ev.push_back(e); cudaEventRecord(e, ctx->stream); return e;
+    lrp_ctx* ctx; size_t used;
+    explicit EventPool(lrp_ctx* c) : ctx(c), used(0) {}
+    cudaEvent_t take() {
+        if (used == ctx->solve_ev->size()) {
+            cudaEvent_t e; if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+            ctx->solve_ev->push_back(e);
+        }
+        return (*ctx->solve_ev)[used++];
     }
+    cudaEvent_t rec(lrp_ctx* c) { cudaEvent_t e = take(); if (e) cudaEventRecord(e, c->stream); return e; }
     static float ms(cudaEvent_t a, cudaEvent_t b) { float t = 0.f; if (a && b) cudaEventElapsedTime(&t, a, b); return t; }
+};
+
+struct FlagsGuard {                   // lrp_solve_opts.flags are visible to the kernels' host wrappers during one solve
+    lrp_ctx* ctx;
+    FlagsGuard(lrp_ctx* c, int f) : ctx(c) { c->flags = f; }
+    ~FlagsGuard() { ctx->flags = 0; }
 };
 
 // Run `expr` (helpers launch on ctx->stream) on another stream.
@@ -184,12 +194,15 @@ void host_union(std::vector<int32_t>& cur, const int32_t* star, int nstar, int* 
     }
 }
 
-int final_rank_host(const double* S, int cnt, double tol, int max_rank, int tol_mode) {
+// Alg. 4 lines 30-31: r* = smallest r with sum_{c>r} S_c^2 < eps^2 (x sum S^2, reading Q15); returns
+// r = max(min(r*, r_max), 1) and r* itself through rstar_out (r* > r_max: the tolerance is not met, reading Q20).
+int final_rank_host(const double* S, int cnt, double tol, int max_rank, int tol_mode, int* rstar_out) {
     double tot = 0.0;
     for (int c = 0; c < cnt; ++c) tot += S[c] * S[c];
     const double thresh = tol * tol * (tol_mode == 0 ? tot : 1.0);
     int rstar = cnt; double tail = 0.0;
     for (int c = cnt - 1; c >= 0; --c) { tail += S[c] * S[c]; if (tail < thresh) rstar = c; else break; }
+    *rstar_out = rstar;
     int r = rstar < max_rank ? rstar : max_rank;
     return r < 1 ? 1 : r;
 }
@@ -211,6 +224,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda = 0; c->launches = 0;
     c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
+    c->flags = 0; c->solve_ev = new std::vector<cudaEvent_t>();
     c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr; c->d_counters = nullptr;
     if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->aux2, cudaStreamNonBlocking) != cudaSuccess ||
@@ -222,6 +236,8 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
         cudaMemset(c->d_counters, 0, 3 * 65 * sizeof(unsigned)) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    // one-time kernel attributes (dynamic shared memory opt-in): not on the per-call path
+    if (tall_qr_init(c) != LRP_OK || lrp_dst1_init(c) != LRP_OK) { lrp_destroy(c); return LRP_ERR_CUDA; }
     *out = c;
     return LRP_OK;
 }
@@ -229,6 +245,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
 int lrp_destroy(lrp_ctx* ctx) {
     if (!ctx) return LRP_OK;
     if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
+    if (ctx->solve_ev) { for (auto e : *ctx->solve_ev) cudaEventDestroy(e); delete ctx->solve_ev; }
     if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     if (ctx->aux2) cudaStreamDestroy(ctx->aux2);
@@ -322,8 +339,8 @@ size_t lrp_dst1_workspace_bytes(int64_t n, int32_t batch) {
 
 size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample) {
     if (check_n(n) != LRP_OK || rF < 1 || max_rank < 1 || oversample < 0) return 0;
-    int Kc = 2 * (max_rank + oversample);
-    if (Kc < rF + oversample + 1) Kc = rF + oversample + 1;
+    const int Kc = 2 * (max_rank + oversample);       // reading Q10; the first sweep needs rF + oversample + 1 <= K_cap
+    if (Kc < rF + oversample + 1) return 0;
     lrp_arena ar((void*)256, (size_t)-1 / 2);
     SolveWs w;
     w.carve(ar, nullptr, n, rF, Kc, max_rank);
@@ -449,8 +466,8 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     if (rF < 1 || !d_UF || !d_SF || !d_VF || !d_UW || !d_SW || !d_VW || ldu < n || ldv < n || lduw < n || ldvw < n) return LRP_ERR_BADARG;
     if (opts->max_rank < 1 || opts->oversample < 0 || opts->max_sweeps < 1 || !(opts->tol > 0.0)) return LRP_ERR_BADARG;
     const int max_rank = opts->max_rank, p_os = opts->oversample;
-    int Kc = 2 * (max_rank + p_os);
-    if (Kc < rF + p_os + 1) Kc = rF + p_os + 1;
+    const int Kc = 2 * (max_rank + p_os);             // reading Q10 (the oracle's K_cap): index lists are cut there
+    if (Kc < rF + p_os + 1) return LRP_ERR_BADARG;    // the first sweep's selection (rF + p_os indices + safeguard) must fit
     if (Kc > n || rF > n) return LRP_ERR_BADARG;
     const bool replay = opts->replay_sweeps > 0;
     const int max_sweeps = replay ? opts->replay_sweeps : opts->max_sweeps;
@@ -466,7 +483,8 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     const int64_t launches0 = ctx->launches;
     const int64_t ld = internal_ld(n);
     const double scale = sqrt(2.0 / (double)(n + 1));
-    EventPool ep;
+    EventPool ep(ctx);
+    FlagsGuard fguard(ctx, opts->flags);
     cudaEvent_t e_start = ep.rec(ctx);
 
     // O3: spectral RHS factors
@@ -491,8 +509,8 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     // columns of this sweep's fiber block that repeat last sweep's block in the same order keep their Q columns (still in
     // Cb / Rb) and their block of R; only the columns after the common prefix are sampled and factored.
     std::vector<int32_t> I_fact, J_fact;          // index lists whose Q factors Rb / Cb hold (empty: none)
-    const bool reuse_qr = getenv("LRP_NO_QR_REUSE") == nullptr;
-    const bool nested_rho = reuse_qr && getenv("LRP_NO_NESTED_RHO") == nullptr;
+    const bool reuse_qr = !(opts->flags & LRP_FLAG_NO_QR_REUSE);
+    const bool nested_rho = reuse_qr && !(opts->flags & LRP_FLAG_NO_NESTED_RHO);
     int kk_prev = 0, l_prev = 0;                  // sizes of the previous sweep's index lists (rows of UcPrev / VcPrev)
     std::vector<double> hS(Kc), hrC(Kc), hrR(Kc), hS_last;
     std::vector<uint8_t> keepI, keepJ;
@@ -583,8 +601,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (l > l0) LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
         cudaEvent_t e2 = ep.rec(ctx);
         // ---- O8: scross
-        cudaEvent_t e3 = nullptr;
-        { cudaEvent_t tmp; if (cudaEventCreate(&tmp) == cudaSuccess) { ep.ev.push_back(tmp); e3 = tmp; } }
+        cudaEvent_t e3 = ep.take();
         LRP_TRY(scross_factor(ctx, n, w.Cb, ld, kk, k0, w.Rb, ld, l, l0, w.dI, w.dJ, w.sc, hS.data(), hrC.data(), hrR.data(), &rank, &smin, e3));
         J_fact = J_k; I_fact = I_k;
         cudaEvent_t e4 = ep.rec(ctx);
@@ -736,9 +753,12 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (!replay && std::max(rho, ind) < thresh) { converged = true; break; }   // Alg. 4 line 26
     }
     // after the swap the last iterate lives in (Up, Vp), rank r_prev
-    int r;
+    int r, rstar = 0;
     if (replay && opts->replay_final_rank > 0) { r = opts->replay_final_rank; converged = true; }
-    else r = final_rank_host(hS_last.data(), r_prev, opts->tol, max_rank, opts->tol_mode);     // O11 over the kept values
+    else {
+        r = final_rank_host(hS_last.data(), r_prev, opts->tol, max_rank, opts->tol_mode, &rstar);     // O11 over the kept values
+        if (rstar > max_rank) converged = false;      // reading Q20: r* > r_max, the tolerance is not met by the truncated result
+    }
     if (r > r_prev) r = r_prev;
     if (r > max_rank) r = max_rank;
     cudaEvent_t e_inv0 = ep.rec(ctx);

@@ -32,6 +32,7 @@ struct lrp_ctx {
     int64_t launches;
     int sm_count;
     int smem_optin;
+    int flags;                            // lrp_solve_opts.flags of the solve in progress (LRP_FLAG_*), 0 otherwise
     int prof_on;
     int prof_pending;                     // kernel id whose start event is recorded, -1 if none
     lrp_prof prof[K_NUM];
@@ -43,6 +44,7 @@ struct lrp_ctx {
     std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)
     std::vector<int>* ev_id;
     size_t ev_used;
+    std::vector<cudaEvent_t>* solve_ev;   // timing events of lrp_cross_deim_solve (created once, reused by every solve)
 };
 
 // call right before a kernel launch: accounts the launch and, when profiling is on, records its start event
@@ -84,6 +86,10 @@ static inline void lrp_prof_end(lrp_ctx* ctx) {
 #define LRP_TRY(expr)                                                            \
     do { int rc_ = (expr); if (rc_ < 0) return rc_; } while (0)
 
+// SM count for grid sizing; without a ctx (host-side workspace sizing, no device query) an upper bound
+constexpr int LRP_SM_UPPER = 192;
+static inline int lrp_sm_count(const lrp_ctx* ctx) { return (ctx && ctx->sm_count > 0 && ctx->sm_count <= LRP_SM_UPPER) ? ctx->sm_count : LRP_SM_UPPER; }
+
 static inline size_t lrp_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 static inline int lrp_ilog2(int64_t x) { int p = 0; while ((int64_t(1) << p) < x) ++p; return p; }
@@ -105,7 +111,9 @@ struct lrp_arena {
 int lrp_dst1_impl(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, int64_t ld_in,
                   double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes);
 size_t lrp_dst1_ws_impl(int64_t n, int32_t batch);
+int lrp_dst1_init(lrp_ctx* ctx);      // one-time kernel attributes (lrp_create)
 // four-step regime (dst1_large.cu), N = n + 1 > 16384
 size_t dst1_large_ws(int64_t N, int32_t batch);
+int dst1_large_init(lrp_ctx* ctx);
 int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
                double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes);

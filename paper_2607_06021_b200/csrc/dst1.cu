@@ -141,7 +141,6 @@ dst1_small_kernel(int batch, const double* __restrict__ in, int64_t ld_in,
 template <int Q>
 int launch_small(lrp_ctx* ctx, int batch, const double* in, int64_t ld_in, double* out, int64_t ld_out, double scale) {
     using C = SmallCfg<Q>;
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_small_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     int grid = (batch + C::CPB - 1) / C::CPB;
     LRP_PROF(ctx, K_DST_SMALL, 16.0 * (2 * C::L - 1) * batch, 0);
     dst1_small_kernel<Q><<<grid, C::NT, C::SMEM, ctx->stream>>>(batch, in, ld_in, out, ld_out, scale);
@@ -164,7 +163,20 @@ int launch_small(lrp_ctx* ctx, int batch, const double* in, int64_t ld_in, doubl
 int dispatch_small(int q, lrp_ctx* ctx, int batch, const double* in, int64_t ld_in, double* out, int64_t ld_out, double scale) {
     LRP_Q_SWITCH(q, launch_small, ctx, batch, in, ld_in, out, ld_out, scale)
 }
+template <int Q>
+int init_small(lrp_ctx* ctx) {
+    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_small_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SmallCfg<Q>::SMEM));
+    return LRP_OK;
+}
 }  // namespace
+
+// dynamic shared memory opt-in of every DST-I kernel: once per context (lrp_create), not per call
+int lrp_dst1_init(lrp_ctx* ctx) {
+    LRP_TRY(init_small<5>(ctx)); LRP_TRY(init_small<6>(ctx)); LRP_TRY(init_small<7>(ctx)); LRP_TRY(init_small<8>(ctx));
+    LRP_TRY(init_small<9>(ctx)); LRP_TRY(init_small<10>(ctx)); LRP_TRY(init_small<11>(ctx)); LRP_TRY(init_small<12>(ctx));
+    LRP_TRY(init_small<13>(ctx));
+    return dst1_large_init(ctx);
+}
 
 size_t lrp_dst1_ws_impl(int64_t n, int32_t batch) {
     int64_t N = n + 1;

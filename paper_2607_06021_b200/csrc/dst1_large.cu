@@ -15,7 +15,6 @@
 #include "common.cuh"
 #include "fft_smem.cuh"
 #include <math.h>
-#include <stdlib.h>
 
 namespace {
 
@@ -354,7 +353,6 @@ dst1_scanapply_kernel(int log2N, int log2L1, const double2* __restrict__ W, doub
 template <int Q1, int TL>
 int launch_pa(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in, double2* W) {
     using C = PACfg<Q1, TL>;
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pa_kernel<Q1, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     const int L2 = 1 << (log2N - 1 - Q1);
     LRP_PROF(ctx, K_DST_P1, 16.0 * ((int64_t)1 << log2N) * cols, 0);
     dst1_pa_kernel<Q1, TL><<<dim3(L2 / C::T2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, in, ld_in, W);
@@ -364,7 +362,6 @@ int launch_pa(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in
 template <int Q2, int TL>
 int launch_pb(lrp_ctx* ctx, int log2N, int cols, double2* W, double scale, double* xlast, int xstride, double* part) {
     using C = PBCfg<Q2, TL>;
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pb_kernel<Q2, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
     const int L1 = 1 << (log2N - 1 - Q2);
     LRP_PROF(ctx, K_DST_P2, 16.0 * ((int64_t)1 << log2N) * cols, 0);
     dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, scale, xlast, xstride, part);
@@ -402,12 +399,9 @@ Plan plan(int log2N) {
     Plan p;
     p.q1 = q <= 14 ? 7 : 8;
     if (q - p.q1 > 12) p.q1 = q - 12;
-    if (const char* e = getenv("LRP_DST_Q1")) { int v = atoi(e); if (v >= 7 && v <= 12 && q - v >= 7 && q - v <= 12) p.q1 = v; }
     p.q2 = q - p.q1;
     p.tla = p.q1 >= 9 ? 13 : 12;
-    if (const char* e = getenv("LRP_DST_TLA")) { int v = atoi(e); if ((v == 12 && p.q1 <= 11) || v == 13) p.tla = v; }
     p.tlb = p.q2 >= 12 ? 13 : 12;
-    if (const char* e = getenv("LRP_DST_TLB")) { int v = atoi(e); if ((v == 12 && p.q2 <= 11) || v == 13) p.tlb = v; }
     p.nB = (1 << p.q1) / tile_rows(p.tlb, p.q2);
     p.nch = (int)(((int64_t)1 << q) / SC_CHUNK);
     return p;
@@ -416,15 +410,30 @@ Plan plan(int log2N) {
 // columns per group (workspace bound: W of one group)
 int group_cols(int64_t N, int batch) {
     int64_t per_col = N * 8;
-    static int64_t budget_mb = 0;
-    if (budget_mb == 0) { const char* e = getenv("LRP_DST_GROUP_MB"); budget_mb = e ? atoll(e) : 4096; if (budget_mb < 1) budget_mb = 4096; }
+    const int64_t budget_mb = 4096;
     int g = (int)((budget_mb << 20) / per_col);
     if (g < 1) g = 1;
     if (g > batch) g = batch;
     return g;
 }
 
+template <int Q, int TL>
+int init_pair(lrp_ctx* ctx) {
+    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pa_kernel<Q, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PACfg<Q, TL>::SMEM));
+    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pb_kernel<Q, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PBCfg<Q, TL>::SMEM));
+    return LRP_OK;
+}
+
 }  // namespace
+
+int dst1_large_init(lrp_ctx* ctx) {
+    LRP_TRY((init_pair<7, 12>(ctx))); LRP_TRY((init_pair<8, 12>(ctx))); LRP_TRY((init_pair<9, 12>(ctx)));
+    LRP_TRY((init_pair<10, 12>(ctx))); LRP_TRY((init_pair<11, 12>(ctx)));
+    LRP_TRY((init_pair<7, 13>(ctx))); LRP_TRY((init_pair<8, 13>(ctx))); LRP_TRY((init_pair<9, 13>(ctx)));
+    LRP_TRY((init_pair<10, 13>(ctx))); LRP_TRY((init_pair<11, 13>(ctx))); LRP_TRY((init_pair<12, 13>(ctx)));
+    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_scanapply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * SC_ARR * (int)sizeof(double)));
+    return LRP_OK;
+}
 
 size_t dst1_large_ws(int64_t N, int32_t batch) {
     const int g = group_cols(N, batch);
@@ -446,7 +455,6 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
     double* part = ar.take<double>((size_t)g * p.nB * p.nch);
     if (!ar.ok()) return LRP_ERR_WORKSPACE;
     constexpr int SC_SMEM = 2 * SC_ARR * (int)sizeof(double);
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_scanapply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SC_SMEM));
     for (int c0 = 0; c0 < batch; c0 += g) {
         const int cols = (batch - c0) < g ? (batch - c0) : g;
         double* o = d_out + (int64_t)c0 * ld_out;

@@ -4,6 +4,7 @@
 // In place: A (n x K, ld lda) <- Q;  R (K x K, ld ldr, device) <- upper-triangular factor.  Requires n >= K.
 // ws: tall_qr_ws_doubles(ctx, n, K) doubles of scratch.
 size_t tall_qr_ws_doubles(const lrp_ctx* ctx, int64_t n, int K);
+int tall_qr_init(lrp_ctx* ctx);                  // one-time kernel attributes (lrp_create)
 int tall_qr(lrp_ctx* ctx, int64_t n, int K, double* A, int64_t lda, double* R, int64_t ldr, double* ws);
 // Two independent factorizations advanced panel by panel on ctx->stream and ctx->aux (joined on return into ctx->stream).
 int tall_qr_pair(lrp_ctx* ctx, int64_t n, int K1, double* A1, int64_t lda1, double* R1, int64_t ldr1, double* ws1,
@@ -18,6 +19,5 @@ int tall_qr_pair_from(lrp_ctx* ctx, int64_t n, int K1, int k01, double* A1, int6
 struct QrJob {
     int k0;                                       // leading columns already factored (0: none)
     int64_t n; int K; double* A; int64_t lda; double* R; int64_t ldr; double* ws; cudaStream_t stream;
-    double* hR;                                   // pinned host scratch, 256 doubles
-    double *stack, *partial, *Stmp, *d_runmax;    // carved from ws by tall_qr_begin
+    double *stack, *partial, *Stmp, *d_small;     // carved from ws by tall_qr_begin
 };

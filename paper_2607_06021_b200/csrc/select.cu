@@ -107,8 +107,7 @@ topk_merge_kernel(int G, int num, const double* __restrict__ cand_s, const int32
 
 void sel_geometry(const lrp_ctx* ctx, int64_t n, int* G, int64_t* chunk) {
     int64_t g = (n + SEL_MAX_CHUNK - 1) / SEL_MAX_CHUNK;
-    (void)ctx;
-    int64_t want = 148 * 4;
+    int64_t want = (int64_t)lrp_sm_count(ctx) * 4;      // without a ctx (workspace sizing): the upper bound of the SM count
     int64_t by_rows = (n + 1023) / 1024;
     int64_t g2 = want < by_rows ? want : by_rows;
     if (g2 > g) g = g2;

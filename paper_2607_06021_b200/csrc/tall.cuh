@@ -18,6 +18,7 @@ struct TallGemmArgs {
     const double* Cin; int64_t ldc;
     double* Out; int64_t ldo;
     double* rownorm2;
+    const int* cond;            // optional device flag: the launch does nothing when *cond == 0 (decided on the device)
 };
 
 int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p);
@@ -26,7 +27,8 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p);
 // reduction over row slabs happens inside the kernel.
 size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m);
 int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
-                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd = nullptr, int64_t ldadd = 0);
+                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd = nullptr, int64_t ldadd = 0,
+                const int* cond = nullptr);
 int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, const unsigned char* colmask, double* out);
 int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const int32_t* idx, int nidx, double* Out, int ldo);
 int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb);

@@ -8,7 +8,6 @@
 #include "common.cuh"
 #include "tall.cuh"
 #include <math.h>
-#include <stdlib.h>
 
 namespace {
 
@@ -41,6 +40,7 @@ __global__ void __launch_bounds__(MG_THREADS, NJ == 2 ? 5 : (NJ <= 4 ? 4 : 3))
 tall_gemm_mma_kernel(TallGemmArgs p) {
     constexpr int MG_CT = 8 * NJ;
     extern __shared__ __align__(16) double smem[];
+    if (p.cond && *p.cond == 0) return;               // conditional launch (device-side decision, qr.cu): grid-uniform
     const int kp = mg_kp(p.k), k4 = (p.k + 3) & ~3;
     double* Bs = smem;                                // [MG_CT][kp]: Bs[c*kp + t] = B(t, c0 + c)
     double* dcol = smem + (size_t)MG_CT * kp;         // [MG_CT]
@@ -147,7 +147,7 @@ tall_gemm_mma_kernel(TallGemmArgs p) {
 constexpr int MT_THREADS = 256;
 constexpr int GT_GROUP = 16;                          // row slabs per first-level reduction group
 constexpr int GT_MAXGRP = 64;                         // counters [0, 64): groups, [64]: the final level
-struct GemmTOut { double* S; int64_t lds; int accumulate; double* Sadd; int64_t ldadd; double* gpartial; unsigned* counters; };
+struct GemmTOut { double* S; int64_t lds; int accumulate; double* Sadd; int64_t ldadd; double* gpartial; unsigned* counters; const int* cond; };
 
 // ---- in-kernel reduction over the row slabs, two levels, fixed summation order (deterministic): the last CTA to
 // finish in a group of GT_GROUP slabs sums the group's partials, the last group to finish sums the groups and writes
@@ -208,6 +208,7 @@ tall_gemm_t_mma_kernel(const double* __restrict__ A, int64_t lda, int k, const d
                        int64_t n, int64_t rows_per_cta, double* partial, int na, int nb, int ntc, GemmTOut o) {
     __shared__ double red[MT_THREADS / 32][8][32];
     __shared__ int s_role;
+    if (o.cond && *o.cond == 0) return;                     // conditional launch: grid-uniform, counters untouched
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, tg = lane & 3;
     const int nsub = (MT_THREADS / 32) / ntc;               // warps per tile
     const int tl = warp % ntc, sub = warp / ntc;
@@ -414,7 +415,7 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
         LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
-    const int64_t resident = 148 * (nj == 2 ? 5 : (nj <= 4 ? 4 : 3));   // persistent over row slabs (B staged once per column tile per CTA):
+    const int64_t resident = (int64_t)lrp_sm_count(ctx) * (nj == 2 ? 5 : (nj <= 4 ? 4 : 3));   // persistent over row slabs (B staged once per column tile per CTA):
     if (grid > resident) grid = resident;            // exactly one resident wave, so that the slabs are balanced
     LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
              8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
@@ -427,24 +428,24 @@ static int tall_gemm_t_ntc(int k, int m) {       // tiles per CTA: 1, 2, 4 or 8 
     int nt = ((k + 15) / 16) * ((m + 15) / 16);
     return nt >= 8 ? 8 : (nt >= 4 ? 4 : (nt >= 2 ? 2 : 1));
 }
-static int tall_gemm_t_nblk(int64_t n, int k, int m) {
+static int tall_gemm_t_nblk(const lrp_ctx* ctx, int64_t n, int k, int m) {
     (void)k; (void)m;
-    int64_t want = 148 * 3;                            // B200: 148 SMs x 3 resident CTAs (one wave); fixed: workspace sizes need no device query
+    int64_t want = (int64_t)lrp_sm_count(ctx) * 3;     // SMs x 3 resident CTAs (one wave); without a ctx (workspace sizing on the host) the upper bound LRP_SM_UPPER
     int64_t by_rows = (n + 511) / 512;
     int64_t nb = want < by_rows ? want : by_rows;
     return (int)(nb < 1 ? 1 : nb);
 }
 
 size_t tall_gemm_t_ws_doubles(const lrp_ctx* ctx, int64_t n, int k, int m) {
-    (void)ctx;
-    return ((size_t)tall_gemm_t_nblk(n, k, m) + GT_MAXGRP) * k * m;      // slab partials + group partials
+    (void)ctx;                                          // sized for the upper bound of the SM count: no device query
+    return ((size_t)tall_gemm_t_nblk(nullptr, n, k, m) + GT_MAXGRP) * k * m;      // slab partials + group partials
 }
 
 int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb, int m,
-                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd, int64_t ldadd) {
+                double* S, int64_t lds, int accumulate, double* partial_ws, double* Sadd, int64_t ldadd, const int* cond) {
     if (k <= 0 || m <= 0) return LRP_OK;
-    int nblk = tall_gemm_t_nblk(n, k, m);
-    const int nblk_max = nblk;
+    int nblk = tall_gemm_t_nblk(ctx, n, k, m);
+    const int nblk_max = tall_gemm_t_nblk(nullptr, n, k, m);
     const int ntc = tall_gemm_t_ntc(k, m);
     int64_t rows_per = (n + nblk - 1) / nblk;
     rows_per = (rows_per + 15) / 16 * 16;
@@ -453,7 +454,7 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
     dim3 grid(nblk, (na * nb + ntc - 1) / ntc);
     if ((nblk + GT_GROUP - 1) / GT_GROUP > GT_MAXGRP) return LRP_ERR_BADARG;
     GemmTOut o{};
-    o.S = S; o.lds = lds; o.accumulate = accumulate; o.Sadd = Sadd; o.ldadd = ldadd;
+    o.S = S; o.lds = lds; o.accumulate = accumulate; o.Sadd = Sadd; o.ldadd = ldadd; o.cond = cond;
     o.gpartial = partial_ws + (size_t)nblk_max * k * m;
     // one counter set per library stream: launches on a stream are ordered, the counters are back at zero when a launch ends
     const int slot = ctx->stream == ctx->aux ? 1 : (ctx->stream == ctx->aux2 ? 2 : 0);
@@ -472,13 +473,13 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
 int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb,
                     const double* Cin, int64_t ldc, int m, double* G, int64_t ldg, double* partial_ws) {
     if (k <= 0 || m <= 0) return 1;
-    if (getenv("LRP_NO_FUSED_RHO")) return 1;                      // test hook: force the two-sweep path
+    if (ctx->flags & LRP_FLAG_NO_FUSED_RHO) return 1;              // lrp_solve_opts.flags: force the two-sweep path
     const int NJ = (m + 7) / 8;
     const bool vec = (lda % 2 == 0) && (ldc % 2 == 0) && ((((uintptr_t)A) | ((uintptr_t)Cin)) & 15u) == 0;
     if (NJ > 8 || !vec) return 1;
-    int nblk = tall_gemm_t_nblk(n, m, m);                          // same partial geometry as tall_gemm_t
-    const int nblk_max = nblk;
-    if (nblk > 148 * (NJ <= 5 ? 3 : 2)) nblk = 148 * (NJ <= 5 ? 3 : 2);   // one resident wave of the persistent CTAs
+    int nblk = tall_gemm_t_nblk(ctx, n, m, m);                     // same partial geometry as tall_gemm_t
+    const int nblk_max = tall_gemm_t_nblk(nullptr, n, m, m);
+    if (nblk > ctx->sm_count * (NJ <= 5 ? 3 : 2)) nblk = ctx->sm_count * (NJ <= 5 ? 3 : 2);   // one resident wave of the persistent CTAs
     const int64_t nslab = (n + RG_THREADS - 1) / RG_THREADS;
     if (nblk > nslab) nblk = (int)nslab;
     const size_t es = (size_t)4 * 32 * rg_lde(8 * NJ), rd = (size_t)4 * NJ * (NJ + 1) * 32;

@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "liblrp.so")
 
 LRP_OK, LRP_ERR_BADARG, LRP_ERR_UNSUPPORTED_N, LRP_ERR_WORKSPACE, LRP_ERR_CUDA, LRP_WARN_NOCONV = 0, -1, -2, -3, -4, 1
 MAX_SWEEPS_INFO = 32
+LRP_FLAG_NO_QR_REUSE, LRP_FLAG_NO_NESTED_RHO, LRP_FLAG_NO_FUSED_RHO = 1, 2, 4
 
 EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "lrp_launch_count",
            "lrp_workspace_bytes", "lrp_dst1_workspace_bytes", "lrp_leverage_workspace_bytes",
@@ -35,7 +36,7 @@ class SolveOpts(C.Structure):
                 ("d_U0", C.c_void_p), ("d_V0", C.c_void_p), ("ld0", C.c_int64), ("r0", C.c_int32),
                 ("replay_sweeps", C.c_int32), ("h_replay_nI", C.c_void_p), ("h_replay_nJ", C.c_void_p),
                 ("h_replay_I", C.c_void_p), ("h_replay_J", C.c_void_p), ("h_replay_keepI", C.c_void_p),
-                ("h_replay_keepJ", C.c_void_p), ("replay_final_rank", C.c_int32)]
+                ("h_replay_keepJ", C.c_void_p), ("replay_final_rank", C.c_int32), ("flags", C.c_int32)]
 
 
 class SolveInfo(C.Structure):
@@ -255,14 +256,14 @@ class Context:
         return dict(U=U[:r], S=S[:r], V=V[:r], S_full=S, rC=rC, rR=rR, rank=r, smin_full=smin.value)
 
     def cross_deim_solve(self, UF, SF, VF, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False):
+                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False, flags=0):
         """Low-rank Poisson solve.  UF, VF: tall tensors (rF, n) in physical space, SF: (rF,) CUDA tensor.
         replay: list of dicts {I, J, keepI, keepJ} (numpy) + optional 'final_rank' on the last one."""
         torch = _torch()
         rF, n, ldu = _check_tall(UF, "UF")
         _, _, ldv = _check_tall(VF, "VF")
         dev = UF.device
-        Kc = max(2 * (max_rank + oversample), rF + oversample + 1)
+        Kc = 2 * (max_rank + oversample)
         self.ensure_workspace(self.lib.lrp_workspace_bytes(n, rF, max_rank, oversample))
         # outputs: only the first info.rank columns are defined (and returned); no fill kernels on the solve's path
         UW = torch.empty((max_rank, n), dtype=torch.float64, device=dev)
@@ -270,6 +271,7 @@ class Context:
         SW = torch.empty(max_rank, dtype=torch.float64, device=dev)
         o = SolveOpts()
         o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
+        o.flags = int(flags)
         keep = []
         if safeguard is not None:
             sg = np.ascontiguousarray(safeguard, dtype=np.int32); keep.append(sg)

@@ -40,9 +40,9 @@ def test_struct_sizes_match_header(lib):
 #include <stdio.h>
 #include <stddef.h>
 #include "lrp.h"
-int main(void){ printf("%zu %zu %zu %zu %zu %zu\n", sizeof(lrp_solve_opts), sizeof(lrp_solve_info),
+int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(lrp_solve_opts), sizeof(lrp_solve_info),
   offsetof(lrp_solve_opts, replay_final_rank), offsetof(lrp_solve_info, ms_dst_fwd),
-  offsetof(lrp_solve_info, launches), offsetof(lrp_solve_opts, h_replay_keepI)); return 0; }
+  offsetof(lrp_solve_info, launches), offsetof(lrp_solve_opts, h_replay_keepI), offsetof(lrp_solve_opts, flags)); return 0; }
 '''
     with tempfile.TemporaryDirectory() as d:
         p = os.path.join(d, "probe.c")
@@ -55,6 +55,7 @@ int main(void){ printf("%zu %zu %zu %zu %zu %zu\n", sizeof(lrp_solve_opts), size
     assert vals[3] == lrp.SolveInfo.ms_dst_fwd.offset
     assert vals[4] == lrp.SolveInfo.launches.offset
     assert vals[5] == lrp.SolveOpts.h_replay_keepI.offset
+    assert vals[6] == lrp.SolveOpts.flags.offset
 
 
 def test_host_only_entry_points(lib):

@@ -99,15 +99,14 @@ def test_set_cap_truncation_and_gpu_trace_replay(ctx):
     assert torch.equal(again["Shat"], res["Shat"])
 
 
-def test_fused_and_two_sweep_stop_test_agree(ctx, monkeypatch):
+def test_fused_and_two_sweep_stop_test_agree(ctx):
     """rho (Alg. 4 line 24) through the fused residual-Gram kernel (E = U_{k-1} - U_k A never written)
     and through the update sweep + Gram sweep it replaces (shapes outside the fused kernel's range take that path):
     the same sweeps, ranks and index decisions, rho equal to rounding of a sum of squares."""
     w = W.make("C2", 3)
+    from paper_2607_06021_b200 import lrp
     a = _solve(ctx, w)
-    monkeypatch.setenv("LRP_NO_FUSED_RHO", "1")
-    b = _solve(ctx, w)
-    monkeypatch.delenv("LRP_NO_FUSED_RHO")
+    b = _solve(ctx, w, flags=lrp.LRP_FLAG_NO_FUSED_RHO)
     assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
     ia, ib = a["info"], b["info"]
     for k in range(a["sweeps"]):
@@ -117,17 +116,15 @@ def test_fused_and_two_sweep_stop_test_agree(ctx, monkeypatch):
 
 
 @pytest.mark.parametrize("cfg,seed,nred", [("C2", 0, None), ("C2", 3, None), ("C3", 0, 16383), ("C4", 0, 32767)])
-def test_qr_prefix_reuse_matches_full_factorization(ctx, monkeypatch, cfg, seed, nred):
+def test_qr_prefix_reuse_matches_full_factorization(ctx, cfg, seed, nred):
     """Fibers of surviving indices do not change between sweeps (G-hat is fixed, eq. (4)) and the QR of a
     column prefix is the prefix of the QR, so the driver keeps the Q columns of the common prefix of consecutive index
-    lists and factors only the new fibers.  Against factoring every block from scratch (LRP_NO_QR_REUSE): the same
+    lists and factors only the new fibers.  Against factoring every block from scratch (LRP_FLAG_NO_QR_REUSE): the same
     index decisions in the first sweeps, the same rank, and reconstructed entries equal to the parity tolerance."""
     from paper_2607_06021_b200 import lrp
     w = W.make(cfg, seed) if nred is None else W.make(cfg, seed, nred)
     a = _solve(ctx, w)
-    monkeypatch.setenv("LRP_NO_QR_REUSE", "1")
-    b = _solve(ctx, w)
-    monkeypatch.delenv("LRP_NO_QR_REUSE")
+    b = _solve(ctx, w, flags=lrp.LRP_FLAG_NO_QR_REUSE)
     assert abs(a["sweeps"] - b["sweeps"]) <= 1 and a["rank"] == b["rank"]
     for ta, tb in list(zip(a["trace"], b["trace"]))[:2]:
         assert list(ta["I"]) == list(tb["I"]) and list(ta["J"]) == list(tb["J"])
@@ -140,22 +137,21 @@ def test_qr_prefix_reuse_matches_full_factorization(ctx, monkeypatch, cfg, seed,
 
 
 @pytest.mark.parametrize("cfg,seed,nred", [("C2", 3, None), ("C4", 0, 32767)])
-def test_nested_stop_test_matches_tall_contractions(ctx, monkeypatch, cfg, seed, nred):
+def test_nested_stop_test_matches_tall_contractions(ctx, cfg, seed, nred):
     """rho (Alg. 4 line 24) when last sweep's index lists are prefixes of this sweep's: U_{k-1} lies in
     span(Q_k), so rho follows from the small core factors alone; with a few dropped trailing indices (the pruned
     safeguard of sweep 0) U_{k-1} = Q_k Y + P Uc_rest with the dropped Q columns set aside (three narrow passes).
     Against the general path (contractions over the tall
-    iterates, LRP_NO_NESTED_RHO): same decisions, rho equal up to the orthonormality of the GPU's Q.  Both forms assume
-    Q^T Q = I; a panel is re-orthogonalised against the earlier ones only when a pivot falls below 1e-5 of its column
-    (DESIGN.md "Thin QR"), which leaves Q^T Q - I at eps/1e-5 ~ 2e-11, and rho at that level of ||S||."""
+    iterates, LRP_FLAG_NO_NESTED_RHO): same decisions, rho equal up to the orthonormality of the GPU's Q.  Both forms assume
+    Q^T Q = I, which the thin QR delivers to ~1e-15 (every panel is re-orthogonalised after its factorization, DESIGN.md
+    "Thin QR"), so the two rho agree to rounding of ||S||."""
     w = W.make(cfg, seed) if nred is None else W.make(cfg, seed, nred)
+    from paper_2607_06021_b200 import lrp
     a = _solve(ctx, w)
-    monkeypatch.setenv("LRP_NO_NESTED_RHO", "1")
-    b = _solve(ctx, w)
-    monkeypatch.delenv("LRP_NO_NESTED_RHO")
+    b = _solve(ctx, w, flags=lrp.LRP_FLAG_NO_NESTED_RHO)
     assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
     ia, ib = a["info"], b["info"]
     for k in range(a["sweeps"]):
         ra, rb = ia.rho_per_sweep[k], ib.rho_per_sweep[k]
-        assert abs(ra - rb) <= 1e-6 * max(abs(ra), abs(rb)) + 5e-11 * ia.snorm
+        assert abs(ra - rb) <= 1e-6 * max(abs(ra), abs(rb)) + 2e-13 * ia.snorm
         assert ia.rank_per_sweep[k] == ib.rank_per_sweep[k] and ia.nI[k] == ib.nI[k] and ia.nJ[k] == ib.nJ[k]

@@ -193,4 +193,4 @@ def test_scross_exact_low_rank(ctx, n, rank, k, l):
     assert np.abs(rR[:rank] - ref.rR[:rank]).max() < 1e-10 * ref.rR.max()
     assert (rC[rank:] < 1e-12 * rC.max()).all() and (rR[rank:] < 1e-12 * rR.max()).all()
     # orthonormal factors
-    assert np.abs(U.T @ U - np.eye(U.shape[1])).max() < 1e-12 and np.abs(V.T @ V - np.eye(V.shape[1])).max() < 1e-12
+    assert np.abs(U.T @ U - np.eye(U.shape[1])).max() <= 1e-13 and np.abs(V.T @ V - np.eye(V.shape[1])).max() <= 1e-13
