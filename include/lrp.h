@@ -25,7 +25,7 @@
  *     their control flow needs device results (documented per function) and are complete on return
  *     only where stated.
  *   - return value: 0 = LRP_OK, negative = error, positive = warning (outputs valid).
- *     No exceptions, no globals, no CPU fallback: without a CUDA device every compute call fails.
+ *     No exceptions, no globals, no environment variables, no CPU fallback: without a CUDA device every compute call fails.
  *   - n + 1 must be a power of two, 2 <= n + 1 <= 2^25 (general n: DESIGN.md "next").
  */
 #ifndef LRP_H_
@@ -74,7 +74,8 @@ int lrp_profile_count(void);
 int lrp_profile_get(lrp_ctx* ctx, int i, const char** name, int64_t* count, double* ms, double* bytes, double* flops);
 
 /* Workspace sizes in bytes (host-side arithmetic only; safe to call without a GPU).
- *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample).
+ *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample)
+ *                                (reading Q10); 0 when the arguments are invalid, e.g. rF + oversample + 1 > K_cap.
  *   lrp_dst1_workspace_bytes   : lrp_dst1_batched (0 for n <= 16383, the single-pass shared-memory regime).
  *   lrp_leverage_workspace_bytes, lrp_scross_workspace_bytes : the standalone calls. */
 size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample);
@@ -181,7 +182,10 @@ typedef struct lrp_solve_info {
  * the previous block keep their Q and R factors, and when the previous index lists are prefixes of the current ones
  * rho (Alg. 4 line 24) is evaluated from the small core factors (readings R4, R5;
  * opts->flags LRP_FLAG_NO_QR_REUSE / LRP_FLAG_NO_NESTED_RHO switch either off for comparison).
- * Synchronous: complete on return.  Returns LRP_WARN_NOCONV when the stop test never passed. */
+ * Index lists are cut to K_cap = 2 (max_rank + oversample) entries (reading Q10); rF + oversample + 1 > K_cap (the first
+ * selection would not fit) is LRP_ERR_BADARG.
+ * Synchronous: complete on return.  Returns LRP_WARN_NOCONV (info->converged = 0, outputs valid) when the stop test never
+ * passed within max_sweeps or when r* > max_rank (Alg. 4 line 31: the truncated result misses the tolerance). */
 int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
                          const double* d_UF, int64_t ldu, const double* d_SF, const double* d_VF, int64_t ldv,
                          const lrp_solve_opts* opts,

@@ -425,6 +425,7 @@ class SolveResult:
     sweeps: int
     converged: bool
     trace: list
+    rank_capped: bool = False   # r* > r_max (Alg. 4 line 31): the truncated result does not meet the tolerance (reading Q20)
 
 
 def _union(prev: np.ndarray, star: np.ndarray) -> tuple[np.ndarray, int]:
@@ -531,17 +532,19 @@ def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, 
         if replay is None and max(rho, ind) < thresh:        # Alg. 4 line 26, Q15
             converged = True
             break
+    rank_capped = False
     if replay is not None and replay[-1].get("final_rank"):
         r = int(replay[-1]["final_rank"])
         converged = True
     else:
         r = final_rank(res.S, tol, max_rank, tol_mode)       # O11
+        rank_capped = final_rank(res.S, tol, res.S.size + 1, tol_mode) > max_rank      # reading Q20: r* > r_max
     r = min(r, res.rank)
     UW = dst1(res.U[:, :r], scale)                           # O12
     VW = dst1(res.V[:, :r], scale)
     return SolveResult(UW=UW, SW=res.S[:r].copy(), VW=VW, Uhat=res.U, Shat=res.S, Vhat=res.V,
                        UhF=UhF, VhF=VhF, d=d, rank=r, sweeps=len(trace), converged=converged,
-                       trace=trace)
+                       trace=trace, rank_capped=rank_capped)
 
 
 def trace_to_replay(trace, final_rank_value: int | None = None) -> list:

@@ -131,7 +131,7 @@ def test_qr_prefix_reuse_matches_full_factorization(ctx, cfg, seed, nred):
     rows, cols = W.sample_pairs(w.n, 4096, seed=5)
     ea = _entries(lrp.tall_to_numpy(a["UW"]), a["SW"].cpu().numpy(), lrp.tall_to_numpy(a["VW"]), rows, cols)
     eb = _entries(lrp.tall_to_numpy(b["UW"]), b["SW"].cpu().numpy(), lrp.tall_to_numpy(b["VW"]), rows, cols)
-    tol = 1e-10 if (a["converged"] and b["converged"]) else 2 * max(a["info"].rho, b["info"].rho) / a["info"].snorm + 1e-10
+    tol = 1e-10 if (a["converged"] and b["converged"]) else max(1e-10, 0.1 * max(a["info"].rho, b["info"].rho) / a["info"].snorm)
     assert np.abs(ea - eb).max() <= tol * np.abs(eb).max()
     assert a["info"].launches < b["info"].launches
 

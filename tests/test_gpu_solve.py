@@ -33,24 +33,26 @@ def _entries(U, S, V, rows, cols):
 
 
 def _parity_tol(ref):
-    """1e-10 when the stop test passed.  A run that the sweep cap ends first (C3 as configured: 5 sweeps) still has
-    a residual of size rho, part of which is fitted by the QR's rounding-level directions: two fp64 implementations
-    are then only defined up to O(rho / ||S||) -- DESIGN.md "Parity tolerance", shown on the oracle itself (Householder
-    vs LAPACK QR under replay) in tests/test_oracle_solve.py::test_unconverged_run_sensitivity."""
+    """Tolerance on PHYSICAL-space entries: 1e-10 when the stop test passed.  A run that the sweep cap ends first (C3 as
+    configured: 5 sweeps) still has a residual of size rho; the final truncation then cuts singular values that are not
+    yet resolved, and two fp64 implementations differ by a fraction of rho / ||S|| on W -- DESIGN.md reading R1, shown on
+    the oracle itself (Householder vs LAPACK QR under replay) in
+    tests/test_oracle_solve.py::test_unconverged_run_sensitivity.  Bound: max(1e-10, 0.1 rho/||S||) (C3: 2.7e-10,
+    measured 1.4e-10).  Singular values and selected fibers are held to 1e-10 in every case."""
     t = ref.trace[-1]
-    return TOL if ref.converged else max(TOL, 2.0 * max(t.rho, t.ind) / t.snorm)
+    return TOL if ref.converged else max(TOL, 0.1 * t.rho / t.snorm)
 
 
 def _continuous_parity(res, ref, w, replay_sets, tol=None):
     from paper_2607_06021_b200 import lrp
     n = w.n
-    TOL = tol if tol is not None else _parity_tol(ref)
+    tolW = tol if tol is not None else _parity_tol(ref)
     UW, VW, SW = lrp.tall_to_numpy(res["UW"]), lrp.tall_to_numpy(res["VW"]), res["SW"].cpu().numpy()
     assert res["rank"] == ref.rank
     rows, cols = W.sample_pairs(n, 4096, seed=1)
     a = _entries(UW, SW, VW, rows, cols); b = _entries(ref.UW, ref.SW, ref.VW, rows, cols)
     wmax = np.abs(b).max()                                   # max |W| over the 4096 samples of the smooth solution
-    assert np.abs(a - b).max() <= TOL * wmax, (np.abs(a - b).max() / wmax, TOL)
+    assert np.abs(a - b).max() <= tolW * wmax, (np.abs(a - b).max() / wmax, tolW)
     # all selected fibers of the spectral iterate
     Uh, Vh, Sh = lrp.tall_to_numpy(res["Uhat"]), lrp.tall_to_numpy(res["Vhat"]), res["Shat"].cpu().numpy()
     assert Uh.shape[1] == ref.Uhat.shape[1]
@@ -97,6 +99,9 @@ def test_solve_free_run_and_replay(ctx, name, seed, n, sweeps):
     if clear and same:
         assert res["converged"] == ref.converged
         _continuous_parity(res, ref, w, (ref.trace[-1].I, ref.trace[-1].J))
+    else:       # decisions inside the tolerance bands: the free runs took different (equally valid) index sets
+        print(f"{name} seed {seed}: free-run continuous comparison not applicable (clear={clear}, same sweeps={same}); "
+              f"replay parity below covers it")
     # ---- replay oracle -> GPU
     rep = O.trace_to_replay(ref.trace, ref.rank)
     res2 = _gpu_solve(ctx, w, replay=rep)
@@ -138,3 +143,31 @@ def test_solve_argument_errors(ctx):
     # max_sweeps = 1 cannot pass the stop test -> warning code, outputs still valid
     r = ctx.cross_deim_solve(UF, SF, VF, tol=1e-12, max_rank=16, max_sweeps=1, safeguard=w.safeguard)
     assert r["code"] == lrp.LRP_WARN_NOCONV and r["rank"] >= 1
+
+
+def test_rank_cap_returns_noconv_warning(ctx):
+    """r* > r_max (Alg. 4 line 31): the result is truncated to r_max and the tolerance is not met --
+    reading Q20: LRP_WARN_NOCONV and converged = 0, as the oracle's rank_capped flag."""
+    from paper_2607_06021_b200 import lrp
+    w = W.make("C2", 0)
+    w.max_rank = 6
+    ref = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, **w.opts())
+    assert ref.rank == 6 and ref.rank_capped
+    res = _gpu_solve(ctx, w)
+    assert res["rank"] == 6 and res["code"] == lrp.LRP_WARN_NOCONV and not res["converged"]
+    assert np.abs(res["SW"].cpu().numpy() - ref.SW).max() <= 1e-6 * ref.SW[0]
+
+
+def test_first_selection_must_fit_the_set_cap(ctx):
+    """K_cap = 2 (r_max + p_os) (reading Q10) as in the oracle; a right-hand side whose first selection
+    (rF + p_os indices + safeguard) does not fit is rejected instead of silently enlarging the cap."""
+    import torch
+    from paper_2607_06021_b200 import lrp
+    w = W.make("C4", 0, 1023)                  # rF = 32
+    UF = lrp.tall_from_numpy(w.UF); VF = lrp.tall_from_numpy(w.VF); SF = torch.from_numpy(w.SF).cuda()
+    assert ctx.lib.lrp_workspace_bytes(w.n, w.rF, 8, 8) == 0           # 2 (8 + 8) = 32 < 32 + 8 + 1
+    with pytest.raises(lrp.LrpError) as e:
+        ctx.cross_deim_solve(UF, SF, VF, tol=1e-8, max_rank=8, oversample=8)
+    assert e.value.code == lrp.LRP_ERR_BADARG
+    ok = ctx.cross_deim_solve(UF, SF, VF, tol=1e-8, max_rank=13, oversample=8, safeguard=w.safeguard)   # 42 >= 41
+    assert ok["rank"] <= 13
