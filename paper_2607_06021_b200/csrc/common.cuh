@@ -11,12 +11,12 @@
 // kernel classes for the per-kernel profile (lrp_profile_*): launch counts, CUDA-event time on the ctx's stream,
 // and the ALGORITHMIC bytes / flops of the launches (what the step must move / compute).
 enum LrpKernelId {
-    K_DST_SMALL, K_DST_NAIVE, K_DST_P1, K_DST_P2, K_DST_UNTANGLE, K_DST_CHUNKSUM, K_DST_SCANSUMS, K_DST_FINISH,
+    K_DST_SMALL, K_DST_NAIVE, K_DST_FUSED,
     K_GEMM_SAMPLE, K_GEMM_PLAIN, K_GEMM_SUBTRACT, K_GEMM_T, K_REDUCE, K_ROWNORM, K_GATHER, K_COPY, K_ENTRIES,
     K_PANEL_QR, K_PANEL_APPLY, K_ADD_BLOCK, K_CORE, K_ETA, K_RHO, K_COLMASK, K_TOPK_CHUNK, K_TOPK_MERGE, K_RESID_GRAM, K_NUM
 };
 static const char* const LRP_KERNEL_NAMES[K_NUM] = {
-    "dst1_small", "dst1_naive", "dst1_p1", "dst1_p2", "dst1_untangle", "dst1_chunksum", "dst1_scansums", "dst1_finish",
+    "dst1_small", "dst1_naive", "dst1_fused",
     "tall_gemm_sample", "tall_gemm_plain", "tall_gemm_subtract", "tall_gemm_t", "reduce_partials", "rownorm2", "gather_rows",
     "copy_tall", "lowrank_entries", "panel_qr", "panel_apply", "add_block", "scross_core", "eta", "rho", "colmask",
     "topk_chunk", "topk_merge", "tall_resid_gram"

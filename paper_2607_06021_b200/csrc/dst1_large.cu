@@ -1,24 +1,35 @@
 // dst1_large.cu -- batched DST-I for N = n + 1 = 2^p > 16384: the column no longer fits one CTA's shared memory.
 //
-// Same folding as dst1.cu (t -> z, complex FFT of length L = N/2, untangle, prefix sum), with the FFT split
-// four-step style, L = L1 * L2, j = j1*L2 + j2, k = k1 + L1*k2:
-//   sweep A: fold x on the fly (every x element enters exactly two t's: the CTA owns a j2 tile AND its mirror tile,
-//            so each element is fetched from HBM once), length-L1 FFTs over the strided index j1, four-step twiddle,
-//            W[k1*L2 + j2] (complex, 8N bytes per column);
-//   sweep B: the CTA owns T rows k1 and their mirror rows L1 - k1: length-L2 FFTs, real-FFT untangle of the pairs
-//            (k, L-k) in shared memory; (R_k, X_{2k}) with R_k = X_{2k+1} - X_{2k-1} go back IN PLACE into the rows of W
-//            (fully coalesced), and the CTA's partial sums of R over every 4096-wide chunk of k go to a small table;
-//   sweep C: one CTA per chunk of 4096 consecutive k: gathers its (R, X_even) from the [k1][k2] layout of W (runs of
-//            4096/L1 entries), transposes through shared memory, two-sided prefix sum of R from the scanned chunk sums,
-//            writes the natural-order output contiguously.
-// L1 is kept small (256 where the row of L2 still fits a CTA) so that sweep A reads x and writes W in >= 128-byte runs.
+// Same folding as dst1.cu (t -> z, complex FFT of length L = N/2, untangle, odd outputs from R_k = X_{2k+1} - X_{2k-1}),
+// with the FFT split four-step style, L = L1 * L2, j = j1*L2 + j2, k = k1 + L1*k2.  ONE persistent kernel runs the
+// whole batch: its CTAs pull work items from a queue in global memory, and the complex intermediate W (8N bytes per
+// column) lives in a two-slot ring of column groups small enough to stay in the 126 MB L2, so that HBM sees each
+// element once on the way in and once on the way out (the r01 version made three full HBM sweeps).  Items, per column:
+//   A (nA tiles): fold x on the fly (the CTA owns a j2 tile AND its mirror tile: every x element is fetched once),
+//       length-L1 FFTs over the strided index j1, four-step twiddle, W[k1*L2 + j2]; the same pass accumulates the
+//       folded sums y_r = sum_{m = r mod Mc, m < L} (x_m + x_{N-m}) e^{i pi m/N} that the anchors need;
+//   D (1 item): exact anchors  X_{2 c CH + 1} = x_L + Im sum_r y_r e^{2 pi i r c / Mc},  Mc = N/CH, CH = 4096: the odd
+//       outputs at the start of every chunk of 4096 k, by one shared-memory FFT of the Mc folded sums;
+//   B (nB tiles): rows k1 and their mirror rows L1 - k1: length-L2 FFTs, real-FFT untangle of the pairs (k, L-k) in
+//       shared memory; (R_k, X_{2k}) go back IN PLACE into the rows of W;
+//   C (nC = L/4096 chunks): gathers its (R, X_even) from the [k1][k2] layout of W, transposes through shared memory,
+//       sums R forward from the chunk's own anchor over the first half and backward from the next chunk's anchor over
+//       the second half (every odd output is reached through a chain of <= 2048 terms from an independently computed
+//       value: the rounding error no longer grows with N as in a global prefix sum), writes the natural-order output.
+// Dependencies (A -> D, A -> B, B + D -> C, C of the group two back -> A: ring slot free) are per-column arrival counters;
+// items are queued in an order in which every dependency points backwards, and a CTA that holds an item is running, so
+// the waits cannot deadlock whatever the number of resident CTAs.
+// Measured alternatives (profiles/r02_l2_dsmem_microbench.md): distributed shared memory in a 16-CTA cluster exchanges
+// 3.2 TB/s over the 112 SMs such clusters can occupy, L2-resident traffic 12 TB/s over all 148 -- hence L2, not DSMEM,
+// also for the sizes (N <= 2^18) whose column would fit a cluster.
 #include "common.cuh"
 #include "fft_smem.cuh"
 #include <math.h>
 
 namespace {
 
-constexpr int SC_CHUNK = 4096, SC_NT = 512;       // sweep C: k's per chunk, threads per chunk
+constexpr int SC_CHUNK = 4096;                                  // k's per chunk of phase C = anchor spacing
+constexpr int64_t RING_SLOT_BYTES = 24ll << 20;                 // W bytes per ring slot (two slots live in L2)
 
 constexpr int row_stride(int Lrow, int nrows) {            // padded row length with (stride mod 16) == max(1, 16/nrows)
     int want = (16 / nrows) > 0 ? (16 / nrows) : 1;
@@ -26,7 +37,9 @@ constexpr int row_stride(int Lrow, int nrows) {            // padded row length 
     return base + (((want - base) % 16) + 16) % 16;
 }
 
-// ------------------------------------------------------------------------------------------------ sweep A
+__device__ __forceinline__ double2 ldcg2(const double2* p) { return __ldcg(p); }
+
+// ------------------------------------------------------------------------------------------------ phase A
 template <int Q1, int TL> struct PACfg {
     static constexpr int L1 = 1 << Q1, GS = L1 / 8;
     static constexpr int T2 = (1 << TL) / L1, T = T2 / 2;        // sub-FFTs per CTA: T of the tile + T of its mirror
@@ -39,16 +52,17 @@ template <int Q1, int TL> struct PACfg {
     static constexpr int CH = 4;                  // loads in flight per thread (register budget)
     static constexpr size_t SMEM = sizeof(double2) * (64 + NHI + 2 * T2 + (size_t)T2 * (SLO + SHI)) +
                                    sizeof(double) * ((size_t)2 * IMOFF);
+    static_assert(sizeof(double) * 2 * IMOFF >= sizeof(double) * 4 * NT, "anchor partial reduction reuses the FFT arrays");
 };
 
+// tile c of one column: x -> W (L complex), ypart[2 j2 + b] (2 L2 complex): the CTA's folded anchor sums
 template <int Q1, int TL>
-__global__ void __launch_bounds__(PACfg<Q1, TL>::NT, TL <= 12 ? 2 : 1)
-dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2* __restrict__ W) {
+__device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int c, const double* __restrict__ x,
+                                        double2* __restrict__ Wc, double2* __restrict__ ypart) {
     using C = PACfg<Q1, TL>;
     constexpr int L1 = C::L1, GS = C::GS, T2 = C::T2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
     const int L2 = (int)(L >> Q1);
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* lo = (double2*)smem_raw;
     double2* hi = lo + 64;
     double2* tB = hi + C::NHI;                       // [T2][2]   exp(-i pi (2 j2 + b)/N)
@@ -57,9 +71,6 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
     double* re = (double*)(t4hi + T2 * C::SHI);
     double* im = re + C::IMOFF;
     const int tid = threadIdx.x;
-    const int c = blockIdx.x;
-    const double* x = in + (int64_t)blockIdx.y * ld_in;            // x_m = x[m-1]
-    double2* Wc = W + (int64_t)blockIdx.y * L;
     auto j2_of = [&](int s) { return s < T ? c * T + s : L2 - c * T - T + (s - T); };
 
     tw_build(lo, hi, 2 * L1, C::NHI, tid, NT);
@@ -75,6 +86,8 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
     }
     __syncthreads();
     // fold: t_m = sin(pi m/N)(x_m + x_{N-m}) + (x_m - x_{N-m})/2 for m = 2j, 2j+1;  z_j = t_{2j} + i t_{2j+1}
+    // anchors: ya[b] += (x_m + x_{N-m}) e^{+i pi m/N} for m = m0 + b < L  (the thread's s = tid % T2 is the same for all its e)
+    double2 ya0 = make_double2(0.0, 0.0), ya1 = make_double2(0.0, 0.0);
 #pragma unroll 1
     for (int i0 = 0; i0 < 8; i0 += C::CH) {
         double x0[C::CH], x1[C::CH], y0[C::CH], y1[C::CH];
@@ -83,10 +96,10 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
             int e = tid + (i0 + i) * NT;
             int s = e % T2, j1 = e / T2;
             int64_t m0 = 2 * ((int64_t)j1 * L2 + j2_of(s));
-            x0[i] = (m0 >= 1) ? x[m0 - 1] : 0.0;
-            x1[i] = x[m0];
-            y0[i] = (m0 >= 1) ? x[N - m0 - 1] : 0.0;
-            y1[i] = x[N - m0 - 2];
+            x0[i] = (m0 >= 1) ? __ldcs(x + m0 - 1) : 0.0;
+            x1[i] = __ldcs(x + m0);
+            y0[i] = (m0 >= 1) ? __ldcs(x + N - m0 - 1) : 0.0;
+            y1[i] = __ldcs(x + N - m0 - 2);
         }
 #pragma unroll
         for (int i = 0; i < C::CH; ++i) {
@@ -96,8 +109,14 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
             double2 b0 = tB[2 * s], b1 = tB[2 * s + 1];
             double s0 = -(a.x * b0.y + a.y * b0.x);               // sin(pi m0 / N)
             double s1 = -(a.x * b1.y + a.y * b1.x);
-            re[s * RS + PADI(j1)] = s0 * (x0[i] + y0[i]) + 0.5 * (x0[i] - y0[i]);
-            im[s * RS + PADI(j1)] = s1 * (x1[i] + y1[i]) + 0.5 * (x1[i] - y1[i]);
+            const double sum0 = x0[i] + y0[i], sum1 = x1[i] + y1[i];
+            re[s * RS + PADI(j1)] = s0 * sum0 + 0.5 * (x0[i] - y0[i]);
+            im[s * RS + PADI(j1)] = s1 * sum1 + 0.5 * (x1[i] - y1[i]);
+            if (j1 < L1 / 2) {                                    // m0, m0 + 1 < L
+                double c0 = a.x * b0.x - a.y * b0.y, c1 = a.x * b1.x - a.y * b1.y;     // cos(pi m / N)
+                ya0.x = fma(sum0, c0, ya0.x); ya0.y = fma(sum0, s0, ya0.y);
+                ya1.x = fma(sum1, c1, ya1.x); ya1.y = fma(sum1, s1, ya1.y);
+            }
         }
     }
     __syncthreads();
@@ -112,11 +131,73 @@ dst1_pa_kernel(int log2N, const double* __restrict__ in, int64_t ld_in, double2*
         int s = e % T2, k1 = e / T2;
         double2 v = make_double2(re[s * RS + PADI(k1)], im[s * RS + PADI(k1)]);
         double2 w = cmul(t4hi[s * C::SHI + (k1 >> 5)], t4lo[s * C::SLO + (k1 & 31)]);
-        Wc[(int64_t)k1 * L2 + j2_of(s)] = cmul(v, w);
+        __stcg(&Wc[(int64_t)k1 * L2 + j2_of(s)], cmul(v, w));
+    }
+    __syncthreads();
+    // anchor partials: sum over the NT / T2 threads that share s (fixed order), one entry per (j2, b)
+    double* red = re;                                 // [NT][4]
+    red[4 * tid + 0] = ya0.x; red[4 * tid + 1] = ya0.y; red[4 * tid + 2] = ya1.x; red[4 * tid + 3] = ya1.y;
+    __syncthreads();
+    if (tid < 2 * T2) {
+        const int s = tid >> 1, b = tid & 1;
+        double ar = 0.0, ai = 0.0;
+        for (int q = 0; q < NT / T2; ++q) { ar += red[4 * (s + q * T2) + 2 * b]; ai += red[4 * (s + q * T2) + 2 * b + 1]; }
+        __stcg(&ypart[2 * j2_of(s) + b], make_double2(ar, ai));
     }
 }
 
-// ------------------------------------------------------------------------------------------------ sweep B
+// ------------------------------------------------------------------------------------------------ phase D (anchors)
+// anchors[c] = scale * X_{2 c CH + 1} = scale * (x_L + Im sum_{r < Mc} y_r e^{2 pi i r c / Mc}),  c < nch = Mc / 2
+template <int NT, int QM>
+__device__ __forceinline__ void phase_d(unsigned char* smem_raw, int log2N, int log2L1, const double* __restrict__ x,
+                                        const double2* __restrict__ ypart, double scale, double* __restrict__ anchors) {
+    constexpr int Mc = 1 << QM, nch = Mc / 2;
+    const int64_t L = (int64_t)1 << (log2N - 1);
+    const int nfold = SC_CHUNK >> log2L1;             // entries of ypart per residue: 2 L2 / Mc = CH / L1
+    const int tid = threadIdx.x;
+    const double xL = x[L - 1];
+    if constexpr (QM <= 7) {                          // Mc <= 128: direct DFT with a full table
+        double2* y = (double2*)smem_raw;              // [Mc]
+        double2* tab = y + Mc;                        // [Mc] e^{2 pi i u / Mc}
+        for (int r = tid; r < Mc; r += NT) {
+            double ar = 0.0, ai = 0.0;
+            for (int q = 0; q < nfold; ++q) { double2 v = ldcg2(ypart + r + (int64_t)q * Mc); ar += v.x; ai += v.y; }
+            y[r] = make_double2(ar, ai);
+            double sn, cs; sincospi(2.0 * (double)r / (double)Mc, &sn, &cs); tab[r] = make_double2(cs, sn);
+        }
+        __syncthreads();
+        for (int c = tid; c < nch; c += NT) {
+            double a0 = 0.0, a1 = 0.0;
+            int u = 0;
+            for (int r = 0; r < Mc; r += 2) {
+                double2 y0 = y[r], w0 = tab[u]; u = (u + c) & (Mc - 1);
+                double2 y1 = y[r + 1], w1 = tab[u]; u = (u + c) & (Mc - 1);
+                a0 = fma(y0.x, w0.y, fma(y0.y, w0.x, a0));
+                a1 = fma(y1.x, w1.y, fma(y1.y, w1.x, a1));
+            }
+            anchors[c] = scale * (xL + (a0 + a1));
+        }
+    } else {                                          // Im IDFT(y) = -Im FFT(conj y): one shared-memory FFT of length Mc
+        constexpr int GS = Mc / 8;
+        double* re = (double*)smem_raw;               // [Mc + 16]
+        double* im = re + Mc + 16;
+        double2* lo = (double2*)(im + Mc + 16);       // [64]
+        double2* hi = lo + 64;                        // [Mc/64 + 1]
+        for (int r = tid; r < Mc; r += NT) {
+            double ar = 0.0, ai = 0.0;
+            for (int q = 0; q < nfold; ++q) { double2 v = ldcg2(ypart + r + (int64_t)q * Mc); ar += v.x; ai += v.y; }
+            re[PADI(r)] = ar; im[PADI(r)] = -ai;
+        }
+        tw_build(lo, hi, Mc, Mc / 64 + 1, tid, NT);
+        __syncthreads();
+        // the first GS threads (whole warps, GS >= 32) run the FFT; their passes synchronise on named barrier 1
+        if (tid < GS) fft_smem<QM, (GS < NT ? 2 : 1)>(re, im, tid, 0, lo, hi, 1);
+        __syncthreads();
+        for (int c = tid; c < nch; c += NT) anchors[c] = scale * (xL - im[PADI(c)]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ phase B
 template <int Q2, int TL> struct PBCfg {
     static constexpr int L2 = 1 << Q2, GS = L2 / 8;
     static constexpr int R2 = (1 << TL) / L2, T = R2 / 2;        // rows per CTA: T rows k1 + their T mirror rows
@@ -137,23 +218,20 @@ __device__ __forceinline__ void untangle_pair(double2& zk, double2& zm, double2 
     zm = make_double2(E.x - wO.x, E.y - wO.y);
 }
 
+// tile c of one column: rows of W -> (R_k, X_{2k}) in place, scaled;  *xlast = scale X_{N-1}  (tile 0)
 template <int Q2, int TL>
-__global__ void __launch_bounds__(PBCfg<Q2, TL>::NT, TL <= 12 ? 2 : 1)
-dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restrict__ xlast, int xstride,
-               double* __restrict__ part) {
+__device__ __forceinline__ void phase_b(unsigned char* smem_raw, int log2N, int c, double2* __restrict__ Wc, double scale,
+                                        double* __restrict__ xlast) {
     using C = PBCfg<Q2, TL>;
     constexpr int L2 = C::L2, GS = C::GS, R2 = C::R2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
     const int L1 = (int)(L >> Q2);
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* lo = (double2*)smem_raw;
     double2* hi = lo + 64;
     double2* rowtw = hi + C::NHI;                    // [R2] exp(-2 pi i row/N)
     double* re = (double*)(rowtw + R2);
     double* im = re + C::IMOFF;
     const int tid = threadIdx.x;
-    const int c = blockIdx.x;
-    double2* Wc = W + (int64_t)blockIdx.y * L;
     auto row_of = [&](int slot) {
         int rho = c * T + (slot < T ? slot : slot - T);
         return slot < T ? rho : (rho == 0 ? L1 / 2 : L1 - rho);
@@ -163,7 +241,7 @@ dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restr
     {
         const double2* row = Wc + (int64_t)row_of(g) * L2;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) v[r] = row[gt + r * GS];
+        for (int r = 0; r < 8; ++r) v[r] = ldcg2(row + gt + r * GS);
     }
     tw_build(lo, hi, 2 * L2, C::NHI, tid, NT);        // exp(-2 pi i u/(2 L2)) = exp(-2 pi i (L1 u)/N)
     for (int i = tid; i < R2; i += NT) {
@@ -186,7 +264,7 @@ dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restr
             if (k2 == 0) {
                 double a = re[0], b = im[0];
                 re[0] = 0.5 * (a + b); im[0] = 0.0;               // R_0 := X_1 = T_0/2
-                xlast[(int64_t)blockIdx.y * xstride] = scale * 0.5 * (b - a);   // X_{N-1} = -T_L/2, start of the backward sum
+                *xlast = scale * 0.5 * (b - a);                    // X_{N-1} = -T_L/2: where the last chunk's backward sum starts
             } else if (k2 <= L2 / 2) {
                 int ia = PADI(k2), ib = PADI(L2 - k2);
                 double2 zk = make_double2(re[ia], im[ia]), zm = make_double2(re[ib], im[ib]);
@@ -209,79 +287,23 @@ dst1_pb_kernel(int log2N, double2* __restrict__ W, double scale, double* __restr
         int e = tid + i * NT;
         int slot = e / L2, k2 = e % L2;
         int ia = slot * RS + PADI(k2);
-        Wc[(int64_t)row_of(slot) * L2 + k2] = make_double2(scale * re[ia], scale * im[ia]);
-    }
-    // partial chunk sums of R: chunk of k = row + L1*k2 is k2 / CW (L1 <= SC_CHUNK), fixed order -> deterministic
-    {
-        const int CW = SC_CHUNK / L1 > 0 ? SC_CHUNK / L1 : 1;
-        const int nch = L2 / CW;
-        double* pc = part + ((int64_t)blockIdx.y * gridDim.x + c) * nch;
-        for (int ch = tid; ch < nch; ch += NT) {
-            double acc = 0.0;
-            for (int slot = 0; slot < R2; ++slot)
-                for (int j = 0; j < CW; ++j) acc += re[slot * RS + PADI(ch * CW + j)];
-            pc[ch] = scale * acc;
-        }
+        __stcg(&Wc[(int64_t)row_of(slot) * L2 + k2], make_double2(scale * re[ia], scale * im[ia]));
     }
 }
 
-// ------------------------------------------------------------------------------------------------ sweep C
-// Odd outputs P_k = X_{2k+1} from R_k = P_k - P_{k-1} (R_0 = X_1): a TWO-SIDED sum.  Lower half of the chunks forward
-// from P_0 = X_1, upper half backward from the independently known P_{L-1} = X_{N-1} (sweep B, xlast): every output is
-// reached through the shorter chain and the small tail of a decaying spectrum is summed from small terms only.
-// sums: per column nchunks chunk sums + 1 slot for X_{N-1}; part: per column [nB][nchunks] partial sums of sweep B.
-
-// chunk sums from sweep B's partials: one thread per chunk, fixed order over the nB contributing CTAs (deterministic)
-__global__ void __launch_bounds__(128)
-dst1_chunkreduce_kernel(int nchunks, int nB, const double* __restrict__ part, double* __restrict__ sums) {
-    const int ch = blockIdx.x * 128 + threadIdx.x;
-    if (ch >= nchunks) return;
-    const double* pc = part + (int64_t)blockIdx.y * nB * nchunks + ch;
-    double acc = 0.0;
-    int b = 0;
-    for (; b + 4 <= nB; b += 4) {
-        double v0 = pc[(int64_t)b * nchunks], v1 = pc[(int64_t)(b + 1) * nchunks];
-        double v2 = pc[(int64_t)(b + 2) * nchunks], v3 = pc[(int64_t)(b + 3) * nchunks];
-        acc += v0; acc += v1; acc += v2; acc += v3;
-    }
-    for (; b < nB; ++b) acc += pc[(int64_t)b * nchunks];
-    sums[(int64_t)blockIdx.y * (nchunks + 1) + ch] = acc;
-}
-
-// per column (one CTA): chunks c < nch/2 get the exclusive prefix of the chunk sums, chunks c >= nch/2 the exclusive
-// suffix (sum of the chunks above them, accumulated from the top)
-__global__ void __launch_bounds__(1024)
-dst1_scansums_kernel(int nchunks, double* __restrict__ sums) {
-    double* s = sums + (int64_t)blockIdx.x * (nchunks + 1);
-    __shared__ double wsum[32];
-    __shared__ double tot;
-    const int half = nchunks / 2;
-    for (int dir = 0; dir < 2; ++dir) {
-        const int cnt = dir == 0 ? half : nchunks - half;
-        double carry = 0.0;
-        for (int base = 0; base < cnt; base += 1024) {
-            const int q = base + threadIdx.x;
-            const int i = dir == 0 ? q : nchunks - 1 - q;
-            double v = q < cnt ? s[i] : 0.0;
-            double incl = group_scan_incl<1024>(v, threadIdx.x, wsum);
-            if (q < cnt) s[i] = carry + incl - v;
-            if (threadIdx.x == 1023) tot = incl;
-            __syncthreads();
-            carry += tot;
-            __syncthreads();
-        }
-    }
-}
-
-// shared-memory index of local k (0..4095): +1 per 8 (blocked scan reads: thread t owns k = 8t..8t+7), +PM per row of
-// K1C (transposed stores: a half-warp holds consecutive k2 of one k1, i.e. k's that are K1C apart)
+// ------------------------------------------------------------------------------------------------ phase C
+// Odd outputs P_k = X_{2k+1} of chunk c (k in [c CH, (c+1) CH)) from R_k = P_k - P_{k-1}: first half forward from the
+// chunk's anchor P_{c CH}, second half backward from the next chunk's anchor P_{(c+1) CH} (last chunk: from X_{N-1}).
+// shared-memory index of local k (0..4095): +1 per 8 (blocked scan reads), +PM per row of K1C (transposed stores: a
+// half-warp holds consecutive k2 of one k1, i.e. k's that are K1C apart)
 __device__ __forceinline__ int sc_pad(int k, int log2K1C, int PM) { return k + (k >> 3) + (k >> log2K1C) * PM; }
 constexpr int SC_ARR = SC_CHUNK + SC_CHUNK / 8 + 32 * 16 + 8;       // doubles per array
 static_assert(SC_ARR % 16 == 8, "R and X_even banks interleave in the output loop");
+constexpr size_t SC_SMEM = 2 * (size_t)SC_ARR * sizeof(double) + 64 * sizeof(double);
 
-__global__ void __launch_bounds__(SC_NT)
-dst1_scanapply_kernel(int log2N, int log2L1, const double2* __restrict__ W, double* __restrict__ out, int64_t ld_out,
-                      const double* __restrict__ sums) {
+template <int NT>
+__device__ __forceinline__ void phase_c(unsigned char* smem_raw, int log2N, int log2L1, int c, const double2* __restrict__ Wc,
+                                        double* __restrict__ o, const double* __restrict__ anchors) {
     const int64_t L = (int64_t)1 << (log2N - 1);
     const int nch = (int)(L / SC_CHUNK);
     const int L1 = 1 << log2L1;
@@ -290,185 +312,270 @@ dst1_scanapply_kernel(int log2N, int log2L1, const double2* __restrict__ W, doub
     const int log2K1C = L1 >= SC_CHUNK ? 12 : log2L1;                 // k1's per chunk K1C = min(L1, 4096)
     const int K1C = 1 << log2K1C;
     const int PM = CW >= 16 ? 1 : 16 / CW;
-    const int c = blockIdx.x;
-    const bool fwd = c < nch / 2;
-    const double2* Wc = W + (int64_t)blockIdx.y * L;
-    double* o = out + (int64_t)blockIdx.y * ld_out;
-    const double* sc = sums + (int64_t)blockIdx.y * (nch + 1);
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sR = (double*)smem_raw;
     double* sX = sR + SC_ARR;
-    __shared__ double wsum[32];
+    double* wsum = sX + SC_ARR;                                        // [2][32]
+    const int tid = threadIdx.x;
     // chunk c holds k = k1 + L1*k2: (L1 <= 4096) all k1, k2 in [c*CW, (c+1)*CW); (L1 > 4096) one k2 and a range of k1
     const int64_t k2base = L1 >= SC_CHUNK ? ((int64_t)c * SC_CHUNK) / L1 : (int64_t)c * CW;
     const int k1base = L1 >= SC_CHUNK ? (int)(((int64_t)c * SC_CHUNK) % L1) : 0;
-    constexpr int PER = SC_CHUNK / SC_NT;
-    double2 v[PER];
+    constexpr int PER = SC_CHUNK / NT;
+    {
+        double2 v[PER];
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
-        const int e = threadIdx.x + i * SC_NT;
-        const int k2o = e % CW, k1 = e / CW;
-        v[i] = Wc[(int64_t)(k1base + k1) * L2 + k2base + k2o];
-    }
+        for (int i = 0; i < PER; ++i) {
+            const int e = tid + i * NT;
+            const int k2o = e % CW, k1 = e / CW;
+            v[i] = ldcg2(Wc + (int64_t)(k1base + k1) * L2 + k2base + k2o);
+        }
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
-        const int e = threadIdx.x + i * SC_NT;
-        const int k2o = e % CW, k1 = e / CW;
-        const int ix = sc_pad(k1 + K1C * k2o, log2K1C, PM);
-        sR[ix] = v[i].x; sX[ix] = v[i].y;
+        for (int i = 0; i < PER; ++i) {
+            const int e = tid + i * NT;
+            const int k2o = e % CW, k1 = e / CW;
+            const int ix = sc_pad(k1 + K1C * k2o, log2K1C, PM);
+            sR[ix] = v[i].x; sX[ix] = v[i].y;
+        }
     }
+    // bases: forward half starts at the anchor; backward half at P_{(c+1)CH - 1} = anchor_{c+1} - R_{(c+1) CH}
+    double base;
+    constexpr int HT = NT / 2;                                         // threads per half
+    const int half = tid / HT, ht = tid % HT;
+    if (half == 0) base = __ldcg(anchors + c);
+    else if (c + 1 < nch) {
+        const int64_t kn = (int64_t)(c + 1) * SC_CHUNK;               // first k of the next chunk
+        base = __ldcg(anchors + c + 1) - ldcg2(Wc + (kn & (L1 - 1)) * L2 + (kn >> log2L1)).x;
+    } else base = __ldcg(anchors + nch);                               // X_{N-1}
     __syncthreads();
-    double loc[PER], val[PER]; double run = 0.0;
+    // both halves: inclusive scan of a sequence whose first term is dropped (forward u_q = R_q, q >= 1; backward
+    // w_j = R_{CH-j}, j >= 1): P_q = base + incl (forward),  P_{CH-1-j} = base - incl (backward)
+    double loc[PER]; double run = 0.0;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-        const int q = threadIdx.x * PER + i;
-        val[i] = sR[sc_pad(fwd ? q : SC_CHUNK - 1 - q, log2K1C, PM)];
-        run += val[i]; loc[i] = run;
+        const int q = ht * PER + i;
+        const double val = q == 0 ? 0.0 : sR[sc_pad(half == 0 ? q : SC_CHUNK - q, log2K1C, PM)];
+        run += val; loc[i] = run;
     }
-    double incl = group_scan_incl<SC_NT>(run, threadIdx.x, wsum);
+    const double incl = group_scan_incl<HT>(run, ht, wsum + 32 * half);       // barriers inside: reads done before the writes below
     const double off = incl - run;
-    if (fwd) {
-        const double base = sc[c];
 #pragma unroll
-        for (int i = 0; i < PER; ++i) sR[sc_pad(threadIdx.x * PER + i, log2K1C, PM)] = base + off + loc[i];     // P_k
-    } else {
-        const double xl = sc[nch], above = sc[c];
-#pragma unroll
-        for (int i = 0; i < PER; ++i)                                // P_k = X_{N-1} - sum_{m > k} R_m
-            sR[sc_pad(SC_CHUNK - 1 - (threadIdx.x * PER + i), log2K1C, PM)] = xl - (above + (off + loc[i] - val[i]));
+    for (int i = 0; i < PER; ++i) {
+        const int q = ht * PER + i;
+        if (half == 0) sR[sc_pad(q, log2K1C, PM)] = base + (off + loc[i]);
+        else sR[sc_pad(SC_CHUNK - 1 - q, log2K1C, PM)] = base - (off + loc[i]);
     }
     __syncthreads();
     // natural order: X_{2k} at o[2k-1], P_k = X_{2k+1} at o[2k]; the chunk's 8192 outputs are contiguous from o[2 k0 - 1]
     const int64_t obase = 2 * (int64_t)c * SC_CHUNK - 1;
 #pragma unroll
     for (int i = 0; i < 2 * PER; ++i) {
-        const int j = threadIdx.x + i * SC_NT;
+        const int j = tid + i * NT;
         const int ix = sc_pad(j >> 1, log2K1C, PM);
         const double val2 = (j & 1) ? sR[ix] : sX[ix];
-        if (obase + j >= 0) o[obase + j] = val2;
+        if (obase + j >= 0) __stcs(o + obase + j, val2);
     }
 }
 
-// ------------------------------------------------------------------------------------------------ host side
-template <int Q1, int TL>
-int launch_pa(lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in, double2* W) {
-    using C = PACfg<Q1, TL>;
-    const int L2 = 1 << (log2N - 1 - Q1);
-    LRP_PROF(ctx, K_DST_P1, 16.0 * ((int64_t)1 << log2N) * cols, 0);
-    dst1_pa_kernel<Q1, TL><<<dim3(L2 / C::T2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, in, ld_in, W);
-    LRP_LAUNCHED(ctx);
-    return LRP_OK;
-}
-template <int Q2, int TL>
-int launch_pb(lrp_ctx* ctx, int log2N, int cols, double2* W, double scale, double* xlast, int xstride, double* part) {
-    using C = PBCfg<Q2, TL>;
-    const int L1 = 1 << (log2N - 1 - Q2);
-    LRP_PROF(ctx, K_DST_P2, 16.0 * ((int64_t)1 << log2N) * cols, 0);
-    dst1_pb_kernel<Q2, TL><<<dim3(L1 / C::R2, cols), C::NT, C::SMEM, ctx->stream>>>(log2N, W, scale, xlast, xstride, part);
-    LRP_LAUNCHED(ctx);
-    return LRP_OK;
-}
+// ------------------------------------------------------------------------------------------------ the persistent kernel
+struct LargeArgs {
+    int log2N, batch, gc, G, nA, nB, nC;
+    const double* in; int64_t ld_in; double* out; int64_t ld_out; double scale;
+    double2* W;            // [2 gc][L]      ring of two column groups
+    double2* ypart;        // [2 gc][2 L2]
+    double* anchors;       // [2 gc][nch + 1]   (last entry: scale * X_{N-1})
+    int* counters;         // [0]: queue head; [1 + 4 col + {0,1,2,3}]: A tiles, B tiles, D, C chunks done for column col
+};
+enum { PH_A = 0, PH_B = 1, PH_D = 2, PH_C = 3, PH_DONE = 4 };
 
-#define LRP_QL_SWITCH(q, TLV, FN, ...)                  \
-    switch (q) {                                        \
-        case 7: return FN<7, TLV>(__VA_ARGS__);         \
-        case 8: return FN<8, TLV>(__VA_ARGS__);         \
-        case 9: return FN<9, TLV>(__VA_ARGS__);         \
-        case 10: return FN<10, TLV>(__VA_ARGS__);       \
-        case 11: return FN<11, TLV>(__VA_ARGS__);       \
-        default: return LRP_ERR_UNSUPPORTED_N;          \
+// queue order: A(0); then for every group g: D(g), B(g), A(g+1), C(g) -- every dependency points at least one phase back
+__device__ __forceinline__ void decode_item(const LargeArgs& a, int item, int& phase, int& g, int& local) {
+    auto cols = [&](int gg) { int r = a.batch - gg * a.gc; return r < a.gc ? r : a.gc; };
+    int i = item;
+    const int c0 = cols(0) * a.nA;
+    if (i < c0) { phase = PH_A; g = 0; local = i; return; }
+    i -= c0;
+    const int full = a.gc * (1 + a.nB + a.nA + a.nC);
+    const int nfull = a.G >= 2 ? a.G - 2 : 0;                 // groups 0 .. G-3 and their successors are full
+    int gg = i / full; if (gg > nfull) gg = nfull;
+    i -= gg * full;
+    for (; gg < a.G; ++gg) {
+        const int cg = cols(gg), cn = gg + 1 < a.G ? cols(gg + 1) : 0;
+        if (i < cg) { phase = PH_D; g = gg; local = i; return; }
+        i -= cg;
+        if (i < a.nB * cg) { phase = PH_B; g = gg; local = i; return; }
+        i -= a.nB * cg;
+        if (i < a.nA * cn) { phase = PH_A; g = gg + 1; local = i; return; }
+        i -= a.nA * cn;
+        if (i < a.nC * cg) { phase = PH_C; g = gg; local = i; return; }
+        i -= a.nC * cg;
     }
-int dispatch_pa(int q1, int tl, lrp_ctx* ctx, int log2N, int cols, const double* in, int64_t ld_in, double2* W) {
-    if (tl == 12) { LRP_QL_SWITCH(q1, 12, launch_pa, ctx, log2N, cols, in, ld_in, W) }
-    if (q1 == 12) return launch_pa<12, 13>(ctx, log2N, cols, in, ld_in, W);
-    LRP_QL_SWITCH(q1, 13, launch_pa, ctx, log2N, cols, in, ld_in, W)
-}
-int dispatch_pb(int q2, int tl, lrp_ctx* ctx, int log2N, int cols, double2* W, double scale, double* xlast, int xstride,
-                double* part) {
-    if (tl == 12) { LRP_QL_SWITCH(q2, 12, launch_pb, ctx, log2N, cols, W, scale, xlast, xstride, part) }
-    if (q2 == 12) return launch_pb<12, 13>(ctx, log2N, cols, W, scale, xlast, xstride, part);
-    LRP_QL_SWITCH(q2, 13, launch_pb, ctx, log2N, cols, W, scale, xlast, xstride, part)
+    phase = PH_DONE; g = 0; local = 0;
 }
 
-// split L = 2^q = L1 * L2 and the tile sizes (2^tl points per CTA) of the two sweeps.  L1 = 256 wherever a pair of
-// rows of L2 still fits a CTA (sweep A then moves x and W in 128-byte runs and its sub-FFTs are one warp each).
-struct Plan { int q1, q2, tla, tlb, nB, nch; };
-int tile_rows(int tl, int q) { return 1 << (tl - q); }
+__device__ __forceinline__ void wait_count(const int* p, int need) {
+    while (*(volatile const int*)p < need) __nanosleep(200);
+}
+
+template <int Q1, int Q2, int TL> struct FusedCfg {
+    static constexpr int NT = (1 << TL) / 8;
+    static constexpr int QM = Q1 + Q2 + 1 - 12;                        // log2 of the folded anchor sums per column (Mc = N / 4096)
+    static constexpr int MC = 1 << QM;
+    static constexpr size_t DSMEM = QM <= 7 ? sizeof(double2) * 2 * MC : sizeof(double) * 2 * (MC + 16) + sizeof(double2) * (64 + MC / 64 + 1);
+    static constexpr size_t m1 = PACfg<Q1, TL>::SMEM > PBCfg<Q2, TL>::SMEM ? PACfg<Q1, TL>::SMEM : PBCfg<Q2, TL>::SMEM;
+    static constexpr size_t m2 = SC_SMEM > DSMEM ? SC_SMEM : DSMEM;
+    static constexpr size_t SMEM = m1 > m2 ? m1 : m2;
+};
+
+template <int Q1, int Q2, int TL>
+__global__ void __launch_bounds__(FusedCfg<Q1, Q2, TL>::NT, TL <= 12 ? 2 : 1)
+dst1_fused_kernel(LargeArgs a) {
+    constexpr int NT = FusedCfg<Q1, Q2, TL>::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int s_item[4];
+    const int64_t L = (int64_t)1 << (a.log2N - 1);
+    const int64_t L2 = L >> Q1;
+    const int nch = (int)(L / SC_CHUNK);
+    const int tid = threadIdx.x;
+#ifdef LRP_DST_STATS
+    unsigned long long* stats = (unsigned long long*)(a.counters + 1 + 4 * a.batch + 1);      // [5 phases incl. wait][cycles, items]
+    long long t_prev = clock64();
+#endif
+    int next_item = 0;
+    if (tid == 0) next_item = atomicAdd(a.counters, 1);
+    for (;;) {
+        __syncthreads();                                   // previous item's shared memory is dead; s_item reusable
+        if (tid == 0) {
+            const int item = next_item;
+            next_item = atomicAdd(a.counters, 1);          // the queue is read one item ahead: its latency hides behind this item
+            int phase, g, local;
+            decode_item(a, item, phase, g, local);
+            int col = 0, tile = 0;
+            if (phase != PH_DONE) {
+                const int nt = phase == PH_A ? a.nA : (phase == PH_B ? a.nB : (phase == PH_C ? a.nC : 1));
+                col = g * a.gc + local / nt; tile = local % nt;
+                const int* cnt = a.counters + 1 + 4 * col;
+                if (phase == PH_A) { if (g >= 2) wait_count(cnt - 4 * 2 * a.gc + 3, a.nC); }          // ring slot free
+                else if (phase == PH_C) { wait_count(cnt + 1, a.nB); wait_count(cnt + 2, 1); }
+                else wait_count(cnt, a.nA);                                                            // B, D
+                __threadfence();
+            }
+#ifdef LRP_DST_STATS
+            { long long t = clock64(); atomicAdd(&stats[8], (unsigned long long)(t - t_prev)); atomicAdd(&stats[9], 1ull); t_prev = t; }
+#endif
+            s_item[0] = phase; s_item[1] = col; s_item[2] = tile; s_item[3] = g;
+        }
+        __syncthreads();
+        const int phase = s_item[0], col = s_item[1], tile = s_item[2], g = s_item[3];
+        if (phase == PH_DONE) break;
+        const int slot = (g & 1) * a.gc + (col - g * a.gc);
+        double2* Wc = a.W + (int64_t)slot * L;
+        double2* yp = a.ypart + (int64_t)slot * 2 * L2;
+        double* anc = a.anchors + (int64_t)slot * (nch + 1);
+        const double* x = a.in + (int64_t)col * a.ld_in;
+        if (phase == PH_A) phase_a<Q1, TL>(smem_raw, a.log2N, tile, x, Wc, yp);
+        else if (phase == PH_B) phase_b<Q2, TL>(smem_raw, a.log2N, tile, Wc, a.scale, anc + nch);
+        else if (phase == PH_D) phase_d<NT, FusedCfg<Q1, Q2, TL>::QM>(smem_raw, a.log2N, Q1, x, yp, a.scale, anc);
+        else phase_c<NT>(smem_raw, a.log2N, Q1, tile, Wc, a.out + (int64_t)col * a.ld_out, anc);
+        __threadfence();                                   // this item's global writes before the arrival below
+        __syncthreads();
+        if (tid == 0) atomicAdd(a.counters + 1 + 4 * col + phase, 1);
+#ifdef LRP_DST_STATS
+        if (tid == 0) { long long t = clock64(); atomicAdd(&stats[2 * phase], (unsigned long long)(t - t_prev)); atomicAdd(&stats[2 * phase + 1], 1ull); t_prev = t; }
+#endif
+    }
+}
+
+// split L = 2^q = L1 * L2 and the tile size (2^tl points per CTA).  L1 = 256 wherever a pair of rows of L2 still
+// fits a CTA (phase A then moves x and W in 128-byte runs and its sub-FFTs are one warp each).
+struct Plan { int q1, q2, tl, nA, nB, nC; };
 Plan plan(int log2N) {
     const int q = log2N - 1;
     Plan p;
     p.q1 = q <= 14 ? 7 : 8;
     if (q - p.q1 > 12) p.q1 = q - 12;
     p.q2 = q - p.q1;
-    p.tla = p.q1 >= 9 ? 13 : 12;
-    p.tlb = p.q2 >= 12 ? 13 : 12;
-    p.nB = (1 << p.q1) / tile_rows(p.tlb, p.q2);
-    p.nch = (int)(((int64_t)1 << q) / SC_CHUNK);
+    p.tl = (p.q1 >= 9 || p.q2 >= 12) ? 13 : 12;
+    p.nA = (1 << p.q2) / ((1 << p.tl) >> p.q1);               // L2 / T2
+    p.nB = (1 << p.q1) / ((1 << p.tl) >> p.q2);               // L1 / R2
+    p.nC = (int)(((int64_t)1 << q) / SC_CHUNK);
     return p;
 }
 
-// columns per group (workspace bound: W of one group)
+// columns per ring slot
 int group_cols(int64_t N, int batch) {
-    int64_t per_col = N * 8;
-    const int64_t budget_mb = 4096;
-    int g = (int)((budget_mb << 20) / per_col);
+    int64_t g = RING_SLOT_BYTES / (N * 8);
     if (g < 1) g = 1;
     if (g > batch) g = batch;
-    return g;
+    return (int)g;
 }
 
-template <int Q, int TL>
-int init_pair(lrp_ctx* ctx) {
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pa_kernel<Q, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PACfg<Q, TL>::SMEM));
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_pb_kernel<Q, TL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PBCfg<Q, TL>::SMEM));
-    return LRP_OK;
+typedef void (*FusedKernel)(LargeArgs);
+struct KernelEntry { int q1, q2, tl; FusedKernel fn; size_t smem; int nt; };
+template <int Q1, int Q2, int TL> KernelEntry entry() {
+    return KernelEntry{Q1, Q2, TL, dst1_fused_kernel<Q1, Q2, TL>, FusedCfg<Q1, Q2, TL>::SMEM, FusedCfg<Q1, Q2, TL>::NT};
+}
+const KernelEntry* kernel_table(int* count) {
+    static const KernelEntry tab[] = {
+        entry<7, 7, 12>(), entry<8, 7, 12>(), entry<8, 8, 12>(), entry<8, 9, 12>(), entry<8, 10, 12>(), entry<8, 11, 12>(),
+        entry<8, 12, 13>(), entry<9, 12, 13>(), entry<10, 12, 13>(), entry<11, 12, 13>(), entry<12, 12, 13>()};
+    *count = (int)(sizeof(tab) / sizeof(tab[0]));
+    return tab;
 }
 
 }  // namespace
 
 int dst1_large_init(lrp_ctx* ctx) {
-    LRP_TRY((init_pair<7, 12>(ctx))); LRP_TRY((init_pair<8, 12>(ctx))); LRP_TRY((init_pair<9, 12>(ctx)));
-    LRP_TRY((init_pair<10, 12>(ctx))); LRP_TRY((init_pair<11, 12>(ctx)));
-    LRP_TRY((init_pair<7, 13>(ctx))); LRP_TRY((init_pair<8, 13>(ctx))); LRP_TRY((init_pair<9, 13>(ctx)));
-    LRP_TRY((init_pair<10, 13>(ctx))); LRP_TRY((init_pair<11, 13>(ctx))); LRP_TRY((init_pair<12, 13>(ctx)));
-    LRP_CUDA(ctx, cudaFuncSetAttribute(dst1_scanapply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * SC_ARR * (int)sizeof(double)));
+    int cnt; const KernelEntry* tab = kernel_table(&cnt);
+    for (int i = 0; i < cnt; ++i)
+        LRP_CUDA(ctx, cudaFuncSetAttribute(tab[i].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab[i].smem));
     return LRP_OK;
 }
 
 size_t dst1_large_ws(int64_t N, int32_t batch) {
-    const int g = group_cols(N, batch);
+    const int gc = group_cols(N, batch);
     const int64_t L = N / 2;
     const Plan p = plan(lrp_ilog2(N));
-    return lrp_align_up((size_t)g * L * sizeof(double2)) + lrp_align_up((size_t)g * (p.nch + 1) * sizeof(double)) +
-           lrp_align_up((size_t)g * p.nB * p.nch * sizeof(double));
+    const int64_t L2 = (int64_t)1 << p.q2;
+    return lrp_align_up((size_t)2 * gc * L * sizeof(double2)) + lrp_align_up((size_t)2 * gc * 2 * L2 * sizeof(double2)) +
+           lrp_align_up((size_t)2 * gc * (p.nC + 1) * sizeof(double)) + lrp_align_up((size_t)(1 + 4 * (size_t)batch + 32) * sizeof(int));
 }
+
+#ifdef LRP_DST_STATS
+static int* g_dbg_counters = nullptr; static int g_dbg_batch = 0;
+extern "C" int lrp_debug_dst_stats(unsigned long long* out) {      // work builds only: 10 values [phase A,B,D,C,wait] x [cycles, items]
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpy(out, g_dbg_counters + 1 + 4 * g_dbg_batch + 1, 10 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+}
+#endif
 
 int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
                double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes) {
     const int64_t N = (int64_t)1 << log2N, L = N / 2;
     if (log2N > 25) return LRP_ERR_UNSUPPORTED_N;
     const Plan p = plan(log2N);
-    const int g = group_cols(N, batch);
+    const int64_t L2 = (int64_t)1 << p.q2;
+    LargeArgs a{};
+    a.log2N = log2N; a.batch = batch; a.gc = group_cols(N, batch); a.G = (batch + a.gc - 1) / a.gc;
+    a.nA = p.nA; a.nB = p.nB; a.nC = p.nC;
+    a.in = d_in; a.ld_in = ld_in; a.out = d_out; a.ld_out = ld_out; a.scale = scale;
     lrp_arena ar(ws, ws_bytes);
-    double2* W = ar.take<double2>((size_t)g * L);
-    double* sums = ar.take<double>((size_t)g * (p.nch + 1));
-    double* part = ar.take<double>((size_t)g * p.nB * p.nch);
+    a.W = ar.take<double2>((size_t)2 * a.gc * L);
+    a.ypart = ar.take<double2>((size_t)2 * a.gc * 2 * L2);
+    a.anchors = ar.take<double>((size_t)2 * a.gc * (p.nC + 1));
+    a.counters = ar.take<int>(1 + 4 * (size_t)batch + 32);
     if (!ar.ok()) return LRP_ERR_WORKSPACE;
-    constexpr int SC_SMEM = 2 * SC_ARR * (int)sizeof(double);
-    for (int c0 = 0; c0 < batch; c0 += g) {
-        const int cols = (batch - c0) < g ? (batch - c0) : g;
-        double* o = d_out + (int64_t)c0 * ld_out;
-        LRP_TRY(dispatch_pa(p.q1, p.tla, ctx, log2N, cols, d_in + (int64_t)c0 * ld_in, ld_in, W));
-        LRP_TRY(dispatch_pb(p.q2, p.tlb, ctx, log2N, cols, W, scale, sums + p.nch, p.nch + 1, part));
-        LRP_PROF(ctx, K_DST_CHUNKSUM, 8.0 * p.nB * p.nch * cols, 0);
-        dst1_chunkreduce_kernel<<<dim3((p.nch + 127) / 128, cols), 128, 0, ctx->stream>>>(p.nch, p.nB, part, sums);
-        LRP_LAUNCHED(ctx);
-        LRP_PROF(ctx, K_DST_SCANSUMS, 0, 0);
-        dst1_scansums_kernel<<<cols, 1024, 0, ctx->stream>>>(p.nch, sums);
-        LRP_LAUNCHED(ctx);
-        LRP_PROF(ctx, K_DST_FINISH, 16.0 * N * cols, 0);
-        dst1_scanapply_kernel<<<dim3(p.nch, cols), SC_NT, SC_SMEM, ctx->stream>>>(log2N, p.q1, W, o, ld_out, sums);
-        LRP_LAUNCHED(ctx);
-    }
+    int cnt; const KernelEntry* tab = kernel_table(&cnt);
+    const KernelEntry* ke = nullptr;
+    for (int i = 0; i < cnt; ++i) if (tab[i].q1 == p.q1 && tab[i].q2 == p.q2 && tab[i].tl == p.tl) ke = &tab[i];
+    if (!ke) return LRP_ERR_UNSUPPORTED_N;
+    LRP_CUDA(ctx, cudaMemsetAsync(a.counters, 0, (1 + 4 * (size_t)batch + 32) * sizeof(int), ctx->stream));
+    const int64_t items = (int64_t)batch * (p.nA + p.nB + p.nC + 1);
+    int64_t grid = (int64_t)ctx->sm_count * (p.tl <= 12 ? 2 : 1);
+    if (grid > items) grid = items;
+#ifdef LRP_DST_STATS
+    g_dbg_counters = a.counters; g_dbg_batch = batch;
+#endif
+    LRP_PROF(ctx, K_DST_FUSED, 16.0 * (double)N * batch, 0);
+    ke->fn<<<(unsigned)grid, ke->nt, ke->smem, ctx->stream>>>(a);
+    LRP_LAUNCHED(ctx);
     return LRP_OK;
 }
