@@ -73,6 +73,11 @@ int lrp_profile_reset(lrp_ctx* ctx);
 int lrp_profile_count(void);
 int lrp_profile_get(lrp_ctx* ctx, int i, const char** name, int64_t* count, double* ms, double* bytes, double* flops);
 
+/* Measured fp64 throughput of the device in TFLOP/s: plain DFMA and the fp64 tensor pipe (DMMA, mma.sync m8n8k4) from
+ * register-only loops; a few milliseconds, synchronises.  bench.py uses the larger one as the peak of its fp64 ("alu")
+ * rooflines (the fp64 peaks are to be measured on the box).  Not on the solve path. */
+int lrp_fp64_peak(lrp_ctx* ctx, double* dfma_tflops, double* dmma_tflops);
+
 /* Workspace sizes in bytes (host-side arithmetic only; safe to call without a GPU).
  *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample)
  *                                (reading Q10); 0 when the arguments are invalid, e.g. rF + oversample + 1 > K_cap.

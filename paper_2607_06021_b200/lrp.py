@@ -27,7 +27,7 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_scross_workspace_bytes", "lrp_set_workspace", "lrp_dst1_batched", "lrp_sample_fibers",
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
-           "lrp_profile_timeline"]
+           "lrp_profile_timeline", "lrp_fp64_peak"]
 
 
 class SolveOpts(C.Structure):
@@ -89,6 +89,7 @@ def load_library():
     lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
     lib.lrp_profile_timeline.argtypes = [vp, C.c_char_p]; lib.lrp_profile_timeline.restype = C.c_int
     lib.lrp_profile_reset.argtypes = [vp]; lib.lrp_profile_reset.restype = C.c_int
+    lib.lrp_fp64_peak.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]; lib.lrp_fp64_peak.restype = C.c_int
     lib.lrp_profile_count.argtypes = []; lib.lrp_profile_count.restype = C.c_int
     lib.lrp_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(dbl),
                                     C.POINTER(dbl), C.POINTER(dbl)]
@@ -177,6 +178,12 @@ class Context:
 
     def profile_timeline(self, path: str):
         self._check(self.lib.lrp_profile_timeline(self.h, path.encode()), "lrp_profile_timeline")
+
+    def fp64_peak(self) -> dict:
+        """Measured fp64 throughput (TFLOP/s) of plain DFMA and of the fp64 tensor pipe (DMMA)."""
+        a, b = C.c_double(), C.c_double()
+        self._check(self.lib.lrp_fp64_peak(self.h, C.byref(a), C.byref(b)), "lrp_fp64_peak")
+        return {"dfma_tflops": a.value, "dmma_tflops": b.value}
 
     def profile_reset(self):
         self._check(self.lib.lrp_profile_reset(self.h), "lrp_profile_reset")
