@@ -114,7 +114,7 @@ NCU_TRAFFIC = {}
 PHASE_OF = {"dst1_small": ("dst", "hbm"), "dst1_naive": ("dst", "hbm"), "dst1_fused": ("dst", "hbm"),
             "tall_gemm_sample": ("sampling", "hbm"), "tall_gemm_plain": ("rebuild", "fp64"),
             "tall_gemm_subtract": ("qr", "fp64"), "tall_gemm_t": ("qr", "fp64"), "panel_qr": ("qr", "fp64"),
-            "panel_apply": ("qr", "fp64"), "add_block": ("qr", "fp64"), "tall_resid_gram": ("rho", "fp64"),
+            "panel_apply": ("qr", "fp64"), "add_block": ("qr", "fp64"), "conditional_refactor": ("qr", "fp64"), "tall_resid_gram": ("rho", "fp64"),
             "rho": ("rho", "latency"), "eta": ("core", "latency"), "scross_core": ("core", "latency"),
             "rownorm2": ("leverage", "hbm"), "topk_chunk": ("leverage", "hbm"), "topk_merge": ("leverage", "latency"),
             "topk": ("leverage", "hbm"), "colmask": ("leverage", "latency"), "copy_tall": ("leverage", "hbm"),

@@ -199,6 +199,30 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
                          int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
                          double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat);
 
+/* Generic function-handle Cross-DEIM (Alg. 4; "G(i,j) as a function handle") on the
+ * paper's closed-form test matrices, eq. (6), PAPER.md:264-267 (0-based i, j; square n x n, any n >= K_cap):
+ *     LRP_G_HILBERT:  H(i,j) = 1 / (1 + i + j)                        (rapid singular value decay)
+ *     LRP_G_KMATRIX:  K(i,j) = (|x_i + y_j| / 2)^5,  x_i = -1 + 2 i/(n-1),  y_j = -1 + 2 j/(n-1)   (C^4, slow decay)
+ * Same sweep loop, selection, scross, prune, stop test and final truncation as lrp_cross_deim_solve; only the fiber
+ * sampler differs and there is no transform before or after.  The initial guess of Alg. 4 is
+ * REQUIRED here: opts->d_U0, d_V0 (n x r0, any full-rank columns; used for the first selection only).
+ * Outputs: d_U, d_V (n x max_rank, ld >= n), d_S (max_rank): G ~= U diag(S) V^T with rank info->rank.  Trace and
+ * last-iterate outputs as for lrp_cross_deim_solve.  Workspace: lrp_matrix_workspace_bytes(n, r0, max_rank, oversample).
+ * Synchronous.  Errors / warning as lrp_cross_deim_solve. */
+#define LRP_G_POISSON  0
+#define LRP_G_HILBERT  1
+#define LRP_G_KMATRIX  2
+size_t lrp_matrix_workspace_bytes(int64_t n, int32_t r0, int32_t max_rank, int32_t oversample);
+int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve_opts* opts,
+                          double* d_U, int64_t ldu, double* d_S, double* d_V, int64_t ldv,
+                          lrp_solve_info* info,
+                          int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                          double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat);
+/* Fibers of a test matrix (the sampler behind lrp_cross_deim_matrix; Alg. 1 line 3):
+ *     d_C (n x nJ): column c = G(:, J[c]);   d_Rt (n x nI): column c = G(I[c], :)^T.   Either may be NULL.  Asynchronous. */
+int lrp_sample_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,
+                      double* d_C, int64_t ldc, double* d_Rt, int64_t ldr);
+
 /* Entries (U diag(S) V^T)(rows[t], cols[t]), t < count (X(i,j) = sum_k sigma_k u_k(i) v_k(j)):
  * the O(r) element access used to read a low-rank result without forming it.  All pointers device.  Asynchronous. */
 int lrp_lowrank_entries(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_U, int64_t ldu, const double* d_S,

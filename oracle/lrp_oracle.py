@@ -460,25 +460,31 @@ def _safeguard(cur: np.ndarray, safeguard, scores) -> np.ndarray:
     return cur
 
 
-def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, tol: float,
-                     max_rank: int, oversample: int = 8, max_sweeps: int = 20,
-                     safeguard=None, tol_mode: int = 0, U0=None, V0=None,
-                     replay=None) -> SolveResult:
-    """Low-rank Poisson solve of T W + W T^T = h^2 F, F = UF diag(SF) VF^T  (PAPER.md:194-196,
-    222-236) by Cross-DEIM (Alg. 4) with leverage-score selection (Alg. 3,
-    PAPER.md:105-114) and scross (Alg. 1).  Steps O3-O12 of SURVEY.md §8(c).
+@dataclass
+class CrossDeimResult:
+    U: np.ndarray          # last iterate before the final truncation (all r_k columns)
+    S: np.ndarray
+    V: np.ndarray
+    rank: int              # r of Alg. 4 lines 30-32
+    sweeps: int
+    converged: bool
+    trace: list
+    rank_capped: bool = False
 
-    replay: optional list of dicts {I, J, keepI, keepJ} (one per sweep) + key 'final_rank' on the
-    last one; then selection, union, safeguard, prune and stopping decisions are taken from it.
+
+def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, max_rank: int, oversample: int = 8,
+               max_sweeps: int = 20, safeguard=None, tol_mode: int = 0, replay=None) -> CrossDeimResult:
+    """Algorithm 4 for a matrix given as a function handle ("G(i,j) as a function
+    handle"): `fibers(I, J)` returns C = G(:, J) (n x |J|) and Rt = G(I, :)^T (n x |I|).  Leverage-score selection
+    (Alg. 3), scross (Alg. 1).  U0, V0: initial guess of Alg. 4,
+    used for the first selection only.  Steps O5-O11 of SURVEY.md 8(c); square case m = n.
+
+    replay: optional list of dicts {I, J, keepI, keepJ} (one per sweep) + key 'final_rank' on the last one; then
+    selection, union, safeguard, prune and stopping decisions are taken from it.
     """
-    scale = orthonormal_scale(n)
-    d = eigenvalues_d(n)                                     # O1
-    UhF = dst1(UF, scale)                                    # O3, PAPER.md:226
-    VhF = dst1(VF, scale)
-    SF = np.asarray(SF, dtype=np.float64)
     K_cap = 2 * (max_rank + oversample)                      # reading Q10
-    Uprev_sel = UhF if U0 is None else np.asarray(U0)        # O5 (reading Q7)
-    Vprev_sel = VhF if V0 is None else np.asarray(V0)
+    Uprev_sel = np.asarray(U0)                               # O5 (reading Q7)
+    Vprev_sel = np.asarray(V0)
     I_prev = np.zeros(0, dtype=np.int32)
     J_prev = np.zeros(0, dtype=np.int32)
     Up = Sp = Vp = None
@@ -506,7 +512,7 @@ def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, 
             scU = scV = None
             I_k = np.asarray(replay[k]["I"], dtype=np.int32)
             J_k = np.asarray(replay[k]["J"], dtype=np.int32)
-        C, Rt = sample_fibers(UhF, SF, VhF, d, I_k, J_k)     # O4
+        C, Rt = fibers(I_k, J_k)                             # O4
         res = scross(C, Rt, I_k, J_k)                        # O8
         if replay is None or replay[k].get("keepI") is None:
             keepI = res.rR >= PRUNE_REL * res.rR.max()       # O9 (rows of R <-> I)
@@ -540,11 +546,65 @@ def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, 
         r = final_rank(res.S, tol, max_rank, tol_mode)       # O11
         rank_capped = final_rank(res.S, tol, res.S.size + 1, tol_mode) > max_rank      # reading Q20: r* > r_max
     r = min(r, res.rank)
-    UW = dst1(res.U[:, :r], scale)                           # O12
-    VW = dst1(res.V[:, :r], scale)
-    return SolveResult(UW=UW, SW=res.S[:r].copy(), VW=VW, Uhat=res.U, Shat=res.S, Vhat=res.V,
-                       UhF=UhF, VhF=VhF, d=d, rank=r, sweeps=len(trace), converged=converged,
-                       trace=trace, rank_capped=rank_capped)
+    return CrossDeimResult(U=res.U, S=res.S, V=res.V, rank=r, sweeps=len(trace), converged=converged, trace=trace,
+                           rank_capped=rank_capped)
+
+
+def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, tol: float,
+                     max_rank: int, oversample: int = 8, max_sweeps: int = 20,
+                     safeguard=None, tol_mode: int = 0, U0=None, V0=None,
+                     replay=None) -> SolveResult:
+    """Low-rank Poisson solve of T W + W T^T = h^2 F, F = UF diag(SF) VF^T  (PAPER.md:194-196,
+    222-236): Cross-DEIM (`cross_deim` above) on the spectral solution G(i,j) = (Uh S Vh^T)(i,j)/(d_i + d_j) (eq. (4),
+    PAPER.md:213) between two batched DST-I.  Steps O1-O12 of SURVEY.md 8(c).
+    """
+    scale = orthonormal_scale(n)
+    d = eigenvalues_d(n)                                     # O1
+    UhF = dst1(UF, scale)                                    # O3, PAPER.md:226
+    VhF = dst1(VF, scale)
+    SF = np.asarray(SF, dtype=np.float64)
+    cd = cross_deim(n, lambda I, J: sample_fibers(UhF, SF, VhF, d, I, J),
+                    UhF if U0 is None else np.asarray(U0), VhF if V0 is None else np.asarray(V0),     # O5 (reading Q7)
+                    tol=tol, max_rank=max_rank, oversample=oversample, max_sweeps=max_sweeps, safeguard=safeguard,
+                    tol_mode=tol_mode, replay=replay)
+    r = cd.rank
+    UW = dst1(cd.U[:, :r], scale)                            # O12, PAPER.md:232-236
+    VW = dst1(cd.V[:, :r], scale)
+    return SolveResult(UW=UW, SW=cd.S[:r].copy(), VW=VW, Uhat=cd.U, Shat=cd.S, Vhat=cd.V,
+                       UhF=UhF, VhF=VhF, d=d, rank=r, sweeps=cd.sweeps, converged=cd.converged,
+                       trace=cd.trace, rank_capped=cd.rank_capped)
+
+
+# ----------------------------------------------------------------------------- test matrices (eq. (6))
+def hilbert_entries(rows, cols) -> np.ndarray:
+    """H(i,j) = 1 / (1 + i + j), 0-based i, j: the Hilbert matrix of eq. (6), PAPER.md:264-266 (rapid singular value decay)."""
+    rows = np.asarray(rows, dtype=np.float64)
+    cols = np.asarray(cols, dtype=np.float64)
+    return 1.0 / (1.0 + rows + cols)
+
+
+def kmatrix_entries(n: int, rows, cols) -> np.ndarray:
+    """K(i,j) = (|x_i + y_j| / 2)^5 on x_i = -1 + 2 i/(n-1), y_j = -1 + 2 j/(n-1), 0-based (eq. (6), PAPER.md:264-267,
+    whose grid is printed 1-based): C^4 with a kink along x + y = 0, slow singular value decay."""
+    x = -1.0 + 2.0 * np.asarray(rows, dtype=np.float64) / (n - 1)
+    y = -1.0 + 2.0 * np.asarray(cols, dtype=np.float64) / (n - 1)
+    return (np.abs(x + y) / 2.0) ** 5
+
+
+def matrix_fibers(kind: str, n: int):
+    """Function handle `fibers(I, J) -> (C, Rt)` of a test matrix of eq. (6) ('hilbert' or 'kmatrix'), square n x n."""
+    i = np.arange(n)
+
+    def entries(r, c):
+        return hilbert_entries(r, c) if kind == "hilbert" else kmatrix_entries(n, r, c)
+
+    def fibers(I, J):
+        I = np.asarray(I, dtype=np.int64)
+        J = np.asarray(J, dtype=np.int64)
+        C = entries(i[:, None], J[None, :])                  # G(:, J)
+        Rt = entries(I[None, :], i[:, None])                 # G(I, :)^T: row c of G(I,:) is column c
+        return C, Rt
+    return fibers
 
 
 def trace_to_replay(trace, final_rank_value: int | None = None) -> list:

@@ -125,9 +125,9 @@ struct SolveWs {
     void *sel_ws, *dst_ws, *dst_ws2;
     size_t eta_stride, dst_ws_bytes;
     ScrossWs sc;
-    bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank) {
+    bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank, bool poisson = true) {
         const size_t ld = (size_t)internal_ld(n);
-        UhF = ar.take<double>(ld * rF); VhF = ar.take<double>(ld * rF);
+        UhF = ar.take<double>(poisson ? ld * rF : 1); VhF = ar.take<double>(poisson ? ld * rF : 1);
         Cb = ar.take<double>(ld * Kc); Rb = ar.take<double>(ld * Kc);
         Ua = ar.take<double>(ld * Kc); Va = ar.take<double>(ld * Kc);
         Ub = ar.take<double>(ld * Kc); Vb = ar.take<double>(ld * Kc);
@@ -152,7 +152,7 @@ struct SolveWs {
         mask = ar.take<unsigned char>(Kc); mask2 = ar.take<unsigned char>(Kc);
         sel_ws = ar.take<char>(select_ws_bytes(ctx, n, 2 * Kc + 1));
         int dcols = rF > max_rank ? rF : max_rank;
-        dst_ws_bytes = lrp_dst1_ws_impl(n, dcols);
+        dst_ws_bytes = poisson ? lrp_dst1_ws_impl(n, dcols) : 0;
         dst_ws = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
         dst_ws2 = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
         bool ok = sc.carve(ar, ctx, n, Kc, Kc);
@@ -347,6 +347,16 @@ size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t over
     return ar.off + 256;
 }
 
+size_t lrp_matrix_workspace_bytes(int64_t n, int32_t r0, int32_t max_rank, int32_t oversample) {
+    if (n < 2 || r0 < 1 || max_rank < 1 || oversample < 0) return 0;
+    const int Kc = 2 * (max_rank + oversample);
+    if (Kc < r0 + oversample + 1) return 0;
+    lrp_arena ar((void*)256, (size_t)-1 / 2);
+    SolveWs w;
+    w.carve(ar, nullptr, n, r0, Kc, max_rank, false);
+    return ar.off + 256;
+}
+
 size_t lrp_leverage_workspace_bytes(int64_t n, int32_t k) {
     if (n < 1 || k < 1) return 0;
     lrp_arena ar((void*)256, (size_t)-1 / 2);
@@ -456,14 +466,22 @@ int lrp_lowrank_entries(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_U, i
     return tall_lowrank_entries(ctx, r, d_U, ldu, d_S, d_V, ldv, d_rows, d_cols, count, d_out);
 }
 
-int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF, int64_t ldu, const double* d_SF,
-                         const double* d_VF, int64_t ldv, const lrp_solve_opts* opts,
-                         double* d_UW, int64_t lduw, double* d_SW, double* d_VW, int64_t ldvw, lrp_solve_info* info,
-                         int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
-                         double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
+// The Cross-DEIM driver (Alg. 4) for a matrix given by its fiber sampler ("G(i,j) as a function handle",
+// PAPER.md:20, 68).  kind = LRP_G_POISSON: the spectral Poisson solution of eq. (4) between the two batched DST-I
+// (rF, d_UF, d_SF, d_VF = right-hand side in physical space); kind = LRP_G_HILBERT / LRP_G_KMATRIX: the closed-form test
+// matrices of eq. (6), no transforms (rF = columns of the required initial guess opts->d_U0 / d_V0; d_UF/d_SF/d_VF unused).
+static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const double* d_UF, int64_t ldu, const double* d_SF,
+                      const double* d_VF, int64_t ldv, const lrp_solve_opts* opts,
+                      double* d_UW, int64_t lduw, double* d_SW, double* d_VW, int64_t ldvw, lrp_solve_info* info,
+                      int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                      double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
     if (!ctx || !opts || !info) return LRP_ERR_BADARG;
-    LRP_TRY(check_n(n));
-    if (rF < 1 || !d_UF || !d_SF || !d_VF || !d_UW || !d_SW || !d_VW || ldu < n || ldv < n || lduw < n || ldvw < n) return LRP_ERR_BADARG;
+    const bool poisson = kind == LRP_G_POISSON;
+    if (poisson) LRP_TRY(check_n(n));
+    else if (kind != LRP_G_HILBERT && kind != LRP_G_KMATRIX) return LRP_ERR_BADARG;
+    else if (n < 2 || n > ((int64_t)1 << 30) || !opts->d_U0 || !opts->d_V0) return LRP_ERR_BADARG;
+    if (rF < 1 || !d_UW || !d_SW || !d_VW || lduw < n || ldvw < n) return LRP_ERR_BADARG;
+    if (poisson && (!d_UF || !d_SF || !d_VF || ldu < n || ldv < n)) return LRP_ERR_BADARG;
     if (opts->max_rank < 1 || opts->oversample < 0 || opts->max_sweeps < 1 || !(opts->tol > 0.0)) return LRP_ERR_BADARG;
     const int max_rank = opts->max_rank, p_os = opts->oversample;
     const int Kc = 2 * (max_rank + p_os);             // reading Q10 (the oracle's K_cap): index lists are cut there
@@ -475,10 +493,10 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     const double* U0 = opts->d_U0; const double* V0 = opts->d_V0; int r0 = opts->r0; int64_t ld0 = opts->ld0;
     if ((U0 == nullptr) != (V0 == nullptr)) return LRP_ERR_BADARG;
     if (U0 && (r0 < 1 || r0 + p_os + 1 > Kc || ld0 < n)) return LRP_ERR_BADARG;
-    if (ctx->ws_bytes < lrp_workspace_bytes(n, rF, max_rank, p_os)) return LRP_ERR_WORKSPACE;
+    if (ctx->ws_bytes < (poisson ? lrp_workspace_bytes(n, rF, max_rank, p_os) : lrp_matrix_workspace_bytes(n, rF, max_rank, p_os))) return LRP_ERR_WORKSPACE;
     lrp_arena ar(ctx->ws, ctx->ws_bytes);
     SolveWs w;
-    if (!w.carve(ar, ctx, n, rF, Kc, max_rank)) return LRP_ERR_WORKSPACE;
+    if (!w.carve(ar, ctx, n, rF, Kc, max_rank, poisson)) return LRP_ERR_WORKSPACE;
     memset(info, 0, sizeof(*info));
     const int64_t launches0 = ctx->launches;
     const int64_t ld = internal_ld(n);
@@ -488,7 +506,7 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     cudaEvent_t e_start = ep.rec(ctx);
 
     // O3: spectral RHS factors
-    {   // the two batched transforms are independent: main and auxiliary stream
+    if (poisson) {   // the two batched transforms are independent: main and auxiliary stream
         cudaStream_t dside = ctx->prof_on == 1 ? ctx->stream : ctx->aux;
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(dside, ctx->ev_fork, 0));
@@ -597,8 +615,13 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
         if (nested && nrI > 0) LRP_TRY(tall_copy(ctx, n, nrI, w.Rb + (int64_t)l0 * ld, ld, w.QrestV, ld));
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(side, ctx->ev_fork, 0));
-        if (kk > k0) LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ + k0, kk - k0, w.Cb + (int64_t)k0 * ld, ld));
-        if (l > l0) LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
+        if (poisson) {
+            if (kk > k0) LRP_TRY(sample_side(ctx, n, rF, w.UhF, ld, d_SF, w.VhF, ld, w.dJ + k0, kk - k0, w.Cb + (int64_t)k0 * ld, ld));
+            if (l > l0) LRP_ON_STREAM(ctx, side, sample_side(ctx, n, rF, w.VhF, ld, d_SF, w.UhF, ld, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
+        } else {
+            if (kk > k0) LRP_TRY(tall_matrix_fibers(ctx, kind, n, 0, w.dJ + k0, kk - k0, w.Cb + (int64_t)k0 * ld, ld));
+            if (l > l0) LRP_ON_STREAM(ctx, side, tall_matrix_fibers(ctx, kind, n, 1, w.dI + l0, l - l0, w.Rb + (int64_t)l0 * ld, ld));
+        }
         cudaEvent_t e2 = ep.rec(ctx);
         // ---- O8: scross
         cudaEvent_t e3 = ep.take();
@@ -762,7 +785,10 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     if (r > r_prev) r = r_prev;
     if (r > max_rank) r = max_rank;
     cudaEvent_t e_inv0 = ep.rec(ctx);
-    {   // O12
+    if (!poisson) {  // no transform: the truncated iterate is the result
+        LRP_TRY(tall_copy(ctx, n, r, Up, ld, d_UW, lduw));
+        LRP_TRY(tall_copy(ctx, n, r, Vp, ld, d_VW, ldvw));
+    } else {   // O12
         cudaStream_t dside = ctx->prof_on == 1 ? ctx->stream : ctx->aux;
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         LRP_CUDA(ctx, cudaStreamWaitEvent(dside, ctx->ev_fork, 0));
@@ -791,6 +817,38 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
     info->ms_total = EventPool::ms(e_start, e_end);
     info->launches = ctx->launches - launches0;
     return converged ? LRP_OK : LRP_WARN_NOCONV;
+}
+
+int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF, int64_t ldu, const double* d_SF,
+                         const double* d_VF, int64_t ldv, const lrp_solve_opts* opts,
+                         double* d_UW, int64_t lduw, double* d_SW, double* d_VW, int64_t ldvw, lrp_solve_info* info,
+                         int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                         double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
+    return solve_impl(ctx, LRP_G_POISSON, n, rF, d_UF, ldu, d_SF, d_VF, ldv, opts, d_UW, lduw, d_SW, d_VW, ldvw, info,
+                      h_trace_I, h_trace_J, h_trace_keepI, h_trace_keepJ, d_Uhat, d_Shat, d_Vhat, ld_hat);
+}
+
+int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve_opts* opts,
+                          double* d_U, int64_t ldu, double* d_S, double* d_V, int64_t ldv, lrp_solve_info* info,
+                          int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
+                          double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
+    if (!opts || kind == LRP_G_POISSON) return LRP_ERR_BADARG;
+    return solve_impl(ctx, kind, n, opts->r0, nullptr, 0, nullptr, nullptr, 0, opts, d_U, ldu, d_S, d_V, ldv, info,
+                      h_trace_I, h_trace_J, h_trace_keepI, h_trace_keepJ, d_Uhat, d_Shat, d_Vhat, ld_hat);
+}
+
+int lrp_sample_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,
+                      double* d_C, int64_t ldc, double* d_Rt, int64_t ldr) {
+    if (!ctx || n < 2 || (kind != LRP_G_HILBERT && kind != LRP_G_KMATRIX) || nI < 0 || nJ < 0) return LRP_ERR_BADARG;
+    if (d_C && nJ > 0) {
+        if (!d_J || ldc < n) return LRP_ERR_BADARG;
+        LRP_TRY(tall_matrix_fibers(ctx, kind, n, 0, d_J, nJ, d_C, ldc));
+    }
+    if (d_Rt && nI > 0) {
+        if (!d_I || ldr < n) return LRP_ERR_BADARG;
+        LRP_TRY(tall_matrix_fibers(ctx, kind, n, 1, d_I, nI, d_Rt, ldr));
+    }
+    return LRP_OK;
 }
 
 }  // extern "C"

@@ -49,7 +49,36 @@ __global__ void copy_tall_kernel(int64_t n, int k, const double* __restrict__ A,
     for (int c = blockIdx.y; c < k; c += gridDim.y) B[i + (int64_t)c * ldb] = A[i + (int64_t)c * lda];
 }
 
+// Fibers of the test matrices of eq. (6), PAPER.md:264-267 (0-based i, j; square n x n):
+//   kind 1 (Hilbert):  G(i,j) = 1 / (1 + i + j)
+//   kind 2 (K):        G(i,j) = (|x_i + y_j| / 2)^5,  x_i = -1 + 2 i/(n-1),  y_j = -1 + 2 j/(n-1)
+// transposed = 0: Out(i, c) = G(i, idx[c]) (columns, C = G(:,J));  transposed = 1: Out(j, c) = G(idx[c], j) (rows, G(I,:)^T)
+__device__ __forceinline__ double matrix_entry(int kind, int64_t n, int64_t i, int64_t j) {
+    if (kind == 1) return 1.0 / (1.0 + (double)i + (double)j);
+    const double x = -1.0 + 2.0 * (double)i / (double)(n - 1), y = -1.0 + 2.0 * (double)j / (double)(n - 1);
+    const double t = fabs(x + y) / 2.0, t2 = t * t;
+    return t2 * t2 * t;
+}
+__global__ void matrix_fibers_kernel(int kind, int64_t n, int transposed, const int32_t* __restrict__ idx, int nidx,
+                                     double* __restrict__ Out, int64_t ldo) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    for (int c = blockIdx.y; c < nidx; c += gridDim.y) {
+        const int64_t f = idx[c];
+        Out[i + (int64_t)c * ldo] = transposed ? matrix_entry(kind, n, f, i) : matrix_entry(kind, n, i, f);
+    }
+}
+
 }  // namespace
+
+int tall_matrix_fibers(lrp_ctx* ctx, int kind, int64_t n, int transposed, const int32_t* idx, int nidx, double* Out, int64_t ldo) {
+    if (nidx <= 0) return LRP_OK;
+    dim3 grid((unsigned)((n + 255) / 256), nidx < 64 ? nidx : 64);
+    LRP_PROF(ctx, K_GEMM_SAMPLE, 8.0 * n * nidx, 6.0 * n * nidx);
+    matrix_fibers_kernel<<<grid, 256, 0, ctx->stream>>>(kind, n, transposed, idx, nidx, Out, ldo);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
 
 int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, const unsigned char* colmask, double* out) {
     LRP_PROF(ctx, K_ROWNORM, 8.0 * n * (k + 1), 2.0 * n * k);

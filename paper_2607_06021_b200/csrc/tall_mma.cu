@@ -417,8 +417,9 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
     const int64_t resident = (int64_t)lrp_sm_count(ctx) * (nj == 2 ? 5 : (nj <= 4 ? 4 : 3));   // persistent over row slabs (B staged once per column tile per CTA):
     if (grid > resident) grid = resident;            // exactly one resident wave, so that the slabs are balanced
-    LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
-             8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
+    if (p.cond) LRP_PROF(ctx, K_COND, 0, 0);             // device-side conditional launch: normally a no-op, no work accounted
+    else LRP_PROF(ctx, p.mode == TG_SAMPLE ? K_GEMM_SAMPLE : (p.mode == TG_SUBTRACT ? K_GEMM_SUBTRACT : K_GEMM_PLAIN),
+                  8.0 * p.n * (p.k + p.m + (p.mode == TG_SUBTRACT ? p.m : 0)), 2.0 * p.n * p.k * p.m);
     kern<<<(unsigned)grid, MG_THREADS, smem, ctx->stream>>>(p);
     LRP_LAUNCHED(ctx);
     return LRP_OK;
@@ -459,7 +460,7 @@ int tall_gemm_t(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, co
     // one counter set per library stream: launches on a stream are ordered, the counters are back at zero when a launch ends
     const int slot = ctx->stream == ctx->aux ? 1 : (ctx->stream == ctx->aux2 ? 2 : 0);
     o.counters = ctx->d_counters + slot * (GT_MAXGRP + 1);
-    LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
+    if (cond) LRP_PROF(ctx, K_COND, 0, 0); else LRP_PROF(ctx, K_GEMM_T, 8.0 * n * (k + m), 2.0 * n * k * m);
     const bool vec = (lda % 2 == 0) && (ldb % 2 == 0) && (((uintptr_t)A | (uintptr_t)B) & 15u) == 0;
     if (vec) tall_gemm_t_mma_kernel<true><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);
     else tall_gemm_t_mma_kernel<false><<<grid, MT_THREADS, 0, ctx->stream>>>(A, lda, k, B, ldb, m, n, rows_per, partial_ws, na, nb, ntc, o);

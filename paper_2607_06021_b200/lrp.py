@@ -21,13 +21,16 @@ LIB_PATH = os.path.join(_HERE, "liblrp.so")
 LRP_OK, LRP_ERR_BADARG, LRP_ERR_UNSUPPORTED_N, LRP_ERR_WORKSPACE, LRP_ERR_CUDA, LRP_WARN_NOCONV = 0, -1, -2, -3, -4, 1
 MAX_SWEEPS_INFO = 32
 LRP_FLAG_NO_QR_REUSE, LRP_FLAG_NO_NESTED_RHO, LRP_FLAG_NO_FUSED_RHO = 1, 2, 4
+LRP_G_POISSON, LRP_G_HILBERT, LRP_G_KMATRIX = 0, 1, 2
+MATRIX_KINDS = {"hilbert": LRP_G_HILBERT, "kmatrix": LRP_G_KMATRIX}
 
 EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "lrp_launch_count",
            "lrp_workspace_bytes", "lrp_dst1_workspace_bytes", "lrp_leverage_workspace_bytes",
            "lrp_scross_workspace_bytes", "lrp_set_workspace", "lrp_dst1_batched", "lrp_sample_fibers",
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
-           "lrp_profile_timeline", "lrp_fp64_peak"]
+           "lrp_profile_timeline", "lrp_fp64_peak", "lrp_matrix_workspace_bytes", "lrp_cross_deim_matrix",
+           "lrp_sample_matrix"]
 
 
 class SolveOpts(C.Structure):
@@ -84,6 +87,11 @@ def load_library():
     lib.lrp_cross_deim_solve.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64,
                                          C.POINTER(SolveInfo), vp, vp, vp, vp, vp, vp, vp, i64]
     lib.lrp_cross_deim_solve.restype = C.c_int
+    lib.lrp_matrix_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_matrix_workspace_bytes.restype = sz
+    lib.lrp_cross_deim_matrix.argtypes = [vp, i32, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64, C.POINTER(SolveInfo),
+                                          vp, vp, vp, vp, vp, vp, vp, i64]
+    lib.lrp_cross_deim_matrix.restype = C.c_int
+    lib.lrp_sample_matrix.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, i64, vp, i64]; lib.lrp_sample_matrix.restype = C.c_int
     lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_lowrank_entries.restype = C.c_int
     lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
@@ -262,16 +270,10 @@ class Context:
         r = rank.value
         return dict(U=U[:r], S=S[:r], V=V[:r], S_full=S, rC=rC, rR=rR, rank=r, smin_full=smin.value)
 
-    def cross_deim_solve(self, UF, SF, VF, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False, flags=0):
-        """Low-rank Poisson solve.  UF, VF: tall tensors (rF, n) in physical space, SF: (rF,) CUDA tensor.
-        replay: list of dicts {I, J, keepI, keepJ} (numpy) + optional 'final_rank' on the last one."""
+    def _run_solve(self, n, dev, Kc, max_rank, call, *, tol, oversample, max_sweeps, safeguard, tol_mode, U0, V0, replay,
+                   want_spectral, flags):
+        """Marshals lrp_solve_opts / lrp_solve_info / trace buffers and runs `call(opts, outputs...)`."""
         torch = _torch()
-        rF, n, ldu = _check_tall(UF, "UF")
-        _, _, ldv = _check_tall(VF, "VF")
-        dev = UF.device
-        Kc = 2 * (max_rank + oversample)
-        self.ensure_workspace(self.lib.lrp_workspace_bytes(n, rF, max_rank, oversample))
         # outputs: only the first info.rank columns are defined (and returned); no fill kernels on the solve's path
         UW = torch.empty((max_rank, n), dtype=torch.float64, device=dev)
         VW = torch.empty((max_rank, n), dtype=torch.float64, device=dev)
@@ -308,10 +310,7 @@ class Context:
             Uhat = torch.empty((Kc, n), dtype=torch.float64, device=dev)
             Vhat = torch.empty((Kc, n), dtype=torch.float64, device=dev)
             Shat = torch.empty(Kc, dtype=torch.float64, device=dev)
-        rc = self._check(self.lib.lrp_cross_deim_solve(
-            self.h, n, rF, _ptr(UF), ldu, _ptr(SF), _ptr(VF), ldv, C.byref(o), _ptr(UW), n, _ptr(SW), _ptr(VW), n,
-            C.byref(info), trI.ctypes.data, trJ.ctypes.data, tkI.ctypes.data, tkJ.ctypes.data,
-            _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_solve")
+        rc = call(o, UW, SW, VW, info, trI, trJ, tkI, tkJ, Uhat, Shat, Vhat)
         del keep
         sweeps, r = info.sweeps, info.rank
         trace, oi, oj = [], 0, 0
@@ -327,6 +326,53 @@ class Context:
             rk = info.rank_per_sweep[sweeps - 1]
             res.update(Uhat=Uhat[:rk], Shat=Shat[:rk], Vhat=Vhat[:rk])
         return res
+
+    def cross_deim_solve(self, UF, SF, VF, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
+                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False, flags=0):
+        """Low-rank Poisson solve.  UF, VF: tall tensors (rF, n) in physical space, SF: (rF,) CUDA tensor.
+        replay: list of dicts {I, J, keepI, keepJ} (numpy) + optional 'final_rank' on the last one."""
+        rF, n, ldu = _check_tall(UF, "UF")
+        _, _, ldv = _check_tall(VF, "VF")
+        self.ensure_workspace(self.lib.lrp_workspace_bytes(n, rF, max_rank, oversample))
+
+        def call(o, UW, SW, VW, info, trI, trJ, tkI, tkJ, Uhat, Shat, Vhat):
+            return self._check(self.lib.lrp_cross_deim_solve(
+                self.h, n, rF, _ptr(UF), ldu, _ptr(SF), _ptr(VF), ldv, C.byref(o), _ptr(UW), n, _ptr(SW), _ptr(VW), n,
+                C.byref(info), trI.ctypes.data, trJ.ctypes.data, tkI.ctypes.data, tkJ.ctypes.data,
+                _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_solve")
+        return self._run_solve(n, UF.device, 2 * (max_rank + oversample), max_rank, call, tol=tol, oversample=oversample,
+                               max_sweeps=max_sweeps, safeguard=safeguard, tol_mode=tol_mode, U0=U0, V0=V0, replay=replay,
+                               want_spectral=want_spectral, flags=flags)
+
+    def cross_deim_matrix(self, kind, n, U0, V0, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
+                          tol_mode=0, replay=None, want_spectral=False, flags=0):
+        """Cross-DEIM on a closed-form test matrix of eq. (6) (kind 'hilbert' or 'kmatrix', n x n).  U0, V0: tall tensors
+        (r0, n), the initial guess of Alg. 4.  Returns the same dictionary as cross_deim_solve (UW, SW, VW = the factors)."""
+        k = MATRIX_KINDS[kind] if isinstance(kind, str) else int(kind)
+        r0, n0, _ = _check_tall(U0, "U0")
+        if n0 != n:
+            raise ValueError("U0 must have n rows")
+        self.ensure_workspace(self.lib.lrp_matrix_workspace_bytes(n, r0, max_rank, oversample))
+
+        def call(o, UW, SW, VW, info, trI, trJ, tkI, tkJ, Uhat, Shat, Vhat):
+            return self._check(self.lib.lrp_cross_deim_matrix(
+                self.h, k, n, C.byref(o), _ptr(UW), n, _ptr(SW), _ptr(VW), n, C.byref(info),
+                trI.ctypes.data, trJ.ctypes.data, tkI.ctypes.data, tkJ.ctypes.data,
+                _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_matrix")
+        return self._run_solve(n, U0.device, 2 * (max_rank + oversample), max_rank, call, tol=tol, oversample=oversample,
+                               max_sweeps=max_sweeps, safeguard=safeguard, tol_mode=tol_mode, U0=U0, V0=V0, replay=replay,
+                               want_spectral=want_spectral, flags=flags)
+
+    def sample_matrix(self, kind, n, I=None, J=None):
+        """Fibers of a test matrix: C = G(:, J) as (|J|, n), Rt = G(I, :)^T as (|I|, n)."""
+        torch = _torch()
+        k = MATRIX_KINDS[kind] if isinstance(kind, str) else int(kind)
+        Cm = torch.empty((J.numel(), n), dtype=torch.float64, device=self.device) if J is not None else None
+        Rt = torch.empty((I.numel(), n), dtype=torch.float64, device=self.device) if I is not None else None
+        self._check(self.lib.lrp_sample_matrix(self.h, k, n, _ptr(I), I.numel() if I is not None else 0,
+                                               _ptr(J), J.numel() if J is not None else 0, _ptr(Cm), n, _ptr(Rt), n),
+                    "lrp_sample_matrix")
+        return Cm, Rt
 
     def lowrank_entries(self, U, S, V, rows, cols):
         torch = _torch()

@@ -165,3 +165,14 @@ def sample_pairs(n: int, count: int, seed: int = 0, active: int | None = None):
         i[:h] = rng.integers(0, a, h)
         j[:h] = rng.integers(0, a, h)
     return i.astype(np.int64), j.astype(np.int64)
+
+
+def matrix_initial_guess(n: int, r0: int = 4, seed: int = 0):
+    """Initial guess U0, V0 (n x r0, orthonormal columns) and safeguard list for Cross-DEIM on the paper's test matrices
+    (eq. (6)): the paper does not say what Alg. 4's U0, V0 are there; seeded Gaussian columns,
+    orthonormalised on the host, are handed to both the CUDA path and the oracle as data."""
+    rng = np.random.default_rng(seed + 4242)
+    U0, _ = np.linalg.qr(rng.standard_normal((n, r0)))
+    V0, _ = np.linalg.qr(rng.standard_normal((n, r0)))
+    safeguard = rng.integers(0, n, SAFEGUARD_LEN).astype(np.int32)
+    return _fortran(U0), _fortran(V0), safeguard
