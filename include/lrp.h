@@ -158,7 +158,21 @@ typedef struct lrp_solve_opts {
     const uint8_t* h_replay_keepJ;
     int32_t replay_final_rank;      /* > 0: use this final rank */
     int32_t flags;                  /* bit mask of LRP_FLAG_* below; 0 = default path */
+    int32_t selection;              /* LRP_SELECT_TOPK (default), LRP_SELECT_BERNOULLI, LRP_SELECT_QDEIM, LRP_SELECT_DEIM */
+    uint64_t ls_seed;               /* LRP_SELECT_BERNOULLI: seed of the counter-based uniforms */
+    double  ls_c;                   /* LRP_SELECT_BERNOULLI: the constant c of Alg. 3 line 4; <= 0: cols + oversample */
 } lrp_solve_opts;
+
+/* lrp_solve_opts.selection: how the index sets are enriched each sweep (Alg. 4 line 5)
+ *   TOPK      leverage scores, the (cols + oversample) largest (deterministic form of Alg. 3, reading Q5)
+ *   BERNOULLI leverage scores as printed (Alg. 3 lines 4-5): keep i with probability
+ *             min{1, c pi_i}, pi_i = l_i / cols; u_i from a counter-based generator keyed by (ls_seed, sweep, side, i)
+ *   QDEIM     column-pivoted QR of U^T (Alg. 2 lines 7-10): cols indices
+ *   DEIM      pivoted LU of U (Alg. 2 lines 3-6): cols indices */
+#define LRP_SELECT_TOPK       0
+#define LRP_SELECT_BERNOULLI  1
+#define LRP_SELECT_QDEIM      2
+#define LRP_SELECT_DEIM       3
 
 /* lrp_solve_opts.flags: switch one of the driver's shortcuts off (comparison runs of the tests; results agree to rounding) */
 #define LRP_FLAG_NO_QR_REUSE    1   /* factor every fiber block from scratch (reading R4 off) */

@@ -297,6 +297,36 @@ def leverage_select(A: np.ndarray, num_select: int, assume_orthonormal: bool = F
     return top_select(sc, num_select), sc
 
 
+# ----------------------------------------------------------------------------- Alg. 3 lines 4-5, randomized form
+_M64 = (1 << 64) - 1
+
+
+def counter_uniforms(seed: int, sweep: int, side: int, n: int) -> np.ndarray:
+    """u_i in [0, 1), i = 0..n-1: a counter-based generator (SplitMix64 finaliser of a key built from seed, sweep, side
+    and i), so that the CUDA path and this oracle draw the SAME numbers without sharing code or state (the paper's
+    randomness is not reproducible across devices):
+        x = seed + 0x9E3779B97F4A7C15 (1 + 2 sweep + side);   z = x + 0xD1B54A32D192ED03 (i + 1)        (mod 2^64)
+        z = (z xor z>>30) 0xBF58476D1CE4E5B9;  z = (z xor z>>27) 0x94D049BB133111EB;  z = z xor z>>31
+        u = (z >> 11) 2^-53."""
+    x = (int(seed) + 0x9E3779B97F4A7C15 * (1 + 2 * int(sweep) + int(side))) & _M64
+    with np.errstate(over="ignore"):
+        z = np.uint64(x) + np.uint64(0xD1B54A32D192ED03) * (np.arange(n, dtype=np.uint64) + np.uint64(1))
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * 2.0 ** -53
+
+
+def bernoulli_select(scores: np.ndarray, cols: int, c: float, u: np.ndarray, cap: int) -> np.ndarray:
+    """Alg. 3 lines 3-6 as printed: pi_i = scores_i / cols (the 1/k-normalised leverage, sum = 1),
+    keep index i with probability p_i = min{1, c pi_i}: i is kept iff u_i < p_i.  The kept indices are returned in
+    (score desc, index asc) order (reading Q8), at most `cap` of them (the best-scoring ones)."""
+    p = np.minimum(1.0, c * (scores / cols))
+    kept = np.nonzero(u < p)[0]
+    order = np.lexsort((kept, -scores[kept]))
+    return kept[order][:cap].astype(np.int32)
+
+
 # ----------------------------------------------------------------------------- O8 scross
 @dataclass
 class ScrossResult:
@@ -473,7 +503,8 @@ class CrossDeimResult:
 
 
 def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, max_rank: int, oversample: int = 8,
-               max_sweeps: int = 20, safeguard=None, tol_mode: int = 0, replay=None) -> CrossDeimResult:
+               max_sweeps: int = 20, safeguard=None, tol_mode: int = 0, replay=None,
+               selection: str = "topk", ls_seed: int = 0, ls_c: float = 0.0) -> CrossDeimResult:
     """Algorithm 4 for a matrix given as a function handle ("G(i,j) as a function
     handle"): `fibers(I, J)` returns C = G(:, J) (n x |J|) and Rt = G(I, :)^T (n x |I|).  Leverage-score selection
     (Alg. 3), scross (Alg. 1).  U0, V0: initial guess of Alg. 4,
@@ -481,6 +512,9 @@ def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, ma
 
     replay: optional list of dicts {I, J, keepI, keepJ} (one per sweep) + key 'final_rank' on the last one; then
     selection, union, safeguard, prune and stopping decisions are taken from it.
+    selection: "topk" = the deterministic top-(cols + p_os) form (reading Q5); "bernoulli" = Alg. 3 lines 4-5 as printed,
+    with c = ls_c if ls_c > 0 else cols + p_os (expected sample size <= the deterministic form's count) and uniforms
+    from `counter_uniforms(ls_seed, sweep, side, n)` (side 0: rows / U, side 1: columns / V).
     """
     K_cap = 2 * (max_rank + oversample)                      # reading Q10
     Uprev_sel = np.asarray(U0)                               # O5 (reading Q7)
@@ -497,8 +531,16 @@ def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, ma
             # O6: selection. k = 0 (user factors) needs the QR; later iterates are orthonormal
             # up to rounding, for which the QR is the identity (reading Q6) -- the oracle still
             # performs it, as the definition.
-            Istar, scU = leverage_select(Uprev_sel, min(Uprev_sel.shape[1] + oversample, n))
-            Jstar, scV = leverage_select(Vprev_sel, min(Vprev_sel.shape[1] + oversample, n))
+            if selection == "bernoulli":
+                scU = leverage_scores(Uprev_sel)
+                scV = leverage_scores(Vprev_sel)
+                cU = ls_c if ls_c > 0 else float(Uprev_sel.shape[1] + oversample)
+                cV = ls_c if ls_c > 0 else float(Vprev_sel.shape[1] + oversample)
+                Istar = bernoulli_select(scU, Uprev_sel.shape[1], cU, counter_uniforms(ls_seed, k, 0, n), 2 * K_cap)
+                Jstar = bernoulli_select(scV, Vprev_sel.shape[1], cV, counter_uniforms(ls_seed, k, 1, n), 2 * K_cap)
+            else:
+                Istar, scU = leverage_select(Uprev_sel, min(Uprev_sel.shape[1] + oversample, n))
+                Jstar, scV = leverage_select(Vprev_sel, min(Vprev_sel.shape[1] + oversample, n))
             I_k, addedI = _union(I_prev, Istar)              # O7
             J_k, addedJ = _union(J_prev, Jstar)
             if addedI == 0 or k == 0:
@@ -553,7 +595,7 @@ def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, ma
 def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, tol: float,
                      max_rank: int, oversample: int = 8, max_sweeps: int = 20,
                      safeguard=None, tol_mode: int = 0, U0=None, V0=None,
-                     replay=None) -> SolveResult:
+                     replay=None, selection: str = "topk", ls_seed: int = 0, ls_c: float = 0.0) -> SolveResult:
     """Low-rank Poisson solve of T W + W T^T = h^2 F, F = UF diag(SF) VF^T  (PAPER.md:194-196,
     222-236): Cross-DEIM (`cross_deim` above) on the spectral solution G(i,j) = (Uh S Vh^T)(i,j)/(d_i + d_j) (eq. (4),
     PAPER.md:213) between two batched DST-I.  Steps O1-O12 of SURVEY.md 8(c).
@@ -566,7 +608,7 @@ def cross_deim_solve(n: int, UF: np.ndarray, SF: np.ndarray, VF: np.ndarray, *, 
     cd = cross_deim(n, lambda I, J: sample_fibers(UhF, SF, VhF, d, I, J),
                     UhF if U0 is None else np.asarray(U0), VhF if V0 is None else np.asarray(V0),     # O5 (reading Q7)
                     tol=tol, max_rank=max_rank, oversample=oversample, max_sweeps=max_sweeps, safeguard=safeguard,
-                    tol_mode=tol_mode, replay=replay)
+                    tol_mode=tol_mode, replay=replay, selection=selection, ls_seed=ls_seed, ls_c=ls_c)
     r = cd.rank
     UW = dst1(cd.U[:, :r], scale)                            # O12
     VW = dst1(cd.V[:, :r], scale)

@@ -237,7 +237,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     // one-time kernel attributes (dynamic shared memory opt-in): not on the per-call path
-    if (tall_qr_init(c) != LRP_OK || lrp_dst1_init(c) != LRP_OK) { lrp_destroy(c); return LRP_ERR_CUDA; }
+    if (tall_qr_init(c) != LRP_OK || lrp_dst1_init(c) != LRP_OK || select_init(c) != LRP_OK) { lrp_destroy(c); return LRP_ERR_CUDA; }
     *out = c;
     return LRP_OK;
 }
@@ -483,6 +483,7 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
     if (rF < 1 || !d_UW || !d_SW || !d_VW || lduw < n || ldvw < n) return LRP_ERR_BADARG;
     if (poisson && (!d_UF || !d_SF || !d_VF || ldu < n || ldv < n)) return LRP_ERR_BADARG;
     if (opts->max_rank < 1 || opts->oversample < 0 || opts->max_sweeps < 1 || !(opts->tol > 0.0)) return LRP_ERR_BADARG;
+    if (opts->selection < LRP_SELECT_TOPK || opts->selection > LRP_SELECT_DEIM) return LRP_ERR_BADARG;
     const int max_rank = opts->max_rank, p_os = opts->oversample;
     const int Kc = 2 * (max_rank + p_os);             // reading Q10 (the oracle's K_cap): index lists are cut there
     if (Kc < rF + p_os + 1) return LRP_ERR_BADARG;    // the first sweep's selection (rF + p_os indices + safeguard) must fit
@@ -560,12 +561,28 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
                 const std::vector<int32_t>& prev = side == 0 ? I_prev : J_prev;
                 double* sc = side == 0 ? w.scoresU : w.scoresV;
                 int32_t* dstar = side == 0 ? w.dIstar : w.dJstar;
-                LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
-                LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
-                LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                int nstar = numsel;
+                if (opts->selection == LRP_SELECT_BERNOULLI) {   // Alg. 3 lines 4-5 as printed, reading Q23
+                    SelectBernoulli b{};
+                    b.cols = sel_cols; b.c = opts->ls_c > 0.0 ? opts->ls_c : (double)(sel_cols + p_os);
+                    b.seed = opts->ls_seed; b.sweep = k; b.side = side;
+                    int64_t cap64 = 2 * (int64_t)Kc; if (cap64 > n) cap64 = n;
+                    const int cap = (int)cap64;
+                    int32_t* d_count = dstar + 2 * (size_t)Kc + 4;
+                    int32_t h_count = 0;
+                    LRP_TRY(select_topk(ctx, n, sc, cap, dstar, w.sel_ws, &b, d_count));
+                    LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * cap, cudaMemcpyDeviceToHost, ctx->stream));
+                    LRP_CUDA(ctx, cudaMemcpyAsync(&h_count, d_count, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+                    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                    nstar = h_count < cap ? h_count : cap;
+                } else {
+                    LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
+                    LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                }
                 cur = prev;
                 int added = 0;
-                host_union(cur, hstar.data(), numsel, &added);
+                host_union(cur, hstar.data(), nstar, &added);
                 if (added == 0 || k == 0) {       // Alg. 4 lines 7-12, reading Q9
                     bool done = false;
                     for (int s = 0; s < opts->n_safeguard && opts->h_safeguard; ++s) {

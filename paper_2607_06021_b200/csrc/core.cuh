@@ -62,6 +62,12 @@ int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const R
 
 int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double rcond, unsigned char* mask);
 
-// top-`num` of scores[0..n) ordered by (score desc, index asc) -> idx_out (device).  ws: select_ws_bytes(ctx, n, num).
+// top-`num` (<= 4096) of scores[0..n) ordered by (score desc, index asc) -> idx_out (device; -1 where fewer exist).
+// ws: select_ws_bytes(ctx, n, num).  bern != nullptr: only the indices kept by the Bernoulli draw of Alg. 3 lines 4-5
+// (u_i < min(1, c score_i / cols), u from the counter-based generator of select.cu) take part; *d_count (device) receives
+// how many were kept.
+struct SelectBernoulli { int cols; double c; unsigned long long seed; int sweep; int side; };
 size_t select_ws_bytes(const lrp_ctx* ctx, int64_t n, int num);
-int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t* idx_out, void* ws);
+int select_init(lrp_ctx* ctx);
+int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t* idx_out, void* ws,
+                const SelectBernoulli* bern = nullptr, int* d_count = nullptr);

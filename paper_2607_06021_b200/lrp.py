@@ -22,6 +22,7 @@ LRP_OK, LRP_ERR_BADARG, LRP_ERR_UNSUPPORTED_N, LRP_ERR_WORKSPACE, LRP_ERR_CUDA, 
 MAX_SWEEPS_INFO = 32
 LRP_FLAG_NO_QR_REUSE, LRP_FLAG_NO_NESTED_RHO, LRP_FLAG_NO_FUSED_RHO = 1, 2, 4
 LRP_G_POISSON, LRP_G_HILBERT, LRP_G_KMATRIX = 0, 1, 2
+SELECTIONS = {"topk": 0, "bernoulli": 1, "qdeim": 2, "deim": 3}
 MATRIX_KINDS = {"hilbert": LRP_G_HILBERT, "kmatrix": LRP_G_KMATRIX}
 
 EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "lrp_launch_count",
@@ -39,7 +40,8 @@ class SolveOpts(C.Structure):
                 ("d_U0", C.c_void_p), ("d_V0", C.c_void_p), ("ld0", C.c_int64), ("r0", C.c_int32),
                 ("replay_sweeps", C.c_int32), ("h_replay_nI", C.c_void_p), ("h_replay_nJ", C.c_void_p),
                 ("h_replay_I", C.c_void_p), ("h_replay_J", C.c_void_p), ("h_replay_keepI", C.c_void_p),
-                ("h_replay_keepJ", C.c_void_p), ("replay_final_rank", C.c_int32), ("flags", C.c_int32)]
+                ("h_replay_keepJ", C.c_void_p), ("replay_final_rank", C.c_int32), ("flags", C.c_int32),
+                ("selection", C.c_int32), ("ls_seed", C.c_uint64), ("ls_c", C.c_double)]
 
 
 class SolveInfo(C.Structure):
@@ -271,7 +273,7 @@ class Context:
         return dict(U=U[:r], S=S[:r], V=V[:r], S_full=S, rC=rC, rR=rR, rank=r, smin_full=smin.value)
 
     def _run_solve(self, n, dev, Kc, max_rank, call, *, tol, oversample, max_sweeps, safeguard, tol_mode, U0, V0, replay,
-                   want_spectral, flags):
+                   want_spectral, flags, selection="topk", ls_seed=0, ls_c=0.0):
         """Marshals lrp_solve_opts / lrp_solve_info / trace buffers and runs `call(opts, outputs...)`."""
         torch = _torch()
         # outputs: only the first info.rank columns are defined (and returned); no fill kernels on the solve's path
@@ -281,6 +283,8 @@ class Context:
         o = SolveOpts()
         o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
         o.flags = int(flags)
+        o.selection = SELECTIONS[selection] if isinstance(selection, str) else int(selection)
+        o.ls_seed, o.ls_c = int(ls_seed), float(ls_c)
         keep = []
         if safeguard is not None:
             sg = np.ascontiguousarray(safeguard, dtype=np.int32); keep.append(sg)
@@ -328,7 +332,8 @@ class Context:
         return res
 
     def cross_deim_solve(self, UF, SF, VF, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False, flags=0):
+                         tol_mode=0, U0=None, V0=None, replay=None, want_spectral=False, flags=0, selection="topk", ls_seed=0,
+                         ls_c=0.0):
         """Low-rank Poisson solve.  UF, VF: tall tensors (rF, n) in physical space, SF: (rF,) CUDA tensor.
         replay: list of dicts {I, J, keepI, keepJ} (numpy) + optional 'final_rank' on the last one."""
         rF, n, ldu = _check_tall(UF, "UF")
@@ -342,10 +347,10 @@ class Context:
                 _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_solve")
         return self._run_solve(n, UF.device, 2 * (max_rank + oversample), max_rank, call, tol=tol, oversample=oversample,
                                max_sweeps=max_sweeps, safeguard=safeguard, tol_mode=tol_mode, U0=U0, V0=V0, replay=replay,
-                               want_spectral=want_spectral, flags=flags)
+                               want_spectral=want_spectral, flags=flags, selection=selection, ls_seed=ls_seed, ls_c=ls_c)
 
     def cross_deim_matrix(self, kind, n, U0, V0, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                          tol_mode=0, replay=None, want_spectral=False, flags=0):
+                          tol_mode=0, replay=None, want_spectral=False, flags=0, selection="topk", ls_seed=0, ls_c=0.0):
         """Cross-DEIM on a closed-form test matrix of eq. (6) (kind 'hilbert' or 'kmatrix', n x n).  U0, V0: tall tensors
         (r0, n), the initial guess of Alg. 4.  Returns the same dictionary as cross_deim_solve (UW, SW, VW = the factors)."""
         k = MATRIX_KINDS[kind] if isinstance(kind, str) else int(kind)
@@ -361,7 +366,7 @@ class Context:
                 _ptr(Uhat), _ptr(Shat), _ptr(Vhat), n), "lrp_cross_deim_matrix")
         return self._run_solve(n, U0.device, 2 * (max_rank + oversample), max_rank, call, tol=tol, oversample=oversample,
                                max_sweeps=max_sweeps, safeguard=safeguard, tol_mode=tol_mode, U0=U0, V0=V0, replay=replay,
-                               want_spectral=want_spectral, flags=flags)
+                               want_spectral=want_spectral, flags=flags, selection=selection, ls_seed=ls_seed, ls_c=ls_c)
 
     def sample_matrix(self, kind, n, I=None, J=None):
         """Fibers of a test matrix: C = G(:, J) as (|J|, n), Rt = G(I, :)^T as (|I|, n)."""

@@ -139,3 +139,71 @@ def test_rank_cap_is_reported():
     assert capped.rank == 3 and capped.rank_capped
     # the kept singular values are the leading ones of a converged iterate
     assert np.abs(capped.SW - free.SW[:3]).max() < 1e-6 * free.SW[0]
+
+
+# ---------------------------------------------------------------------------------------------- Alg. 3 lines 4-5 (Bernoulli)
+def test_counter_uniforms_are_uniform_and_keyed():
+    """The generator is a pure function of (seed, sweep, side, i): reproducible, different for different keys, and
+    statistically uniform on [0, 1) (moments, a Kolmogorov-Smirnov distance, lag-1 correlation, bit balance)."""
+    n = 200000
+    u = O.counter_uniforms(5, 3, 1, n)
+    assert np.array_equal(u, O.counter_uniforms(5, 3, 1, n))
+    assert np.array_equal(u[:1000], O.counter_uniforms(5, 3, 1, 1000))          # entry i does not depend on n
+    for other in (O.counter_uniforms(6, 3, 1, n), O.counter_uniforms(5, 4, 1, n), O.counter_uniforms(5, 3, 0, n)):
+        assert np.mean(other == u) < 1e-3
+    assert u.min() >= 0.0 and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 4 / np.sqrt(12 * n) and abs(u.var() - 1 / 12) < 1e-3
+    ks = np.abs(np.sort(u) - (np.arange(n) + 0.5) / n).max()
+    assert ks < 2.0 / np.sqrt(n)
+    assert abs(np.corrcoef(u[:-1], u[1:])[0, 1]) < 4 / np.sqrt(n)
+    bits = (u * 2.0 ** 53).astype(np.uint64)
+    for b in (0, 1, 17, 40, 52):
+        assert abs(np.mean((bits >> np.uint64(b)) & np.uint64(1)) - 0.5) < 4 / np.sqrt(4 * n)
+
+
+def test_bernoulli_select_by_hand():
+    scores = np.array([0.5, 0.0, 1.0, 0.25, 0.25])             # cols = 2: pi = scores / 2
+    # c = 2: p = min(1, scores) = [0.5, 0, 1, 0.25, 0.25]
+    u = np.array([0.49, 0.0, 0.999, 0.25, 0.2499])
+    # kept iff u < p: index 0 (0.49 < 0.5), not 1 (0 < 0 false), 2 (p = 1), not 3 (0.25 < 0.25 false), 4
+    # order: score desc, index asc -> 2 (1.0), 0 (0.5), 4 (0.25)
+    assert O.bernoulli_select(scores, 2, 2.0, u, 10).tolist() == [2, 0, 4]
+    assert O.bernoulli_select(scores, 2, 2.0, u, 2).tolist() == [2, 0]                      # cap keeps the best
+    # c large: every index with a positive score has p = 1 and is kept whatever u is
+    assert O.bernoulli_select(scores, 2, 1e9, np.full(5, 0.999999), 10).tolist() == [2, 0, 3, 4]
+    # c = 0: nothing
+    assert O.bernoulli_select(scores, 2, 0.0, np.zeros(5), 10).size == 0
+
+
+def test_bernoulli_expected_sample_size():
+    """E #kept = sum_i min(1, c pi_i) (Alg. 3 line 5): averaged over 400 independent keys."""
+    rng = np.random.default_rng(0)
+    n, cols = 5000, 6
+    Q, _ = np.linalg.qr(rng.standard_normal((n, cols)) * np.exp(-np.arange(n) / 300.0)[:, None])
+    sc = O.leverage_scores(Q)
+    c = 14.0
+    expect = np.minimum(1.0, c * sc / cols).sum()
+    counts = [O.bernoulli_select(sc, cols, c, O.counter_uniforms(s, 0, 0, n), n).size for s in range(400)]
+    assert abs(np.mean(counts) - expect) < 4 * np.sqrt(expect / 400) + 0.05
+    assert expect <= c + 1e-9
+
+
+def test_bernoulli_selection_escapes_the_deterministic_stall():
+    """with LS 'its probabilistic nature makes it exceedingly unlikely that exactly the same index set is
+    selected twice in a row'.  The deterministic top-k form re-selects the same indices on the Hilbert matrix (n = 1024,
+    this initial guess) and never passes the stop test; the printed Bernoulli form converges to the same matrix."""
+    n = 1024
+    U0, V0, sg = W.matrix_initial_guess(n, 4, 1)
+    kw = dict(tol=1e-9, max_rank=64, oversample=8, max_sweeps=12, safeguard=sg)
+    det = O.cross_deim(n, O.matrix_fibers("hilbert", n), U0, V0, **kw)
+    assert not det.converged and [len(t.I) for t in det.trace][-4:] == [len(t.I) for t in det.trace][-6:-2]      # period-2 stall
+    rnd = O.cross_deim(n, O.matrix_fibers("hilbert", n), U0, V0, selection="bernoulli", ls_seed=7, **kw)
+    assert rnd.converged and rnd.sweeps <= 8
+    i = np.arange(n)
+    G = O.hilbert_entries(i[:, None], i[None, :])
+    A = (rnd.U[:, :rnd.rank] * rnd.S[:rnd.rank]) @ rnd.V[:, :rnd.rank].T
+    assert np.linalg.norm(A - G) <= 5e-9 * np.linalg.norm(G)
+    # every sweep's selection is exactly the Bernoulli draw of that sweep's key, in (score desc, index asc) order
+    t = rnd.trace[1]
+    expect = O.bernoulli_select(t.scoresU, rnd.trace[0].rank, float(rnd.trace[0].rank + 8), O.counter_uniforms(7, 1, 0, n), 2 * 2 * (64 + 8))
+    assert t.Istar.tolist() == expect.tolist()
