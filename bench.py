@@ -117,7 +117,7 @@ PHASE_OF = {"dst1_small": ("dst", "hbm"), "dst1_naive": ("dst", "hbm"), "dst1_fu
             "panel_apply": ("qr", "fp64"), "add_block": ("qr", "fp64"), "conditional_refactor": ("qr", "fp64"), "tall_resid_gram": ("rho", "fp64"),
             "rho": ("rho", "latency"), "eta": ("core", "latency"), "scross_core": ("core", "latency"),
             "rownorm2": ("leverage", "hbm"), "topk_chunk": ("leverage", "hbm"), "topk_merge": ("leverage", "latency"),
-            "topk": ("leverage", "hbm"), "colmask": ("leverage", "latency"), "copy_tall": ("leverage", "hbm"),
+            "topk": ("leverage", "hbm"), "deim_step": ("leverage", "hbm"), "colmask": ("leverage", "latency"), "copy_tall": ("leverage", "hbm"),
             "gather_rows": ("core", "latency"), "lowrank_entries": ("core", "latency"), "reduce_partials": ("qr", "fp64")}
 
 

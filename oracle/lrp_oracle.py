@@ -327,6 +327,54 @@ def bernoulli_select(scores: np.ndarray, cols: int, c: float, u: np.ndarray, cap
     return kept[order][:cap].astype(np.int32)
 
 
+# ----------------------------------------------------------------------------- Alg. 2: DEIM / QDEIM
+def qdeim_select(U: np.ndarray) -> np.ndarray:
+    """QDEIM (Alg. 2 lines 7-10): column-pivoted Householder QR of U^T (cols x n); the pivot columns, in
+    pivot order, are the selected row indices of U (as many as U has columns).  Written out: at step c the column of
+    the trailing block with the largest 2-norm (recomputed exactly, lowest index on ties) is swapped to position c, a
+    Householder reflector annihilates it below the diagonal and is applied to the remaining columns."""
+    A = np.array(np.asarray(U, dtype=np.float64).T, copy=True)           # cols x n
+    r, n = A.shape
+    perm = np.arange(n)
+    steps = min(r, n)
+    for c in range(steps):
+        nrm2 = np.einsum("ij,ij->j", A[c:, c:], A[c:, c:])
+        j = c + int(np.argmax(nrm2))                                       # first maximum = lowest index on ties
+        if j != c:
+            A[:, [c, j]] = A[:, [j, c]]
+            perm[[c, j]] = perm[[j, c]]
+        x = A[c:, c].copy()
+        alpha = x[0]
+        xnorm = np.linalg.norm(x[1:]) if x.size > 1 else 0.0
+        if xnorm != 0.0:
+            beta = -math.copysign(math.hypot(alpha, xnorm), alpha)
+            tau = (beta - alpha) / beta
+            v = x / (alpha - beta)
+            v[0] = 1.0
+            A[c:, c:] -= tau * np.outer(v, v @ A[c:, c:])
+    return perm[:steps].astype(np.int32)
+
+
+def deim_select(U: np.ndarray) -> np.ndarray:
+    """DEIM (Alg. 2 lines 3-6): LU with partial (row) pivoting of U (n x cols); the pivot rows, in pivot
+    order, are the selected indices.  Written out: at step c the row with the largest |entry| of column c among the
+    rows not yet chosen (lowest index on ties) becomes the pivot, and column c is eliminated from the other unchosen rows."""
+    A = np.array(U, dtype=np.float64, copy=True)
+    n, r = A.shape
+    free = np.ones(n, dtype=bool)
+    out = []
+    for c in range(min(r, n)):
+        col = np.where(free, np.abs(A[:, c]), -1.0)
+        p = int(np.argmax(col))
+        out.append(p)
+        free[p] = False
+        if A[p, c] != 0.0 and c + 1 < r:
+            m = A[:, c] / A[p, c]
+            m[~free] = 0.0
+            A[:, c + 1:] -= np.outer(m, A[p, c + 1:])
+    return np.asarray(out, dtype=np.int32)
+
+
 # ----------------------------------------------------------------------------- O8 scross
 @dataclass
 class ScrossResult:
@@ -514,7 +562,8 @@ def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, ma
     selection, union, safeguard, prune and stopping decisions are taken from it.
     selection: "topk" = the deterministic top-(cols + p_os) form (reading Q5); "bernoulli" = Alg. 3 lines 4-5 as printed,
     with c = ls_c if ls_c > 0 else cols + p_os (expected sample size <= the deterministic form's count) and uniforms
-    from `counter_uniforms(ls_seed, sweep, side, n)` (side 0: rows / U, side 1: columns / V).
+    from `counter_uniforms(ls_seed, sweep, side, n)` (side 0: rows / U, side 1: columns / V); "qdeim" / "deim" = Alg. 2
+    applied to the orthonormal factor of the previous iterate (its thin QR; cols indices, in pivot order).
     """
     K_cap = 2 * (max_rank + oversample)                      # reading Q10
     Uprev_sel = np.asarray(U0)                               # O5 (reading Q7)
@@ -531,7 +580,14 @@ def cross_deim(n: int, fibers, U0: np.ndarray, V0: np.ndarray, *, tol: float, ma
             # O6: selection. k = 0 (user factors) needs the QR; later iterates are orthonormal
             # up to rounding, for which the QR is the identity (reading Q6) -- the oracle still
             # performs it, as the definition.
-            if selection == "bernoulli":
+            if selection in ("qdeim", "deim"):
+                QU, _ = householder_qr(Uprev_sel)            # Alg. 2 line 1: "Input: orthogonal matrix U"
+                QV, _ = householder_qr(Vprev_sel)
+                scU = np.einsum("ij,ij->i", QU, QU)          # kept for the safeguard fallback and the trace
+                scV = np.einsum("ij,ij->i", QV, QV)
+                Istar = qdeim_select(QU) if selection == "qdeim" else deim_select(QU)
+                Jstar = qdeim_select(QV) if selection == "qdeim" else deim_select(QV)
+            elif selection == "bernoulli":
                 scU = leverage_scores(Uprev_sel)
                 scV = leverage_scores(Vprev_sel)
                 cU = ls_c if ls_c > 0 else float(Uprev_sel.shape[1] + oversample)

@@ -122,7 +122,7 @@ struct SolveWs {
     double *Sprev, *Amat, *Bmat, *GU, *GV, *rho_out, *eta, *eta_work, *gemmt_ws, *gemmt_ws2, *Rlev, *Rlev2;
     int32_t *dI, *dJ, *dIpr, *dJpr, *dIstar, *dJstar, *eta_iwork;
     unsigned char *mask, *mask2;
-    void *sel_ws, *dst_ws, *dst_ws2;
+    void *sel_ws, *dst_ws, *dst_ws2, *deim_ws;
     size_t eta_stride, dst_ws_bytes;
     ScrossWs sc;
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int rF, int Kc, int max_rank, bool poisson = true) {
@@ -151,6 +151,7 @@ struct SolveWs {
         dIstar = ar.take<int32_t>(2 * (size_t)Kc + 8); dJstar = ar.take<int32_t>(2 * (size_t)Kc + 8);
         mask = ar.take<unsigned char>(Kc); mask2 = ar.take<unsigned char>(Kc);
         sel_ws = ar.take<char>(select_ws_bytes(ctx, n, 2 * Kc + 1));
+        deim_ws = ar.take<char>(deim_ws_bytes(n, Kc));
         int dcols = rF > max_rank ? rF : max_rank;
         dst_ws_bytes = poisson ? lrp_dst1_ws_impl(n, dcols) : 0;
         dst_ws = ar.take<char>(dst_ws_bytes ? dst_ws_bytes : 1);
@@ -562,7 +563,18 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
                 double* sc = side == 0 ? w.scoresU : w.scoresV;
                 int32_t* dstar = side == 0 ? w.dIstar : w.dJstar;
                 int nstar = numsel;
-                if (opts->selection == LRP_SELECT_BERNOULLI) {   // Alg. 3 lines 4-5 as printed, reading Q23
+                if (opts->selection == LRP_SELECT_QDEIM || opts->selection == LRP_SELECT_DEIM) {
+                    // Alg. 2 on the orthonormal factor of the previous iterate: at k = 0 the Q of the
+                    // initial guess (left in Cb / Rb by the leverage QR above), later the iterate itself; the target
+                    // buffer of this sweep's rebuild is free and serves as the (destroyed) working copy
+                    const double* src = k == 0 ? (side == 0 ? w.Cb : w.Rb) : (side == 0 ? Up : Vp);
+                    double* work = side == 0 ? Uk : Vk;
+                    nstar = sel_cols;
+                    LRP_TRY(tall_copy(ctx, n, sel_cols, src, ld, work, ld));
+                    LRP_TRY(deim_select(ctx, opts->selection == LRP_SELECT_QDEIM ? 1 : 0, n, sel_cols, work, ld, dstar, w.deim_ws));
+                    LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * nstar, cudaMemcpyDeviceToHost, ctx->stream));
+                    LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                } else if (opts->selection == LRP_SELECT_BERNOULLI) {   // Alg. 3 lines 4-5 as printed, reading Q23
                     SelectBernoulli b{};
                     b.cols = sel_cols; b.c = opts->ls_c > 0.0 ? opts->ls_c : (double)(sel_cols + p_os);
                     b.seed = opts->ls_seed; b.sweep = k; b.side = side;

@@ -13,13 +13,13 @@
 enum LrpKernelId {
     K_DST_SMALL, K_DST_NAIVE, K_DST_FUSED,
     K_GEMM_SAMPLE, K_GEMM_PLAIN, K_GEMM_SUBTRACT, K_GEMM_T, K_REDUCE, K_ROWNORM, K_GATHER, K_COPY, K_ENTRIES,
-    K_PANEL_QR, K_PANEL_APPLY, K_ADD_BLOCK, K_CORE, K_ETA, K_RHO, K_COLMASK, K_TOPK, K_RESID_GRAM, K_COND, K_NUM
+    K_PANEL_QR, K_PANEL_APPLY, K_ADD_BLOCK, K_CORE, K_ETA, K_RHO, K_COLMASK, K_TOPK, K_RESID_GRAM, K_COND, K_DEIM, K_NUM
 };
 static const char* const LRP_KERNEL_NAMES[K_NUM] = {
     "dst1_small", "dst1_naive", "dst1_fused",
     "tall_gemm_sample", "tall_gemm_plain", "tall_gemm_subtract", "tall_gemm_t", "reduce_partials", "rownorm2", "gather_rows",
     "copy_tall", "lowrank_entries", "panel_qr", "panel_apply", "add_block", "scross_core", "eta", "rho", "colmask",
-    "topk", "tall_resid_gram", "conditional_refactor"
+    "topk", "tall_resid_gram", "conditional_refactor", "deim_step"
 };
 struct lrp_prof { int64_t count; double ms, bytes, flops; };
 

@@ -71,3 +71,7 @@ size_t select_ws_bytes(const lrp_ctx* ctx, int64_t n, int num);
 int select_init(lrp_ctx* ctx);
 int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t* idx_out, void* ws,
                 const SelectBernoulli* bern = nullptr, int* d_count = nullptr);
+
+// (Q)DEIM index selection (Alg. 2; deim.cu): r indices in pivot order of the n x r matrix A (destroyed).
+size_t deim_ws_bytes(int64_t n, int r);
+int deim_select(lrp_ctx* ctx, int qdeim, int64_t n, int r, double* A, int64_t lda, int32_t* idx_out, void* ws);

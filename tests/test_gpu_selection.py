@@ -89,3 +89,54 @@ def test_bernoulli_escapes_the_stall_on_the_gpu(ctx):
     U, V, S = lrp.tall_to_numpy(rnd["UW"]), lrp.tall_to_numpy(rnd["VW"]), rnd["SW"].cpu().numpy()
     a = np.einsum("tk,k,tk->t", U[rows], S, V[cols])
     assert np.abs(a - O.hilbert_entries(rows, cols)).max() <= 5e-8
+
+
+@pytest.mark.parametrize("sel", ["qdeim", "deim"])
+@pytest.mark.parametrize("kind,n,seed", [("hilbert", 1024, 1), ("hilbert", 777, 0), ("kmatrix", 512, 0)])
+def test_deim_variants_on_test_matrices(ctx, sel, kind, n, seed):
+    """NEXT-3 of SURVEY.md 8(f): QDEIM (column-pivoted QR of U^T) and DEIM (pivoted LU) selection, Alg. 2, as
+    hand-written kernels (the paper had to leave them to JAX / MAGMA).  Free run: the ordered pivot lists
+    of the first sweeps equal the oracle's (pivot gaps of these generic matrices are far above rounding); replay: 1e-10."""
+    from paper_2607_06021_b200 import lrp
+    tol = 1e-9 if kind == "hilbert" else 1e-6
+    U0, V0, sg = W.matrix_initial_guess(n, 4, seed)
+    kw = dict(tol=tol, max_rank=64, oversample=8, max_sweeps=10, safeguard=sg)
+    ref = O.cross_deim(n, O.matrix_fibers(kind, n), U0, V0, selection=sel, **kw)
+    res = ctx.cross_deim_matrix(kind, n, lrp.tall_from_numpy(U0), lrp.tall_from_numpy(V0), selection=sel, want_spectral=True, **kw)
+    same = 0
+    for s in range(min(res["sweeps"], ref.sweeps)):
+        if res["trace"][s]["I"].tolist() != ref.trace[s].I.tolist() or res["trace"][s]["J"].tolist() != ref.trace[s].J.tolist():
+            break
+        same += 1
+    print(f"{kind} n={n} {sel}: GPU {res['sweeps']} sweeps rank {res['rank']} conv {res['converged']}; oracle {ref.sweeps} sweeps rank "
+          f"{ref.rank} conv {ref.converged}; identical index lists on the first {same} sweeps")
+    assert same >= 2                                           # sweep 0 (random initial guess) and sweep 1 at least
+    assert abs(res["sweeps"] - ref.sweeps) <= 1
+    rep = O.trace_to_replay(ref.trace, ref.rank)
+    res2 = ctx.cross_deim_matrix(kind, n, lrp.tall_from_numpy(U0), lrp.tall_from_numpy(V0), replay=rep, want_spectral=True, **kw)
+    rows, cols = W.sample_pairs(n, 4096, seed=4)
+    U, V, S = lrp.tall_to_numpy(res2["UW"]), lrp.tall_to_numpy(res2["VW"]), res2["SW"].cpu().numpy()
+    a = np.einsum("tk,k,tk->t", U[rows], S, V[cols])
+    b = O.lowrank_entries(ref.U[:, :ref.rank], ref.S[:ref.rank], ref.V[:, :ref.rank], rows, cols)
+    t = ref.trace[-1]
+    tolW = 1e-10 if ref.converged else max(1e-10, 0.1 * t.rho / t.snorm, t.ind / t.snorm)
+    assert np.abs(a - b).max() <= tolW * np.abs(b).max(), (np.abs(a - b).max() / np.abs(b).max(), tolW)
+
+
+@pytest.mark.parametrize("sel", ["qdeim", "deim"])
+def test_deim_variants_on_the_poisson_solve(ctx, sel):
+    from paper_2607_06021_b200 import lrp
+    w = W.make("C4", 0, 16383)
+    w.max_sweeps = 6
+    ref = O.cross_deim_solve(w.n, w.UF, w.SF, w.VF, selection=sel, **w.opts())
+    res = _solve(ctx, w, selection=sel)
+    for s in range(2):
+        assert res["trace"][s]["I"].tolist() == ref.trace[s].I.tolist() and res["trace"][s]["J"].tolist() == ref.trace[s].J.tolist()
+    rep = O.trace_to_replay(ref.trace, ref.rank)
+    res2 = _solve(ctx, w, replay=rep)
+    rows, cols_ = W.sample_pairs(w.n, 4096, seed=1)
+    UW, VW, SW = lrp.tall_to_numpy(res2["UW"]), lrp.tall_to_numpy(res2["VW"]), res2["SW"].cpu().numpy()
+    a = np.einsum("tk,k,tk->t", UW[rows], SW, VW[cols_]); b = O.lowrank_entries(ref.UW, ref.SW, ref.VW, rows, cols_)
+    t = ref.trace[-1]
+    tolW = 1e-10 if ref.converged else max(1e-10, 0.1 * t.rho / t.snorm, t.ind / t.snorm)
+    assert np.abs(a - b).max() <= tolW * np.abs(b).max()
