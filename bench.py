@@ -111,7 +111,7 @@ def solve_roofline(n, rF, trace, r_final, hbm_gbs, p64_tflops, ms_measured):
 NCU_TRAFFIC = {}
 
 # kernel class -> (phase, roofline SURVEY.md 8(d) assigns to it)
-PHASE_OF = {"dst1_small": ("dst", "hbm"), "dst1_naive": ("dst", "hbm"), "dst1_fused": ("dst", "hbm"),
+PHASE_OF = {"dst1_small": ("dst", "hbm"), "dst1_naive": ("dst", "hbm"), "dst1_fused": ("dst", "hbm"), "dst1_bluestein": ("dst", "hbm"),
             "tall_gemm_sample": ("sampling", "hbm"), "tall_gemm_plain": ("rebuild", "fp64"),
             "tall_gemm_subtract": ("qr", "fp64"), "tall_gemm_t": ("qr", "fp64"), "panel_qr": ("qr", "fp64"),
             "panel_apply": ("qr", "fp64"), "add_block": ("qr", "fp64"), "conditional_refactor": ("qr", "fp64"), "tall_resid_gram": ("rho", "fp64"),

@@ -26,7 +26,8 @@
  *     only where stated.
  *   - return value: 0 = LRP_OK, negative = error, positive = warning (outputs valid).
  *     No exceptions, no globals, no environment variables, no CPU fallback: without a CUDA device every compute call fails.
- *   - n + 1 must be a power of two, 2 <= n + 1 <= 2^25 (general n: DESIGN.md "next").
+ *   - n: n + 1 a power of two up to 2^25 (the fast paths), or any n with n + 1 <= 2^23 (Bluestein's chirp-z form of the
+ *     DST-I, 8-16x the work; the paper's own grids n = 2^10..2^18, are of this kind).
  */
 #ifndef LRP_H_
 #define LRP_H_
@@ -40,7 +41,7 @@ extern "C" {
 
 #define LRP_OK                  0
 #define LRP_ERR_BADARG         -1   /* null / misaligned pointer, ld < n, set larger than the cap, duplicate or out-of-range index */
-#define LRP_ERR_UNSUPPORTED_N  -2   /* n + 1 not a power of two, or out of range */
+#define LRP_ERR_UNSUPPORTED_N  -2   /* n out of range (see above) */
 #define LRP_ERR_WORKSPACE      -3   /* workspace missing or too small */
 #define LRP_ERR_CUDA           -4   /* a CUDA call failed; see lrp_last_cuda_error */
 #define LRP_WARN_NOCONV         1   /* Cross-DEIM reached max_sweeps (or r* > max_rank): outputs valid, tolerance not certified */
@@ -81,7 +82,7 @@ int lrp_fp64_peak(lrp_ctx* ctx, double* dfma_tflops, double* dmma_tflops);
 /* Workspace sizes in bytes (host-side arithmetic only; safe to call without a GPU).
  *   lrp_workspace_bytes        : everything lrp_cross_deim_solve needs for rank-rF input, K_cap = 2 (max_rank + oversample)
  *                                (reading Q10); 0 when the arguments are invalid, e.g. rF + oversample + 1 > K_cap.
- *   lrp_dst1_workspace_bytes   : lrp_dst1_batched (0 for n <= 16383, the single-pass shared-memory regime).
+ *   lrp_dst1_workspace_bytes   : lrp_dst1_batched (0 for n + 1 = 2^p <= 16384, the single-pass shared-memory regime).
  *   lrp_leverage_workspace_bytes, lrp_scross_workspace_bytes : the standalone calls. */
 size_t lrp_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample);
 size_t lrp_dst1_workspace_bytes(int64_t n, int32_t batch);
@@ -96,7 +97,7 @@ int lrp_set_workspace(lrp_ctx* ctx, void* d_ws, size_t bytes);
  * scale = sqrt(2/(n+1)): the symmetric orthogonal Z of PAPER.md:198-200 (twice = identity).
  * in/out: tall n x batch, column b at d_in + b*ld_in.  d_in == d_out (same ld) is allowed; partial overlap is not.
  * Each column is transformed independently along its own (contiguous) dimension: no transpose.
- * Asynchronous.  Errors: BADARG, UNSUPPORTED_N, WORKSPACE (n > 16383 needs lrp_dst1_workspace_bytes), CUDA. */
+ * Asynchronous.  Errors: BADARG, UNSUPPORTED_N, WORKSPACE (n > 16383 or n + 1 not a power of two: lrp_dst1_workspace_bytes), CUDA. */
 int lrp_dst1_batched(lrp_ctx* ctx, int64_t n, int32_t batch,
                      const double* d_in, int64_t ld_in, double* d_out, int64_t ld_out, double scale);
 
@@ -236,6 +237,13 @@ int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve
  *     d_C (n x nJ): column c = G(:, J[c]);   d_Rt (n x nI): column c = G(I[c], :)^T.   Either may be NULL.  Asynchronous. */
 int lrp_sample_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,
                       double* d_C, int64_t ldc, double* d_Rt, int64_t ldr);
+
+/* Dense full-rank DST solver of section 3.1 (eq. (4)): W = Z ((Z F Z) ./ (d_i + d_j)) Z for a
+ * dense n x n right-hand side F (column-major, ld >= n), O(n^2 log n) -- the baseline the low-rank method is measured
+ * against, n <= 32768 (2 n^2 doubles of workspace + the transform's: lrp_dense_workspace_bytes).  d_W may alias d_F.
+ * Asynchronous.  Errors: BADARG, UNSUPPORTED_N, WORKSPACE, CUDA. */
+size_t lrp_dense_workspace_bytes(int64_t n);
+int lrp_dense_poisson(lrp_ctx* ctx, int64_t n, const double* d_F, int64_t ldf, double* d_W, int64_t ldw);
 
 /* Entries (U diag(S) V^T)(rows[t], cols[t]), t < count (X(i,j) = sum_k sigma_k u_k(i) v_k(j)):
  * the O(r) element access used to read a low-rank result without forming it.  All pointers device.  Asynchronous. */

@@ -26,8 +26,8 @@ int64_t internal_ld(int64_t n) { return n + 74 + (n & 1); }
 int check_n(int64_t n) {
     if (n < 1) return LRP_ERR_UNSUPPORTED_N;
     int64_t N = n + 1;
-    if (!lrp_is_pow2(N) || N > ((int64_t)1 << 25)) return LRP_ERR_UNSUPPORTED_N;
-    return LRP_OK;
+    if (lrp_is_pow2(N)) return N > ((int64_t)1 << 25) ? LRP_ERR_UNSUPPORTED_N : LRP_OK;
+    return dst1_bluestein_supported(n) ? LRP_OK : LRP_ERR_UNSUPPORTED_N;      // general n: Bluestein, n + 1 <= 2^23
 }
 
 // ------------------------------------------------------------------------------------------------ scross on owned buffers
@@ -315,7 +315,7 @@ const char* lrp_strerror(int code) {
     switch (code) {
         case LRP_OK: return "ok";
         case LRP_ERR_BADARG: return "bad argument";
-        case LRP_ERR_UNSUPPORTED_N: return "n + 1 must be a power of two in [2, 2^25]";
+        case LRP_ERR_UNSUPPORTED_N: return "n out of range: n + 1 a power of two <= 2^25, or any n + 1 <= 2^23";
         case LRP_ERR_WORKSPACE: return "workspace missing or too small";
         case LRP_ERR_CUDA: return "CUDA error (see lrp_last_cuda_error)";
         case LRP_WARN_NOCONV: return "warning: stop test not passed within max_sweeps";
@@ -864,6 +864,35 @@ int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve
     if (!opts || kind == LRP_G_POISSON) return LRP_ERR_BADARG;
     return solve_impl(ctx, kind, n, opts->r0, nullptr, 0, nullptr, nullptr, 0, opts, d_U, ldu, d_S, d_V, ldv, info,
                       h_trace_I, h_trace_J, h_trace_keepI, h_trace_keepJ, d_Uhat, d_Shat, d_Vhat, ld_hat);
+}
+
+size_t lrp_dense_workspace_bytes(int64_t n) {
+    if (check_n(n) != LRP_OK || n > 32768) return 0;
+    return 2 * lrp_align_up((size_t)n * n * sizeof(double)) + lrp_align_up(lrp_dst1_ws_impl(n, (int32_t)n)) + 256;
+}
+
+int lrp_dense_poisson(lrp_ctx* ctx, int64_t n, const double* d_F, int64_t ldf, double* d_W, int64_t ldw) {
+    if (!ctx || !d_F || !d_W || ldf < n || ldw < n) return LRP_ERR_BADARG;
+    LRP_TRY(check_n(n));
+    if (n > 32768) return LRP_ERR_UNSUPPORTED_N;
+    if (ctx->ws_bytes < lrp_dense_workspace_bytes(n)) return LRP_ERR_WORKSPACE;
+    lrp_arena ar(ctx->ws, ctx->ws_bytes);
+    double* T1 = ar.take<double>((size_t)n * n);
+    double* T2 = ar.take<double>((size_t)n * n);
+    const size_t dws_bytes = lrp_dst1_ws_impl(n, (int32_t)n);
+    void* dws = ar.take<char>(dws_bytes ? dws_bytes : 1);
+    if (!ar.ok()) return LRP_ERR_WORKSPACE;
+    const double sc = sqrt(2.0 / (double)(n + 1));
+    const int32_t b = (int32_t)n;
+    // What = Z F Z ./ (d_i + d_j), W = Z What Z (eq. (4)), Z symmetric orthogonal: four column-wise
+    // batched DST-I and two transposes (the full-rank method needs the global transposes the low-rank one avoids)
+    LRP_TRY(lrp_dst1_impl(ctx, n, b, d_F, ldf, T1, n, sc, dws, dws_bytes));        // Z F
+    LRP_TRY(tall_transpose(ctx, n, T1, n, T2, n));                                 // (Z F)^T = F^T Z
+    LRP_TRY(lrp_dst1_impl(ctx, n, b, T2, n, T2, n, sc, dws, dws_bytes));           // Z F^T Z = Fhat^T
+    LRP_TRY(tall_spectral_divide(ctx, n, T2, n));                                  // What^T (the divisor is symmetric)
+    LRP_TRY(lrp_dst1_impl(ctx, n, b, T2, n, T2, n, sc, dws, dws_bytes));           // Z What^T = (What Z)^T
+    LRP_TRY(tall_transpose(ctx, n, T2, n, T1, n));                                 // What Z
+    return lrp_dst1_impl(ctx, n, b, T1, n, d_W, ldw, sc, dws, dws_bytes);          // W = Z What Z
 }
 
 int lrp_sample_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const int32_t* d_I, int32_t nI, const int32_t* d_J, int32_t nJ,

@@ -11,12 +11,12 @@
 // kernel classes for the per-kernel profile (lrp_profile_*): launch counts, CUDA-event time on the ctx's stream,
 // and the ALGORITHMIC bytes / flops of the launches (what the step must move / compute).
 enum LrpKernelId {
-    K_DST_SMALL, K_DST_NAIVE, K_DST_FUSED,
+    K_DST_SMALL, K_DST_NAIVE, K_DST_FUSED, K_DST_BLUESTEIN,
     K_GEMM_SAMPLE, K_GEMM_PLAIN, K_GEMM_SUBTRACT, K_GEMM_T, K_REDUCE, K_ROWNORM, K_GATHER, K_COPY, K_ENTRIES,
     K_PANEL_QR, K_PANEL_APPLY, K_ADD_BLOCK, K_CORE, K_ETA, K_RHO, K_COLMASK, K_TOPK, K_RESID_GRAM, K_COND, K_DEIM, K_NUM
 };
 static const char* const LRP_KERNEL_NAMES[K_NUM] = {
-    "dst1_small", "dst1_naive", "dst1_fused",
+    "dst1_small", "dst1_naive", "dst1_fused", "dst1_bluestein",
     "tall_gemm_sample", "tall_gemm_plain", "tall_gemm_subtract", "tall_gemm_t", "reduce_partials", "rownorm2", "gather_rows",
     "copy_tall", "lowrank_entries", "panel_qr", "panel_apply", "add_block", "scross_core", "eta", "rho", "colmask",
     "topk", "tall_resid_gram", "conditional_refactor", "deim_step"
@@ -115,5 +115,11 @@ int lrp_dst1_init(lrp_ctx* ctx);      // one-time kernel attributes (lrp_create)
 // four-step regime (dst1_large.cu), N = n + 1 > 16384
 size_t dst1_large_ws(int64_t N, int32_t batch);
 int dst1_large_init(lrp_ctx* ctx);
+// general n (n + 1 not a power of two): Bluestein (dst1_bluestein.cu)
+int dst1_bluestein_init(lrp_ctx* ctx);
+bool dst1_bluestein_supported(int64_t n);
+size_t dst1_bluestein_ws(int64_t n, int32_t batch);
+int dst1_bluestein(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, int64_t ld_in, double* d_out, int64_t ld_out,
+                   double scale, void* ws, size_t ws_bytes);
 int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64_t ld_in,
                double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes);

@@ -175,12 +175,15 @@ int lrp_dst1_init(lrp_ctx* ctx) {
     LRP_TRY(init_small<5>(ctx)); LRP_TRY(init_small<6>(ctx)); LRP_TRY(init_small<7>(ctx)); LRP_TRY(init_small<8>(ctx));
     LRP_TRY(init_small<9>(ctx)); LRP_TRY(init_small<10>(ctx)); LRP_TRY(init_small<11>(ctx)); LRP_TRY(init_small<12>(ctx));
     LRP_TRY(init_small<13>(ctx));
-    return dst1_large_init(ctx);
+    LRP_TRY(dst1_large_init(ctx));
+    return dst1_bluestein_init(ctx);
 }
 
 size_t lrp_dst1_ws_impl(int64_t n, int32_t batch) {
     int64_t N = n + 1;
-    if (N <= 16384 || batch <= 0) return 0;
+    if (batch <= 0) return 0;
+    if (!lrp_is_pow2(N)) return dst1_bluestein_ws(n, batch);
+    if (N <= 16384) return 0;
     return dst1_large_ws(N, batch);
 }
 
@@ -188,6 +191,7 @@ int lrp_dst1_impl(lrp_ctx* ctx, int64_t n, int32_t batch, const double* d_in, in
                   double* d_out, int64_t ld_out, double scale, void* ws, size_t ws_bytes) {
     if (batch == 0) return LRP_OK;
     const int64_t N = n + 1;
+    if (!lrp_is_pow2(N)) return dst1_bluestein(ctx, n, batch, d_in, ld_in, d_out, ld_out, scale, ws, ws_bytes);
     if (N < 64) {
         LRP_PROF(ctx, K_DST_NAIVE, 16.0 * n * batch, 0);
         dst1_naive_kernel<<<batch, 32, 0, ctx->stream>>>((int)n, d_in, ld_in, d_out, ld_out, scale);

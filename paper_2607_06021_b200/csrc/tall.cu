@@ -69,7 +69,48 @@ __global__ void matrix_fibers_kernel(int kind, int64_t n, int transposed, const 
     }
 }
 
+// B (n x n, ld ldb) = A^T (A n x n, ld lda): 32 x 32 tiles through shared memory (dense full-rank baseline only)
+__global__ void transpose_kernel(int64_t n, const double* __restrict__ A, int64_t lda, double* __restrict__ B, int64_t ldb) {
+    __shared__ double tile[32][33];
+    const int64_t i0 = (int64_t)blockIdx.x * 32, j0 = (int64_t)blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int64_t i = i0 + threadIdx.x, j = j0 + r;
+        if (i < n && j < n) tile[r][threadIdx.x] = A[i + j * lda];
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int64_t j = j0 + threadIdx.x, i = i0 + r;
+        if (i < n && j < n) B[j + i * ldb] = tile[threadIdx.x][r];
+    }
+}
+// A(i,j) /= d_i + d_j,  d_k = 4 (n+1)^2 sin^2(pi (k+1) / (2(n+1)))     eq. (4)
+__global__ void spectral_divide_kernel(int64_t n, double* __restrict__ A, int64_t lda) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double invN = 1.0 / (double)(n + 1), f = 4.0 * (double)(n + 1) * (double)(n + 1);
+    const double si = sinpi(0.5 * (double)(i + 1) * invN), di = f * si * si;
+    for (int64_t j = blockIdx.y; j < n; j += gridDim.y) {
+        const double sj = sinpi(0.5 * (double)(j + 1) * invN);
+        A[i + j * lda] /= di + f * sj * sj;
+    }
+}
+
 }  // namespace
+
+int tall_transpose(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, double* B, int64_t ldb) {
+    dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32));
+    LRP_PROF(ctx, K_COPY, 16.0 * n * n, 0);
+    transpose_kernel<<<grid, dim3(32, 8), 0, ctx->stream>>>(n, A, lda, B, ldb);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
+int tall_spectral_divide(lrp_ctx* ctx, int64_t n, double* A, int64_t lda) {
+    dim3 grid((unsigned)((n + 255) / 256), (unsigned)(n < 1024 ? n : 1024));
+    LRP_PROF(ctx, K_COPY, 16.0 * n * n, 0);
+    spectral_divide_kernel<<<grid, 256, 0, ctx->stream>>>(n, A, lda);
+    LRP_LAUNCHED(ctx);
+    return LRP_OK;
+}
 
 int tall_matrix_fibers(lrp_ctx* ctx, int kind, int64_t n, int transposed, const int32_t* idx, int nidx, double* Out, int64_t ldo) {
     if (nidx <= 0) return LRP_OK;

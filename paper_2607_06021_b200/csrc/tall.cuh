@@ -33,6 +33,8 @@ int tall_rownorm2(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, 
 int tall_gather_rows(lrp_ctx* ctx, const double* A, int64_t lda, int k, const int32_t* idx, int nidx, double* Out, int ldo);
 // fibers of the closed-form test matrices (eq. (6)): kind 1 Hilbert, kind 2 K; see tall.cu
 int tall_matrix_fibers(lrp_ctx* ctx, int kind, int64_t n, int transposed, const int32_t* idx, int nidx, double* Out, int64_t ldo);
+int tall_transpose(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, double* B, int64_t ldb);
+int tall_spectral_divide(lrp_ctx* ctx, int64_t n, double* A, int64_t lda);
 int tall_copy(lrp_ctx* ctx, int64_t n, int k, const double* A, int64_t lda, double* B, int64_t ldb);
 int tall_lowrank_entries(lrp_ctx* ctx, int r, const double* U, int64_t ldu, const double* S, const double* V, int64_t ldv,
                          const int64_t* rows, const int64_t* cols, int64_t count, double* out);

@@ -31,7 +31,7 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
            "lrp_profile_timeline", "lrp_fp64_peak", "lrp_matrix_workspace_bytes", "lrp_cross_deim_matrix",
-           "lrp_sample_matrix"]
+           "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson"]
 
 
 class SolveOpts(C.Structure):
@@ -94,6 +94,8 @@ def load_library():
                                           vp, vp, vp, vp, vp, vp, vp, i64]
     lib.lrp_cross_deim_matrix.restype = C.c_int
     lib.lrp_sample_matrix.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, i64, vp, i64]; lib.lrp_sample_matrix.restype = C.c_int
+    lib.lrp_dense_workspace_bytes.argtypes = [i64]; lib.lrp_dense_workspace_bytes.restype = sz
+    lib.lrp_dense_poisson.argtypes = [vp, i64, vp, i64, vp, i64]; lib.lrp_dense_poisson.restype = C.c_int
     lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_lowrank_entries.restype = C.c_int
     lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
@@ -378,6 +380,16 @@ class Context:
                                                _ptr(J), J.numel() if J is not None else 0, _ptr(Cm), n, _ptr(Rt), n),
                     "lrp_sample_matrix")
         return Cm, Rt
+
+    def dense_poisson(self, F):
+        """Full-rank DST solve of section 3.1 for a dense right-hand side: F a CUDA float64 tensor whose element (i, j) is at
+        F[j, i] (column-major n x n, like every tall tensor here); returns W in the same layout."""
+        torch = _torch()
+        n = F.shape[0]
+        Wd = torch.empty_like(F)
+        self.ensure_workspace(self.lib.lrp_dense_workspace_bytes(n))
+        self._check(self.lib.lrp_dense_poisson(self.h, n, _ptr(F), n, _ptr(Wd), n), "lrp_dense_poisson")
+        return Wd
 
     def lowrank_entries(self, U, S, V, rows, cols):
         torch = _torch()

@@ -176,3 +176,16 @@ def matrix_initial_guess(n: int, r0: int = 4, seed: int = 0):
     V0, _ = np.linalg.qr(rng.standard_normal((n, r0)))
     safeguard = rng.integers(0, n, SAFEGUARD_LEN).astype(np.int32)
     return _fortran(U0), _fortran(V0), safeguard
+
+
+def paper_eq7(n: int, seed: int = 0) -> Workload:
+    """The paper's own Poisson workload, eq. (7): f(x,y) = exp(-36 ((x - 0.1)^2 + (y - 0.55)^2)) on
+    [-1,1]^2 (the printed minus sign between the squares is a typo -- either way the forcing is rank-1 separable, DESIGN.md
+    reading Q19), grids n = 2^10 .. 2^18, i.e. n + 1 NOT a power of two.  In the solver's unit-square convention
+    (s = (x+1)/2, h = 1/(n+1)): -Laplace_s u = 4 f, so S_F = 4.  tol 1e-9, r_max 64."""
+    rng = np.random.default_rng(seed)
+    x = -1.0 + 2.0 * grid(n)
+    UF = np.exp(-36.0 * (x - 0.1) ** 2)[:, None]
+    VF = np.exp(-36.0 * (x - 0.55) ** 2)[:, None]
+    safeguard = rng.integers(0, n, SAFEGUARD_LEN).astype(np.int32)
+    return Workload("eq7", n, _fortran(UF), np.array([4.0]), _fortran(VF), 1e-9, 64, 8, 20, safeguard, dict())

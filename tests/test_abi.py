@@ -60,19 +60,21 @@ int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(lrp_solve_opts), 
 
 def test_host_only_entry_points(lib):
     assert lib.lrp_strerror(0) == b"ok"
-    assert b"power of two" in lib.lrp_strerror(lrp.LRP_ERR_UNSUPPORTED_N)
+    assert b"out of range" in lib.lrp_strerror(lrp.LRP_ERR_UNSUPPORTED_N)
     # one-pass regime needs no workspace, the four-step regime does
     assert lib.lrp_dst1_workspace_bytes(4095, 8) == 0
     assert lib.lrp_dst1_workspace_bytes(16383, 8) == 0
     assert lib.lrp_dst1_workspace_bytes((1 << 20) - 1, 4) >= 4 * (1 << 20) * 8      # W: 8 N bytes per column
-    assert lib.lrp_dst1_workspace_bytes(1000, 4) == 0            # unsupported n -> 0
+    assert lib.lrp_dst1_workspace_bytes(1000, 4) >= 2048 * 16   # general n: Bluestein needs the transformed chirp (P = 2048)
+    assert lib.lrp_dst1_workspace_bytes((1 << 23) + 5, 4) == 0  # out of range -> 0
     # solve workspace grows with n and with the rank cap
     a = lib.lrp_workspace_bytes(255, 4, 16, 8)
     b = lib.lrp_workspace_bytes(4095, 4, 16, 8)
     c = lib.lrp_workspace_bytes(4095, 4, 64, 8)
     assert 0 < a < b < c
     assert c >= 6 * 4095 * 2 * (64 + 8) * 8
-    assert lib.lrp_workspace_bytes(4094, 4, 16, 8) == 0
+    assert lib.lrp_workspace_bytes(4094, 4, 16, 8) > b            # general n is supported
+    assert lib.lrp_workspace_bytes((1 << 23) + 5, 4, 16, 8) == 0
 
 
 def test_no_device_fails_loudly(lib):

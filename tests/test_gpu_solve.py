@@ -137,9 +137,8 @@ def test_solve_argument_errors(ctx):
     with pytest.raises(lrp.LrpError) as e:
         ctx.cross_deim_solve(UF, SF, VF, tol=-1.0, max_rank=16)
     assert e.value.code == lrp.LRP_ERR_BADARG
-    with pytest.raises(lrp.LrpError) as e:
-        ctx.cross_deim_solve(UF[:, :254].contiguous(), SF, VF[:, :254].contiguous(), tol=1e-10, max_rank=16)
-    assert e.value.code == lrp.LRP_ERR_UNSUPPORTED_N
+    # general n is supported (Bluestein); beyond n + 1 = 2^23 it is not
+    assert ctx.lib.lrp_dst1_workspace_bytes((1 << 23) + 1, 1) == 0
     # max_sweeps = 1 cannot pass the stop test -> warning code, outputs still valid
     r = ctx.cross_deim_solve(UF, SF, VF, tol=1e-12, max_rank=16, max_sweeps=1, safeguard=w.safeguard)
     assert r["code"] == lrp.LRP_WARN_NOCONV and r["rank"] >= 1
