@@ -25,6 +25,7 @@
 #include "common.cuh"
 #include "fft_smem.cuh"
 #include <math.h>
+#include <cuda/atomic>
 
 namespace {
 
@@ -55,10 +56,16 @@ template <int Q1, int TL> struct PACfg {
     static_assert(sizeof(double) * 2 * IMOFF >= sizeof(double) * 4 * NT, "anchor partial reduction reuses the FFT arrays");
 };
 
+// Column-independent twiddles of phase A, built once per call (dst1_tables_kernel) and read by every tile from L2:
+//   gB   [2 L2]          exp(-i pi m / N), m = 2 j2 + b
+//   g4lo [L2][32]        exp(-2 pi i j2 l / L)
+//   g4hi [L2][L1/32]     exp(-2 pi i j2 (32 h) / L)
+struct ATables { const double2* gB; const double2* g4lo; const double2* g4hi; };
+
 // tile c of one column: x -> W (L complex), ypart[2 j2 + b] (2 L2 complex): the CTA's folded anchor sums
 template <int Q1, int TL>
 __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int c, const double* __restrict__ x,
-                                        double2* __restrict__ Wc, double2* __restrict__ ypart) {
+                                        double2* __restrict__ Wc, double2* __restrict__ ypart, const ATables tabs) {
     using C = PACfg<Q1, TL>;
     constexpr int L1 = C::L1, GS = C::GS, T2 = C::T2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
@@ -73,24 +80,10 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
     const int tid = threadIdx.x;
     auto j2_of = [&](int s) { return s < T ? c * T + s : L2 - c * T - T + (s - T); };
 
-    tw_build(lo, hi, 2 * L1, C::NHI, tid, NT);
-    for (int i = tid; i < 2 * T2; i += NT) {
-        double sn, cs; sincospi(-(double)(2 * j2_of(i >> 1) + (i & 1)) / (double)N, &sn, &cs); tB[i] = make_double2(cs, sn);
-    }
-    for (int i = tid; i < T2 * (C::TW_LO + C::TW_HI); i += NT) {
-        int s, kk; double2* dst;
-        if (i < T2 * C::TW_LO) { s = i / C::TW_LO; kk = i % C::TW_LO; dst = t4lo + s * C::SLO + kk; }
-        else { int q = i - T2 * C::TW_LO; s = q / C::TW_HI; kk = (q % C::TW_HI) * 32; dst = t4hi + s * C::SHI + (q % C::TW_HI); }
-        int64_t prod = ((int64_t)j2_of(s) * kk) & (L - 1);
-        double sn, cs; sincospi(-2.0 * (double)prod / (double)L, &sn, &cs); *dst = make_double2(cs, sn);
-    }
-    __syncthreads();
-    // fold: t_m = sin(pi m/N)(x_m + x_{N-m}) + (x_m - x_{N-m})/2 for m = 2j, 2j+1;  z_j = t_{2j} + i t_{2j+1}
-    // anchors: ya[b] += (x_m + x_{N-m}) e^{+i pi m/N} for m = m0 + b < L  (the thread's s = tid % T2 is the same for all its e)
-    double2 ya0 = make_double2(0.0, 0.0), ya1 = make_double2(0.0, 0.0);
-#pragma unroll 1
-    for (int i0 = 0; i0 < 8; i0 += C::CH) {
-        double x0[C::CH], x1[C::CH], y0[C::CH], y1[C::CH];
+    // the first half of the tile's x elements is requested before anything else: the table loads and the barrier below
+    // overlap its latency
+    double x0[C::CH], x1[C::CH], y0[C::CH], y1[C::CH];
+    auto load_half = [&](int i0) {
 #pragma unroll
         for (int i = 0; i < C::CH; ++i) {
             int e = tid + (i0 + i) * NT;
@@ -101,6 +94,21 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
             y0[i] = (m0 >= 1) ? __ldcs(x + N - m0 - 1) : 0.0;
             y1[i] = __ldcs(x + N - m0 - 2);
         }
+    };
+    load_half(0);
+    tw_build(lo, hi, 2 * L1, C::NHI, tid, NT);
+    for (int i = tid; i < 2 * T2; i += NT) tB[i] = __ldg(tabs.gB + 2 * j2_of(i >> 1) + (i & 1));
+    for (int i = tid; i < T2 * (C::TW_LO + C::TW_HI); i += NT) {
+        if (i < T2 * C::TW_LO) { const int s = i / C::TW_LO, kk = i % C::TW_LO; t4lo[s * C::SLO + kk] = __ldg(tabs.g4lo + (int64_t)j2_of(s) * C::TW_LO + kk); }
+        else { const int q = i - T2 * C::TW_LO, s = q / C::TW_HI, h = q % C::TW_HI; t4hi[s * C::SHI + h] = __ldg(tabs.g4hi + (int64_t)j2_of(s) * C::TW_HI + h); }
+    }
+    __syncthreads();
+    // fold: t_m = sin(pi m/N)(x_m + x_{N-m}) + (x_m - x_{N-m})/2 for m = 2j, 2j+1;  z_j = t_{2j} + i t_{2j+1}
+    // anchors: ya[b] += (x_m + x_{N-m}) e^{+i pi m/N} for m = m0 + b < L  (the thread's s = tid % T2 is the same for all its e)
+    double2 ya0 = make_double2(0.0, 0.0), ya1 = make_double2(0.0, 0.0);
+#pragma unroll 1
+    for (int i0 = 0; i0 < 8; i0 += C::CH) {
+        if (i0 > 0) load_half(i0);
 #pragma unroll
         for (int i = 0; i < C::CH; ++i) {
             int e = tid + (i0 + i) * NT;
@@ -143,6 +151,23 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
         double ar = 0.0, ai = 0.0;
         for (int q = 0; q < NT / T2; ++q) { ar += red[4 * (s + q * T2) + 2 * b]; ai += red[4 * (s + q * T2) + 2 * b + 1]; }
         __stcg(&ypart[2 * j2_of(s) + b], make_double2(ar, ai));
+    }
+}
+
+// one thread per table entry; exact arguments (powers of two), sincospi
+__global__ void dst1_tables_kernel(int log2N, int q1, double2* __restrict__ gB, double2* __restrict__ g4lo, double2* __restrict__ g4hi) {
+    const int64_t N = (int64_t)1 << log2N, L = N >> 1, L2 = L >> q1;
+    const int nhi = ((1 << q1) + 31) / 32;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nB = 2 * L2, nlo = L2 * 32, nh = L2 * nhi;
+    double sn, cs;
+    if (i < nB) { sincospi(-(double)i / (double)N, &sn, &cs); gB[i] = make_double2(cs, sn); }
+    else if (i < nB + nlo) {
+        const int64_t e = i - nB, j2 = e / 32, kk = e % 32;
+        sincospi(-2.0 * (double)((j2 * kk) & (L - 1)) / (double)L, &sn, &cs); g4lo[e] = make_double2(cs, sn);
+    } else if (i < nB + nlo + nh) {
+        const int64_t e = i - nB - nlo, j2 = e / nhi, kk = (e % nhi) * 32;
+        sincospi(-2.0 * (double)((j2 * kk) & (L - 1)) / (double)L, &sn, &cs); g4hi[e] = make_double2(cs, sn);
     }
 }
 
@@ -382,6 +407,7 @@ struct LargeArgs {
     double2* W;            // [2 gc][L]      ring of two column groups
     double2* ypart;        // [2 gc][2 L2]
     double* anchors;       // [2 gc][nch + 1]   (last entry: scale * X_{N-1})
+    ATables tabs;          // phase A twiddles (dst1_tables_kernel)
     int* counters;         // [0]: queue head; [1 + 4 col + {0,1,2,3}]: A tiles, B tiles, D, C chunks done for column col
 };
 enum { PH_A = 0, PH_B = 1, PH_D = 2, PH_C = 3, PH_DONE = 4 };
@@ -411,8 +437,15 @@ __device__ __forceinline__ void decode_item(const LargeArgs& a, int item, int& p
     phase = PH_DONE; g = 0; local = 0;
 }
 
-__device__ __forceinline__ void wait_count(const int* p, int need) {
-    while (*(volatile const int*)p < need) __nanosleep(200);
+// arrival counters: release increment by one thread after the CTA barrier (the barrier orders the other threads' writes
+// before it), acquire load by the waiting CTA's thread 0 before its barrier -- no device-wide fence per thread
+__device__ __forceinline__ void wait_count(int* p, int need) {
+    cuda::atomic_ref<int, cuda::thread_scope_device> a(*p);
+    while (a.load(cuda::memory_order_acquire) < need) __nanosleep(100);
+}
+__device__ __forceinline__ void arrive_count(int* p) {
+    cuda::atomic_ref<int, cuda::thread_scope_device> a(*p);
+    a.fetch_add(1, cuda::memory_order_release);
 }
 
 template <int Q1, int Q2, int TL> struct FusedCfg {
@@ -452,11 +485,10 @@ dst1_fused_kernel(LargeArgs a) {
             if (phase != PH_DONE) {
                 const int nt = phase == PH_A ? a.nA : (phase == PH_B ? a.nB : (phase == PH_C ? a.nC : 1));
                 col = g * a.gc + local / nt; tile = local % nt;
-                const int* cnt = a.counters + 1 + 4 * col;
+                int* cnt = a.counters + 1 + 4 * col;
                 if (phase == PH_A) { if (g >= 2) wait_count(cnt - 4 * 2 * a.gc + 3, a.nC); }          // ring slot free
                 else if (phase == PH_C) { wait_count(cnt + 1, a.nB); wait_count(cnt + 2, 1); }
                 else wait_count(cnt, a.nA);                                                            // B, D
-                __threadfence();
             }
 #ifdef LRP_DST_STATS
             { long long t = clock64(); atomicAdd(&stats[8], (unsigned long long)(t - t_prev)); atomicAdd(&stats[9], 1ull); t_prev = t; }
@@ -471,13 +503,12 @@ dst1_fused_kernel(LargeArgs a) {
         double2* yp = a.ypart + (int64_t)slot * 2 * L2;
         double* anc = a.anchors + (int64_t)slot * (nch + 1);
         const double* x = a.in + (int64_t)col * a.ld_in;
-        if (phase == PH_A) phase_a<Q1, TL>(smem_raw, a.log2N, tile, x, Wc, yp);
+        if (phase == PH_A) phase_a<Q1, TL>(smem_raw, a.log2N, tile, x, Wc, yp, a.tabs);
         else if (phase == PH_B) phase_b<Q2, TL>(smem_raw, a.log2N, tile, Wc, a.scale, anc + nch);
         else if (phase == PH_D) phase_d<NT, FusedCfg<Q1, Q2, TL>::QM>(smem_raw, a.log2N, Q1, x, yp, a.scale, anc);
         else phase_c<NT>(smem_raw, a.log2N, Q1, tile, Wc, a.out + (int64_t)col * a.ld_out, anc);
-        __threadfence();                                   // this item's global writes before the arrival below
-        __syncthreads();
-        if (tid == 0) atomicAdd(a.counters + 1 + 4 * col + phase, 1);
+        __syncthreads();                                   // every thread's global writes of this item ...
+        if (tid == 0) arrive_count(a.counters + 1 + 4 * col + phase);      // ... are released by this increment
 #ifdef LRP_DST_STATS
         if (tid == 0) { long long t = clock64(); atomicAdd(&stats[2 * phase], (unsigned long long)(t - t_prev)); atomicAdd(&stats[2 * phase + 1], 1ull); t_prev = t; }
 #endif
@@ -535,7 +566,8 @@ size_t dst1_large_ws(int64_t N, int32_t batch) {
     const int64_t L = N / 2;
     const Plan p = plan(lrp_ilog2(N));
     const int64_t L2 = (int64_t)1 << p.q2;
-    return lrp_align_up((size_t)2 * gc * L * sizeof(double2)) + lrp_align_up((size_t)2 * gc * 2 * L2 * sizeof(double2)) +
+    const size_t tab = (size_t)(2 * L2 + L2 * 32 + L2 * (((int64_t)1 << p.q1) + 31) / 32);
+    return lrp_align_up(tab * sizeof(double2)) + lrp_align_up((size_t)2 * gc * L * sizeof(double2)) + lrp_align_up((size_t)2 * gc * 2 * L2 * sizeof(double2)) +
            lrp_align_up((size_t)2 * gc * (p.nC + 1) * sizeof(double)) + lrp_align_up((size_t)(1 + 4 * (size_t)batch + 32) * sizeof(int));
 }
 
@@ -558,6 +590,10 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
     a.nA = p.nA; a.nB = p.nB; a.nC = p.nC;
     a.in = d_in; a.ld_in = ld_in; a.out = d_out; a.ld_out = ld_out; a.scale = scale;
     lrp_arena ar(ws, ws_bytes);
+    const int64_t nhi = (((int64_t)1 << p.q1) + 31) / 32;
+    const int64_t ntab = 2 * L2 + L2 * 32 + L2 * nhi;
+    double2* twt = ar.take<double2>((size_t)ntab);
+    a.tabs.gB = twt; a.tabs.g4lo = twt + 2 * L2; a.tabs.g4hi = twt + 2 * L2 + L2 * 32;
     a.W = ar.take<double2>((size_t)2 * a.gc * L);
     a.ypart = ar.take<double2>((size_t)2 * a.gc * 2 * L2);
     a.anchors = ar.take<double>((size_t)2 * a.gc * (p.nC + 1));
@@ -574,6 +610,11 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
 #ifdef LRP_DST_STATS
     g_dbg_counters = a.counters; g_dbg_batch = batch;
 #endif
+    {
+        LRP_PROF(ctx, K_DST_FUSED, 0, 0);
+        dst1_tables_kernel<<<(unsigned)((ntab + 255) / 256), 256, 0, ctx->stream>>>(log2N, p.q1, twt, twt + 2 * L2, twt + 2 * L2 + L2 * 32);
+        LRP_LAUNCHED(ctx);
+    }
     LRP_PROF(ctx, K_DST_FUSED, 16.0 * (double)N * batch, 0);
     ke->fn<<<(unsigned)grid, ke->nt, ke->smem, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);

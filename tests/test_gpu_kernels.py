@@ -91,10 +91,11 @@ def test_dst1_leading_dimension_and_errors(ctx):
     view = big[:, :n]
     out = ctx.dst1_batched(view)
     assert _rel(lrp.tall_to_numpy(out), O.dst1(x)) < 1e-12
-    bad = torch.zeros((2, 1000), dtype=torch.float64, device="cuda")
-    with pytest.raises(lrp.LrpError) as e:
-        ctx.dst1_batched(bad)
-    assert e.value.code == lrp.LRP_ERR_UNSUPPORTED_N
+    # n + 1 need not be a power of two (Bluestein, tests/test_gpu_general_n.py); beyond 2^23 it is refused
+    import ctypes as C
+    rc = ctx.lib.lrp_dst1_batched(ctx.h, (1 << 23) + 1, 1, C.c_void_p(big.data_ptr()), (1 << 23) + 1, C.c_void_p(big.data_ptr()),
+                                  (1 << 23) + 1, 1.0)
+    assert rc == lrp.LRP_ERR_UNSUPPORTED_N
     empty = torch.zeros((0, n), dtype=torch.float64, device="cuda")
     assert ctx.dst1_batched(empty).shape == (0, n)
 
