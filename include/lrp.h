@@ -44,6 +44,7 @@ extern "C" {
 #define LRP_ERR_UNSUPPORTED_N  -2   /* n out of range (see above) */
 #define LRP_ERR_WORKSPACE      -3   /* workspace missing or too small */
 #define LRP_ERR_CUDA           -4   /* a CUDA call failed; see lrp_last_cuda_error */
+#define LRP_ERR_STATIC_LIMIT   -5   /* lrp_topk_static: n or num_select beyond the fixed capacity of its built-in scratch */
 #define LRP_WARN_NOCONV         1   /* Cross-DEIM reached max_sweeps (or r* > max_rank): outputs valid, tolerance not certified */
 
 #define LRP_MAX_SWEEPS_INFO    32   /* per-sweep arrays in lrp_solve_info hold this many sweeps */
@@ -250,6 +251,22 @@ int lrp_dense_poisson(lrp_ctx* ctx, int64_t n, const double* d_F, int64_t ldf, d
 int lrp_lowrank_entries(lrp_ctx* ctx, int64_t n, int32_t r, const double* d_U, int64_t ldu, const double* d_S,
                         const double* d_V, int64_t ldv, const int64_t* d_rows, const int64_t* d_cols,
                         int64_t count, double* d_out);
+
+/* Allocation-free top-k (the index selection of Alg. 3 line 6, deterministic form, reading Q5) for
+ * callers that cannot call cudaMalloc or own a workspace (CUDA graph capture, serving loops, harnesses that forbid it):
+ *     d_idx_out[0..num_select) = the indices of the num_select largest d_scores[0..n), ordered by (score descending,
+ *     index ascending) -- bit-identical to what lrp_leverage_select returns for the same scores.
+ * No ctx and no workspace: the candidate buffers of the multi-level sort live in a 1.6 MB device array built into the
+ * library (held by every GPU that loads it until the process exits).  Limits: n <= LRP_TOPK_STATIC_MAX_N,
+ * num_select <= LRP_TOPK_STATIC_MAX_NUM, else LRP_ERR_STATIC_LIMIT.  The call allocates nothing and frees nothing.  The
+ * FIRST call on a device looks up the array's device address (do it once outside a capture); the device that owns
+ * `cuda_stream` (a cudaStream_t, NULL = legacy default stream) must be current.  d_scores (n doubles, 8-byte aligned) and
+ * d_idx_out (num_select int32) are device pointers owned by the caller.  Asynchronous on `cuda_stream`.
+ * All calls share the one array: calls that overlap on the GPU (different streams or host threads) race -- serialise them.
+ * Errors: BADARG (null / misaligned pointer, n < 1, num_select < 0 or > n), STATIC_LIMIT, CUDA. */
+#define LRP_TOPK_STATIC_MAX_N    4194304
+#define LRP_TOPK_STATIC_MAX_NUM  256
+int lrp_topk_static(void* cuda_stream, int64_t n, const double* d_scores, int32_t num_select, int32_t* d_idx_out);
 
 #ifdef __cplusplus
 }

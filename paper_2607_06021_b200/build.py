@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "liblrp.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["dst1.cu", "dst1_large.cu", "dst1_bluestein.cu", "tall.cu", "tall_mma.cu", "qr.cu", "core.cu", "select.cu", "deim.cu", "peak.cu", "api.cu"]
+SOURCES = ["dst1.cu", "dst1_large.cu", "dst1_bluestein.cu", "tall.cu", "tall_mma.cu", "qr.cu", "core.cu", "select.cu", "deim.cu", "peak.cu", "topk_static.cu", "api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-warn-spills"]
 

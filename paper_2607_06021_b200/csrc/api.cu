@@ -318,6 +318,7 @@ const char* lrp_strerror(int code) {
         case LRP_ERR_UNSUPPORTED_N: return "n out of range: n + 1 a power of two <= 2^25, or any n + 1 <= 2^23";
         case LRP_ERR_WORKSPACE: return "workspace missing or too small";
         case LRP_ERR_CUDA: return "CUDA error (see lrp_last_cuda_error)";
+        case LRP_ERR_STATIC_LIMIT: return "size beyond the fixed capacity of the built-in scratch (n <= 4194304, num_select <= 256)";
         case LRP_WARN_NOCONV: return "warning: stop test not passed within max_sweeps";
         default: return "unknown code";
     }

@@ -19,6 +19,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblrp.so")
 
 LRP_OK, LRP_ERR_BADARG, LRP_ERR_UNSUPPORTED_N, LRP_ERR_WORKSPACE, LRP_ERR_CUDA, LRP_WARN_NOCONV = 0, -1, -2, -3, -4, 1
+LRP_ERR_STATIC_LIMIT = -5
+TOPK_STATIC_MAX_N, TOPK_STATIC_MAX_NUM = 4194304, 256
 MAX_SWEEPS_INFO = 32
 LRP_FLAG_NO_QR_REUSE, LRP_FLAG_NO_NESTED_RHO, LRP_FLAG_NO_FUSED_RHO = 1, 2, 4
 LRP_G_POISSON, LRP_G_HILBERT, LRP_G_KMATRIX = 0, 1, 2
@@ -31,7 +33,7 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
            "lrp_profile_timeline", "lrp_fp64_peak", "lrp_matrix_workspace_bytes", "lrp_cross_deim_matrix",
-           "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson"]
+           "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson", "lrp_topk_static"]
 
 
 class SolveOpts(C.Structure):
@@ -98,6 +100,7 @@ def load_library():
     lib.lrp_dense_poisson.argtypes = [vp, i64, vp, i64, vp, i64]; lib.lrp_dense_poisson.restype = C.c_int
     lib.lrp_lowrank_entries.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_lowrank_entries.restype = C.c_int
+    lib.lrp_topk_static.argtypes = [vp, i64, vp, i32, vp]; lib.lrp_topk_static.restype = C.c_int
     lib.lrp_profile_enable.argtypes = [vp, C.c_int]; lib.lrp_profile_enable.restype = C.c_int
     lib.lrp_profile_timeline.argtypes = [vp, C.c_char_p]; lib.lrp_profile_timeline.restype = C.c_int
     lib.lrp_profile_reset.argtypes = [vp]; lib.lrp_profile_reset.restype = C.c_int
@@ -145,6 +148,23 @@ def _check_tall(t, name):
         raise ValueError(f"{name}: expected a CUDA float64 tensor of shape (cols, n) with contiguous rows")
     ld = t.stride(0) if t.shape[0] > 1 else t.shape[1]
     return t.shape[0], t.shape[1], max(ld, t.shape[1])
+
+
+def topk_static(scores, num_select: int, out, stream=None):
+    """lrp_topk_static (include/lrp.h): allocation-free top-k into the caller's `out` (int32, >= num_select elements) on
+    `stream` (a torch.cuda.Stream, default: the current one).  n <= TOPK_STATIC_MAX_N, num_select <= TOPK_STATIC_MAX_NUM.
+    The library keeps one built-in scratch array per GPU: overlapping calls race."""
+    torch = _torch()
+    if not (scores.is_cuda and scores.dtype == torch.float64 and scores.dim() == 1 and scores.is_contiguous()):
+        raise ValueError("scores: contiguous 1-D float64 CUDA tensor")
+    if not (out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() >= num_select):
+        raise ValueError("out: contiguous int32 CUDA tensor with room for num_select indices")
+    st = stream if stream is not None else torch.cuda.current_stream(scores.device)
+    with torch.cuda.device(scores.device):
+        rc = load_library().lrp_topk_static(C.c_void_p(st.cuda_stream), scores.numel(), _ptr(scores), int(num_select), _ptr(out))
+    if rc < 0:
+        raise LrpError(rc, "lrp_topk_static")
+    return out[:num_select]
 
 
 class Context:
