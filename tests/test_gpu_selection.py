@@ -35,6 +35,25 @@ def test_topk_matches_full_sort(ctx, n, num):
     assert idx.cpu().numpy().tolist() == ref.tolist()
 
 
+@pytest.mark.parametrize("n,num,kind", [(100_000, 50, "flat"), ((1 << 20) - 1, 300, "flat"), (300_000, 4096, "two_levels"),
+                                        (50_000, 64, "narrow"), (9000, 9000 // 3, "flat")])
+def test_topk_flat_distributions_take_the_multi_level_sort(ctx, n, num, kind):
+    """More than 4096 keys share the threshold bin of the histogram pass (equal scores; scores within one 2^(1/4) band):
+    the device-side flag routes the call to the multi-level sort.  Same bit-exact order."""
+    from paper_2607_06021_b200 import lrp
+    rng = np.random.default_rng(n)
+    if kind == "flat":
+        sc = np.full(n, 0.25)
+    elif kind == "narrow":
+        sc = 0.5 + 0.01 * rng.random(n)                                   # all inside one bin, no ties
+    else:
+        sc = np.where(np.arange(n) % 7 == 0, 0.5, 0.25 + 1e-3 * rng.random(n))   # 1/7 in a higher bin (> 4096 of them), rest flat
+    A = np.sqrt(sc)[:, None]
+    idx, got_sc = ctx.leverage_select(lrp.tall_from_numpy(A), num, assume_orthonormal=True)
+    ref = O.top_select(got_sc.cpu().numpy(), num)
+    assert idx.cpu().numpy().tolist() == ref.tolist()
+
+
 def _solve(ctx, w, **kw):
     import torch
     from paper_2607_06021_b200 import lrp
