@@ -10,7 +10,7 @@
 
 namespace {
 
-constexpr int CORE_NT = 1024;
+constexpr int CORE_NT = 512;
 constexpr int JACOBI_MAX_SWEEPS = 60;
 
 // 1/sqrt(x) and 1/x for normal positive x to ~1 ulp, branch free: the hardware seed (MUFU.RSQ64H / RCP64H, ~22 bits)
@@ -32,64 +32,151 @@ __device__ __forceinline__ double fast_rcp(double x) {
     return fma(y, e, y);
 }
 
+// Column access of the small dense kernels.  SH: the pointer is known to lie in shared memory -- explicit ld.shared /
+// st.shared through the 32-bit window address (a generic LD / ST would be emitted otherwise: the working set is chosen
+// between shared and global memory at run time).
+template <bool SH> struct ColPtr {
+    double* g; unsigned s;
+    __device__ __forceinline__ explicit ColPtr(double* p) : g(p), s(SH ? (unsigned)__cvta_generic_to_shared(p) : 0u) {}
+    __device__ __forceinline__ double ld(int t) const {
+        if (SH) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(s + 8u * (unsigned)t)); return v; }
+        return g[t];
+    }
+    __device__ __forceinline__ void st(int t, double v) const {
+        if (SH) asm volatile("st.shared.f64 [%0], %1;" :: "r"(s + 8u * (unsigned)t), "d"(v) : "memory");
+        else g[t] = v;
+    }
+};
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
     return v;
 }
 
-// One pair (p, q) of the sweep with the two columns in registers (JR rows per lane: m <= 32 JR) from the dot product to
-// the rotated store -- one shared-memory read and one write per element.  Returns false when the pair is converged.
-template <int JR>
-__device__ __forceinline__ bool jacobi_pair_regs(double* ap, double* aq, int m, double* V, int ldv, int n, int p, int q,
-                                             double al, double be, int lane, double& aln_out, double& ben_out) {
-    double x[JR], y[JR];
-    double ga = 0.0;
-#pragma unroll
-    for (int u = 0; u < JR; ++u) {
-        const int t = lane + 32 * u;
-        x[u] = t < m ? ap[t] : 0.0; y[u] = t < m ? aq[t] : 0.0;
-        ga = fma(x[u], y[u], ga);
-    }
-    ga = warp_sum(ga);
-    if (ga == 0.0 || ga * ga <= (DBL_EPSILON * DBL_EPSILON) * (al * be)) return false;
-    const double dd = be - al, g2 = 2.0 * ga;
-    const double q2 = fma(dd, dd, g2 * g2);
-    const double hh = q2 * fast_rsqrt(q2);
-    const double tt = copysign(1.0, dd) * g2 * fast_rcp(fabs(dd) + hh);
-    const double c = fast_rsqrt(fma(tt, tt, 1.0)), s = c * tt;
-    double aln = fma(-tt, ga, al), ben = fma(tt, ga, be);
-    const bool redo = !(aln > 1e-4 * al) || !(ben > 1e-4 * be);  // cancellation: recompute exactly
-    double sa = 0.0, sb = 0.0;
-#pragma unroll
-    for (int u = 0; u < JR; ++u) {
-        const int t = lane + 32 * u;
-        const double xn = c * x[u] - s * y[u], yn = s * x[u] + c * y[u];
-        if (t < m) { ap[t] = xn; aq[t] = yn; }
-        sa = fma(xn, xn, sa); sb = fma(yn, yn, sb);
-    }
-    if (redo) {
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            sa += __shfl_xor_sync(0xffffffffu, sa, d);
-            sb += __shfl_xor_sync(0xffffffffu, sb, d);
+// One round of the tournament with G lanes per column pair (32 / G pairs per warp, JR rows per lane: m <= G JR).  The
+// two columns, the two columns of V and the two running norms are all requested up front and stay in registers until
+// the rotated stores; the reductions take log2(G) shuffles and one warp instruction serves 32 / G pairs.  A round is the
+// dependent chain of one pair (load, dot, reduce, rotation parameters, rotate, store, barrier): measured 1350-1900
+// cycles per round at 57 x 56 whatever G (profiles/r02_core_jacobi.md); G = 16 is the fastest by a few per cent.
+// SH: A, V and nrm2 are in shared memory -- explicit ld.shared / st.shared (ColPtr) instead of generic accesses.
+// Pairs of a round are disjoint: no ordering inside it.
+template <int G, int JR, bool SH>
+__device__ __forceinline__ void jacobi_round_sub(double* __restrict__ A, int lda, int m, int n, double* __restrict__ V, int ldv,
+                                                 double* __restrict__ nrm2, int np, int r, int* s_flag) {
+    constexpr int GPW = 32 / G;
+    const int tid = threadIdx.x, lane = tid & 31, gl = lane & (G - 1);
+    const int ngroups = (blockDim.x >> 5) * GPW;
+    const bool hasV = V != nullptr;
+    for (int i0 = (tid >> 5) * GPW; i0 < np / 2; i0 += ngroups) {          // warp-uniform bounds
+        const int i = i0 + lane / G;
+        int p = 0, q = 0;
+        bool act = i < np / 2;
+        if (act) {
+            if (i == 0) { p = np - 1; q = r; }
+            else {
+                p = r + i; if (p >= np - 1) p -= np - 1;
+                q = r - i; if (q < 0) q += np - 1;
+            }
+            if (p > q) { const int t = p; p = q; q = t; }
+            act = q < n;
         }
-        aln = sa; ben = sb;
-    }
-    if (V != nullptr) {
-        double* vp = V + (size_t)p * ldv;
-        double* vq = V + (size_t)q * ldv;
+        if (!act) { p = 0; q = 0; }                                         // inactive groups read column 0, write nothing
+        const ColPtr<SH> ap(A + (size_t)p * lda), aq(A + (size_t)q * lda), nr(nrm2);
+        const ColPtr<SH> vp(hasV ? V + (size_t)p * ldv : A), vq(hasV ? V + (size_t)q * ldv : A);
+        double x[JR], y[JR], xv[JR], yv[JR];
 #pragma unroll
         for (int u = 0; u < JR; ++u) {
-            const int t = lane + 32 * u;
-            if (t < n) {
-                const double xv = vp[t], yv = vq[t];
-                vp[t] = c * xv - s * yv; vq[t] = s * xv + c * yv;
+            const int t = gl + G * u;
+            const bool in = t < m;
+            x[u] = in ? ap.ld(t) : 0.0; y[u] = in ? aq.ld(t) : 0.0;
+        }
+        const double al = nr.ld(p), be = nr.ld(q);
+        if (hasV) {
+#pragma unroll
+            for (int u = 0; u < JR; ++u) {
+                const int t = gl + G * u;
+                const bool in = t < n;
+                xv[u] = in ? vp.ld(t) : 0.0; yv[u] = in ? vq.ld(t) : 0.0;
             }
         }
+        double ga0 = 0.0, ga1 = 0.0;
+#pragma unroll
+        for (int u = 0; u < JR; u += 2) { ga0 = fma(x[u], y[u], ga0); if (u + 1 < JR) ga1 = fma(x[u + 1], y[u + 1], ga1); }
+        double ga = ga0 + ga1;
+#pragma unroll
+        for (int d = G / 2; d > 0; d >>= 1) ga += __shfl_xor_sync(0xffffffffu, ga, d);
+        const bool rot = act && !(ga == 0.0 || ga * ga <= (DBL_EPSILON * DBL_EPSILON) * (al * be));
+        if (!__any_sync(0xffffffffu, rot)) continue;
+        // t = sign(d) g2 / (|d| + hypot(d, g2)), d = be - al, g2 = 2 ga;  c = 1/sqrt(1 + t^2), s = c t
+        const double dd = be - al, g2 = 2.0 * ga;
+        const double q2 = fma(dd, dd, g2 * g2);
+        const double hh = q2 * fast_rsqrt(rot ? q2 : 1.0);
+        const double tt = copysign(1.0, dd) * g2 * fast_rcp(rot ? fabs(dd) + hh : 1.0);
+        const double c = fast_rsqrt(fma(tt, tt, 1.0)), sn = c * tt;
+        double aln = fma(-tt, ga, al), ben = fma(tt, ga, be);
+        const bool redo = rot && (!(aln > 1e-4 * al) || !(ben > 1e-4 * be));   // cancellation: recompute exactly
+#pragma unroll
+        for (int u = 0; u < JR; ++u) {
+            const double xn = c * x[u] - sn * y[u], yn = sn * x[u] + c * y[u];
+            x[u] = xn; y[u] = yn;
+        }
+        if (__any_sync(0xffffffffu, redo)) {
+            double sa = 0.0, sb = 0.0, sa1 = 0.0, sb1 = 0.0;
+#pragma unroll
+            for (int u = 0; u < JR; u += 2) {
+                sa = fma(x[u], x[u], sa); sb = fma(y[u], y[u], sb);
+                if (u + 1 < JR) { sa1 = fma(x[u + 1], x[u + 1], sa1); sb1 = fma(y[u + 1], y[u + 1], sb1); }
+            }
+            sa += sa1; sb += sb1;
+#pragma unroll
+            for (int d = G / 2; d > 0; d >>= 1) {
+                sa += __shfl_xor_sync(0xffffffffu, sa, d);
+                sb += __shfl_xor_sync(0xffffffffu, sb, d);
+            }
+            if (redo) { aln = sa; ben = sb; }
+        }
+        if (rot) {
+#pragma unroll
+            for (int u = 0; u < JR; ++u) {
+                const int t = gl + G * u;
+                if (t < m) { ap.st(t, x[u]); aq.st(t, y[u]); }
+            }
+            if (hasV) {
+#pragma unroll
+                for (int u = 0; u < JR; ++u) {
+                    const int t = gl + G * u;
+                    if (t < n) { vp.st(t, c * xv[u] - sn * yv[u]); vq.st(t, sn * xv[u] + c * yv[u]); }
+                }
+            }
+            if (gl == 0) { nr.st(p, aln); nr.st(q, ben); *s_flag = 1; }
+        }
     }
-    aln_out = aln; ben_out = ben;
-    return true;
+}
+
+// the whole Jacobi iteration for m <= G JR (one compiled body per shape class; see cta_jacobi for the contract)
+template <int G, int JR, bool SH>
+__device__ __noinline__ void cta_jacobi_sub(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag, double* nrm2) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int np = (n + 1) & ~1;
+    for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
+        if (tid == 0) *s_flag = 0;
+        for (int c = warp; c < n; c += nwarps) {
+            const double* ac = A + (size_t)c * lda;
+            double acc = 0.0;
+            for (int t = lane; t < m; t += 32) acc = fma(ac[t], ac[t], acc);
+            acc = warp_sum(acc);
+            if (lane == 0) nrm2[c] = acc;
+        }
+        __syncthreads();
+        for (int r = 0; r < np - 1; ++r) {
+            jacobi_round_sub<G, JR, SH>(A, lda, m, n, V, ldv, nrm2, np, r, s_flag);
+            __syncthreads();
+        }
+        const int again = *s_flag;
+        __syncthreads();
+        if (!again) break;
+    }
 }
 
 // One-sided Jacobi on A (m x n, m >= n, ld lda), accumulating the rotations into V (n x n, ld ldv, must be I on
@@ -97,10 +184,22 @@ __device__ __forceinline__ bool jacobi_pair_regs(double* ap, double* aq, int m, 
 // A = U diag(s), columns orthogonal.  nrm2 (n doubles, shared or global): squared column norms, recomputed at the
 // start of every sweep and updated by the rotation formulas in between (al' = al - t ga, be' = be + t ga), with an
 // explicit recomputation whenever the update cancels (so a pair costs one dot product instead of three).
-__device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag, double* nrm2) {
+__device__ __noinline__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv, int* s_flag, double* nrm2, bool sh = false) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int np = (n + 1) & ~1;                 // players (padded to even)
     if (n < 2) return;
+    if (m <= 128) {
+        if (sh) {
+            if (m <= 32) cta_jacobi_sub<8, 4, true>(A, lda, m, n, V, ldv, s_flag, nrm2);
+            else if (m <= 64) cta_jacobi_sub<16, 4, true>(A, lda, m, n, V, ldv, s_flag, nrm2);
+            else cta_jacobi_sub<16, 8, true>(A, lda, m, n, V, ldv, s_flag, nrm2);
+        } else {
+            if (m <= 32) cta_jacobi_sub<8, 4, false>(A, lda, m, n, V, ldv, s_flag, nrm2);
+            else if (m <= 64) cta_jacobi_sub<16, 4, false>(A, lda, m, n, V, ldv, s_flag, nrm2);
+            else cta_jacobi_sub<16, 8, false>(A, lda, m, n, V, ldv, s_flag, nrm2);
+        }
+        return;
+    }
     for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS; ++sweep) {
         if (tid == 0) *s_flag = 0;
         for (int c = warp; c < n; c += nwarps) {
@@ -124,14 +223,6 @@ __device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv,
                 double* ap = A + (size_t)p * lda;
                 double* aq = A + (size_t)q * lda;
                 const double al = nrm2[p], be = nrm2[q];
-                if (m <= 128) {
-                    double aln, ben;
-                    const bool rot = m <= 64 ? jacobi_pair_regs<2>(ap, aq, m, V, ldv, n, p, q, al, be, lane, aln, ben)
-                                             : jacobi_pair_regs<4>(ap, aq, m, V, ldv, n, p, q, al, be, lane, aln, ben);
-                    if (!rot) continue;
-                    if (lane == 0) { nrm2[p] = aln; nrm2[q] = ben; *s_flag = 1; }
-                    continue;
-                }
                 double ga = 0.0;
                 for (int t = lane; t < m; t += 32) ga = fma(ap[t], aq[t], ga);
                 ga = warp_sum(ga);
@@ -181,7 +272,7 @@ __device__ void cta_jacobi(double* A, int lda, int m, int n, double* V, int ldv,
 
 // Thin SVD of M (m x n, ld ldm): U (m x p), s (p, descending), V (n x p), p = min(m, n).
 // work: max(m,n)*p + p*p + p doubles, iwork: p ints.  Columns of U for exactly-zero singular values are zero.
-__device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int ldu, double* s, double* V, int ldv,
+__device__ __noinline__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int ldu, double* s, double* V, int ldv,
                         double* work, int* iwork, int* s_flag, double* sm = nullptr, int sm_doubles = 0,
                         bool vectors = true) {
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -200,7 +291,7 @@ __device__ void cta_svd(const double* M, int ldm, int m, int n, double* U, int l
     }
     if (vectors) for (int e = tid; e < p * p; e += nt) W[e] = (e % p == e / p) ? 1.0 : 0.0;
     __syncthreads();
-    cta_jacobi(A, T, T, p, vectors ? W : nullptr, p, s_flag, nrm2);
+    cta_jacobi(A, T, T, p, vectors ? W : nullptr, p, s_flag, nrm2, in_smem);
     __syncthreads();
     {   // column norms, one warp per column
         const int lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
@@ -253,17 +344,20 @@ __device__ void cta_matmul(double* C, int ldc, int m, int n, int kk, const doubl
 // Y (xn x nb, ld ldy) = R^-1 (Q^T B)(0:xn, :).  Equals pinv(X) B when X has full column rank, which is how the
 // pseudo-inverse of Alg. 1 lines 5-14 is applied when X is well conditioned ("\" in the paper);
 // *cond_flag is set to 1 when min|R_cc| < 1e-8 max|R_cc| (the caller then takes the SVD pseudo-inverse instead).
-__device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb, double* Y, int ldy,
-                                   double* s_scal, int* cond_flag) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+template <int G, bool SH>
+__device__ __noinline__ void cta_ls_householder_t(double* __restrict__ W, int ldw, int rows, int xn, int nb, double* __restrict__ Y, int ldy,
+                                                  double* s_scal, int* cond_flag) {
+    constexpr int GPW = 32 / G;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gl = lane & (G - 1);
+    const int ngroups = (blockDim.x >> 5) * GPW;
     const int ncol = xn + nb;
     for (int c = 0; c < xn; ++c) {
-        double* xc = W + (size_t)c * ldw;
+        const ColPtr<SH> xc(W + (size_t)c * ldw);
         if (warp == 0) {
             double sig = 0.0;
-            for (int r = c + 1 + lane; r < rows; r += 32) sig = fma(xc[r], xc[r], sig);
+            for (int r = c + 1 + lane; r < rows; r += 32) { const double v = xc.ld(r); sig = fma(v, v, sig); }
             sig = warp_sum(sig);
-            const double alpha = xc[c];
+            const double alpha = xc.ld(c);
             double beta, tau, inv;
             if (sig == 0.0) { beta = alpha; tau = 0.0; inv = 0.0; }
             else {
@@ -273,19 +367,25 @@ __device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb,
                 tau = fma(aa, rs, 1.0);                                      // (beta - alpha) / beta
                 inv = copysign(fast_rcp(aa + mu), alpha);                    // 1 / (alpha - beta)
             }
-            for (int r = c + 1 + lane; r < rows; r += 32) xc[r] *= inv;       // v (unit diagonal implicit)
-            if (lane == 0) { xc[c] = beta; s_scal[0] = tau; }
+            for (int r = c + 1 + lane; r < rows; r += 32) xc.st(r, xc.ld(r) * inv);   // v (unit diagonal implicit)
+            if (lane == 0) { xc.st(c, beta); s_scal[0] = tau; }
         }
         __syncthreads();
         const double tau = s_scal[0];
-        for (int j = c + 1 + warp; j < ncol; j += nwarps) {
-            double* aj = W + (size_t)j * ldw;
+        // one column per group of G lanes: 32 / G columns per warp instruction
+        for (int j0 = c + 1 + warp * GPW; j0 < ncol; j0 += ngroups) {        // warp-uniform bounds
+            const int j = j0 + lane / G;
+            const bool act = j < ncol;
+            const ColPtr<SH> aj(W + (size_t)(act ? j : c + 1) * ldw);
             double acc = 0.0;
-            for (int r = c + 1 + lane; r < rows; r += 32) acc = fma(xc[r], aj[r], acc);
-            acc = warp_sum(acc);
-            const double w = tau * (aj[c] + acc);
-            for (int r = c + 1 + lane; r < rows; r += 32) aj[r] = fma(-xc[r], w, aj[r]);
-            if (lane == 0) aj[c] -= w;
+            for (int r = c + 1 + gl; r < rows; r += G) acc = fma(xc.ld(r), aj.ld(r), acc);
+#pragma unroll
+            for (int d = G / 2; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+            if (act) {
+                const double w = tau * (aj.ld(c) + acc);
+                for (int r = c + 1 + gl; r < rows; r += G) aj.st(r, fma(-xc.ld(r), w, aj.ld(r)));
+                if (gl == 0) aj.st(c, aj.ld(c) - w);
+            }
         }
         __syncthreads();
     }
@@ -314,6 +414,20 @@ __device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb,
         Y[i + (size_t)j * ldy] = W[i + (size_t)(xn + j) * ldw];
     }
     __syncthreads();
+}
+
+// sh: W is in shared memory (LDS / STS instead of generic accesses)
+__device__ void cta_ls_householder(double* W, int ldw, int rows, int xn, int nb, double* Y, int ldy,
+                                   double* s_scal, int* cond_flag, bool sh) {
+    if (sh) {
+        if (rows <= 64) cta_ls_householder_t<8, true>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+        else if (rows <= 128) cta_ls_householder_t<16, true>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+        else cta_ls_householder_t<32, true>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+    } else {
+        if (rows <= 64) cta_ls_householder_t<8, false>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+        else if (rows <= 128) cta_ls_householder_t<16, false>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+        else cta_ls_householder_t<32, false>(W, ldw, rows, xn, nb, Y, ldy, s_scal, cond_flag);
+    }
 }
 
 // ----------------------------------------------------------------------------------------------------------
@@ -359,7 +473,7 @@ scross_core_kernel(CoreArgs a) {
                 Wls[i + (size_t)(xn + j) * ldw] = Ro[j + (size_t)i * ldo];
             }
             __syncthreads();
-            cta_ls_householder(Wls, ldw, xm, xn, xm, P, xn, s_scal, &s_cond);   // Y (xn x xm) into P's storage
+            cta_ls_householder(Wls, ldw, xm, xn, xm, P, xn, s_scal, &s_cond, fits);   // Y (xn x xm) into P's storage
         } else {
             if (tid == 0) s_cond = 1;
             __syncthreads();
