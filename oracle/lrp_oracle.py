@@ -2,7 +2,7 @@
 
 TEST INFRASTRUCTURE ONLY.  Plain, slow, fp64 numpy restatement of what the hot path
 computes, written from PAPER.md (citations are `PAPER.md:<line>` + section/algorithm) under the
-readings Q1..Q22 of SURVEY.md §8(c) (repeated in DESIGN.md).  It shares no code with the CUDA
+readings Q1..Q22 of SURVEY.md §8(c) and Q23..Q26, R1..R7 of DESIGN.md section 2.  It shares no code with the CUDA
 path, imports nothing from `paper_2607_06021_b200`, and may only be imported by `tests/`,
 `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference` leg.
 
@@ -14,8 +14,9 @@ independent pin).
 
 Parity pins (tests/test_oracle_*.py, `-m "not gpu"`): every function below is pinned by closed
 forms / invariants / brute force as listed in DESIGN.md §"Oracle pins".
-Parity unpinned: the *choice* of the constants PINV_RCOND, RANK_RCOND, PRUNE_REL, K_cap and
-the initial guess U0=Uhat_F (paper silent; validated only by convergence to the dense
+Parity unpinned: the *choice* of the constants PINV_RCOND, RANK_RCOND, PRUNE_REL, K_cap, the
+initial guess U0=Uhat_F, the Bernoulli constant c = cols + p_os (Q23) and the random initial guess
+of the test-matrix runs (Q25) (paper silent; validated only by convergence to the dense
 definition), and the paper's seed-dependent iteration counts (figures only).
 """
 from __future__ import annotations
