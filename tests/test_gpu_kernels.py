@@ -56,20 +56,21 @@ def test_dst1_four_step_regime(ctx, n):
     assert _rel(lrp.tall_to_numpy(t), x) < 1e-12
 
 
-@pytest.mark.parametrize("p", [20, 22])
+@pytest.mark.parametrize("p", [20, 22, 24, 25])
 def test_dst1_full_size_sampled(ctx, p):
-    """BASELINE sizes n = 2^20-1, 2^22-1: sampled outputs against the O(n) definition sum per entry."""
+    """BASELINE sizes n = 2^20-1, 2^22-1 and the largest sizes the call accepts (2^24-1, 2^25-1): sampled outputs against
+    the O(n) definition sum per entry."""
     import torch
     from paper_2607_06021_b200 import lrp
     n = (1 << p) - 1
-    batch = 3
+    batch = 3 if p <= 22 else (2 if p == 24 else 1)
     x = W.dst_batch(n, batch, seed=p)
     t = lrp.tall_from_numpy(x)
     out = ctx.dst1_batched(t)
     torch.cuda.synchronize()
     got = out.cpu().numpy()
     rng = np.random.default_rng(p)
-    ks = np.concatenate([[1, 2, 3, n - 1, n, (n + 1) // 2, (n + 1) // 2 + 1], rng.integers(1, n + 1, 25)])
+    ks = np.concatenate([[1, 2, 3, n - 1, n, (n + 1) // 2, (n + 1) // 2 + 1], rng.integers(1, n + 1, 25 if p <= 22 else 3)])
     for c in range(batch):
         ref = O.dst1_entries(x[:, c], ks)
         scale = np.abs(got[c]).max()
