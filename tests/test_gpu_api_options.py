@@ -136,6 +136,25 @@ def test_qr_prefix_reuse_matches_full_factorization(ctx, cfg, seed, nred):
     assert a["info"].launches < b["info"].launches
 
 
+@pytest.mark.parametrize("cfg,seed,nred", [("C2", 0, None), ("C3", 0, 16383), ("C4", 0, 32767), ("C4", 1, 262143)])
+def test_cholesky_qr_leverage_of_the_initial_guess_matches_householder(ctx, cfg, seed, nred):
+    """Leverage scores are the diagonal of the projector onto span(U_0) (Alg. 3 lines 1-3): whichever
+    orthonormal basis is used.  The driver takes CholeskyQR2 for a well-conditioned initial guess (reading R8)
+    and the Householder TSQR otherwise (LRP_FLAG_NO_CHOLQR_LEVERAGE forces it): same first selection, same run."""
+    from paper_2607_06021_b200 import lrp
+    w = W.make(cfg, seed) if nred is None else W.make(cfg, seed, nred)
+    a = _solve(ctx, w)
+    b = _solve(ctx, w, flags=lrp.LRP_FLAG_NO_CHOLQR_LEVERAGE)
+    assert list(a["trace"][0]["I"]) == list(b["trace"][0]["I"]) and list(a["trace"][0]["J"]) == list(b["trace"][0]["J"])
+    assert a["sweeps"] == b["sweeps"] and a["rank"] == b["rank"] and a["converged"] == b["converged"]
+    rows, cols = W.sample_pairs(w.n, 4096, seed=5)
+    ea = _entries(lrp.tall_to_numpy(a["UW"]), a["SW"].cpu().numpy(), lrp.tall_to_numpy(a["VW"]), rows, cols)
+    eb = _entries(lrp.tall_to_numpy(b["UW"]), b["SW"].cpu().numpy(), lrp.tall_to_numpy(b["VW"]), rows, cols)
+    tol = 1e-10 if (a["converged"] and b["converged"]) else max(1e-10, 0.1 * max(a["info"].rho, b["info"].rho) / a["info"].snorm)
+    assert np.abs(ea - eb).max() <= tol * np.abs(eb).max()
+    assert a["info"].launches < b["info"].launches
+
+
 @pytest.mark.parametrize("cfg,seed,nred", [("C2", 3, None), ("C4", 0, 32767)])
 def test_nested_stop_test_matches_tall_contractions(ctx, cfg, seed, nred):
     """rho (Alg. 4 line 24) when last sweep's index lists are prefixes of this sweep's: U_{k-1} lies in
