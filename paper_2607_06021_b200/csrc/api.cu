@@ -35,13 +35,17 @@ struct ScrossWs {
     double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws, *qr_ws2;
     int32_t *scal_i, *iwork;
     int ldrc, ldrr;               // leading dimensions of RC / RR: fixed (kmax / lmax), so that a factor survives a change of k
+    int Kblk;
     bool carve(lrp_arena& ar, const lrp_ctx* ctx, int64_t n, int kmax, int lmax) {
         int K = kmax > lmax ? kmax : lmax;
         ldrc = kmax; ldrr = lmax;
         RC = ar.take<double>((size_t)kmax * kmax); RR = ar.take<double>((size_t)lmax * lmax);
-        Uc = ar.take<double>((size_t)K * K); S = ar.take<double>(K); Vc = ar.take<double>((size_t)K * K);
-        rC = ar.take<double>(kmax); rR = ar.take<double>(lmax);
-        scal_d = ar.take<double>(8); scal_i = ar.take<int32_t>(8); iwork = ar.take<int32_t>(K);
+        Uc = ar.take<double>((size_t)K * K); Vc = ar.take<double>((size_t)K * K);
+        // what the host reads after the core, in one block (one copy into pinned memory): S | rC | rR | scal_d | scal_i
+        Kblk = K;
+        double* rb = ar.take<double>(3 * (size_t)K + 8);
+        S = rb; rC = rb + K; rR = rb + 2 * (size_t)K; scal_d = rb + 3 * (size_t)K; scal_i = (int32_t*)(scal_d + 4);
+        iwork = ar.take<int32_t>(K);
         core_work = ar.take<double>(core_work_doubles(K, K));
         qr_ws = ar.take<double>(tall_qr_ws_doubles(ctx, n, K));
         qr_ws2 = ar.take<double>(tall_qr_ws_doubles(ctx, n, K));
@@ -66,14 +70,18 @@ int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, int k
     a.work = w.core_work; a.iwork = w.iwork;
     LRP_TRY(scross_core(ctx, a));
     const int p = k < l ? k : l;
-    int32_t hi[1]; double hd[1];
-    LRP_CUDA(ctx, cudaMemcpyAsync(h_S, w.S, sizeof(double) * p, cudaMemcpyDeviceToHost, ctx->stream));
-    LRP_CUDA(ctx, cudaMemcpyAsync(h_rC, w.rC, sizeof(double) * k, cudaMemcpyDeviceToHost, ctx->stream));
-    LRP_CUDA(ctx, cudaMemcpyAsync(h_rR, w.rR, sizeof(double) * l, cudaMemcpyDeviceToHost, ctx->stream));
-    LRP_CUDA(ctx, cudaMemcpyAsync(hi, w.scal_i, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
-    LRP_CUDA(ctx, cudaMemcpyAsync(hd, w.scal_d, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    const size_t blk = (3 * (size_t)w.Kblk + 8) * sizeof(double);
+    std::vector<double> pageable;
+    double* hb = ctx->pinned;
+    if (blk > LRP_PINNED_BYTES) { pageable.resize(blk / sizeof(double)); hb = pageable.data(); }
+    LRP_CUDA(ctx, cudaMemcpyAsync(hb, w.S, blk, cudaMemcpyDeviceToHost, ctx->stream));
     LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    *h_rank = hi[0]; *h_smin = hd[0];
+    memcpy(h_S, hb, sizeof(double) * p);
+    memcpy(h_rC, hb + w.Kblk, sizeof(double) * k);
+    memcpy(h_rR, hb + 2 * (size_t)w.Kblk, sizeof(double) * l);
+    *h_smin = hb[3 * (size_t)w.Kblk];
+    int32_t hi; memcpy(&hi, hb + 3 * (size_t)w.Kblk + 4, sizeof(int32_t));
+    *h_rank = hi;
     return LRP_OK;
 }
 
@@ -141,7 +149,7 @@ struct SolveWs {
         QrestU = ar.take<double>(ld * NREST_MAX); QrestV = ar.take<double>(ld * NREST_MAX);
         TU = ar.take<double>((size_t)Kc * NREST_MAX); TV = ar.take<double>((size_t)Kc * NREST_MAX);
         GpU = ar.take<double>(NREST_MAX * NREST_MAX); GpV = ar.take<double>(NREST_MAX * NREST_MAX);
-        rho_out = ar.take<double>(8); eta = ar.take<double>(8);
+        rho_out = ar.take<double>(16); eta = rho_out + 8;      // read back together
         eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
         eta_work = ar.take<double>(2 * eta_stride);
         eta_iwork = ar.take<int32_t>(2 * (size_t)Kc);
@@ -259,7 +267,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
         cudaEventCreateWithFlags(&c->ev_join2, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
-        cudaHostAlloc((void**)&c->pinned, 8192, cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc((void**)&c->pinned, LRP_PINNED_BYTES, cudaHostAllocDefault) != cudaSuccess ||
         cudaMalloc((void**)&c->d_counters, 3 * 65 * sizeof(unsigned)) != cudaSuccess ||
         cudaMemset(c->d_counters, 0, 3 * 65 * sizeof(unsigned)) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -673,8 +681,10 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
                     nstar = h_count < cap ? h_count : cap;
                 } else {
                     LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
-                    LRP_CUDA(ctx, cudaMemcpyAsync(hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                    const bool pin = sizeof(int32_t) * (size_t)numsel <= LRP_PINNED_BYTES;
+                    LRP_CUDA(ctx, cudaMemcpyAsync(pin ? (void*)ctx->pinned : (void*)hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
                     LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+                    if (pin) memcpy(hstar.data(), ctx->pinned, sizeof(int32_t) * numsel);
                 }
                 cur = prev;
                 int added = 0;
@@ -865,13 +875,13 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
         LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join2, 0));
         LRP_TRY(rho_small(ctx, ra));
         double h_rho[2], h_eta[2];
-        LRP_CUDA(ctx, cudaMemcpyAsync(h_rho, w.rho_out, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
-        LRP_CUDA(ctx, cudaMemcpyAsync(h_eta, w.eta, sizeof(double) * 2, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(ctx->pinned, w.rho_out, sizeof(double) * 16, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.Sprev, w.sc.S, sizeof(double) * rank, cudaMemcpyDeviceToDevice, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.UcPrev, w.sc.Uc, sizeof(double) * (size_t)kk * rank, cudaMemcpyDeviceToDevice, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.VcPrev, w.sc.Vc, sizeof(double) * (size_t)l * rank, cudaMemcpyDeviceToDevice, ctx->stream));
         kk_prev = kk; l_prev = l;
         LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        h_rho[0] = ctx->pinned[0]; h_rho[1] = ctx->pinned[1]; h_eta[0] = ctx->pinned[8]; h_eta[1] = ctx->pinned[9];
         cudaEvent_t e6 = ep.rec(ctx);
         const double rho = h_rho[0], snorm = h_rho[1], eta1 = h_eta[0], eta2 = h_eta[1];
         const double ind = (smin == 0.0) ? 0.0 : std::min(eta1 * (1.0 + eta2), eta2 * (1.0 + eta1)) * smin;

@@ -23,6 +23,8 @@ static const char* const LRP_KERNEL_NAMES[K_NUM] = {
 };
 struct lrp_prof { int64_t count; double ms, bytes, flops; };
 
+constexpr size_t LRP_PINNED_BYTES = 16384;
+
 struct lrp_ctx {
     int device;
     cudaStream_t stream;
@@ -40,7 +42,7 @@ struct lrp_ctx {
     cudaStream_t aux2;                    // third stream: the one-CTA eta SVDs beside the two rho contractions
     cudaEvent_t ev_fork, ev_join, ev_join2;
     unsigned* d_counters;                 // 3 x 65 arrival counters (one set per stream) of the in-kernel reductions; zero between launches
-    double* pinned;                       // 8 KB of pinned host memory for the small per-panel read-backs
+    double* pinned;                       // LRP_PINNED_BYTES of pinned host memory: target of the small read-backs of a sweep
     std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)
     std::vector<int>* ev_id;
     size_t ev_used;
