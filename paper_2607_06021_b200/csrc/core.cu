@@ -343,7 +343,10 @@ __device__ void cta_matmul(double* C, int ldc, int m, int n, int kk, const doubl
 // Least squares X Y = B by Householder QR of W = [X | B] (rows x (xn + nb), column-major, ld ldw, overwritten):
 // Y (xn x nb, ld ldy) = R^-1 (Q^T B)(0:xn, :).  Equals pinv(X) B when X has full column rank, which is how the
 // pseudo-inverse of Alg. 1 lines 5-14 is applied when X is well conditioned ("\" in the paper);
-// *cond_flag is set to 1 when min|R_cc| < 1e-8 max|R_cc| (the caller then takes the SVD pseudo-inverse instead).
+// *cond_flag is set to 1 (the caller then takes the SVD pseudo-inverse, whose 1e-13 cut is reading Q4) unless
+// kappa_F(R) = ||R||_F ||R^-1||_F <= 1e8, a rigorous bound (kappa_2 <= kappa_F <= n kappa_2): the diagonal of an
+// unpivoted R alone can look harmless for a numerically singular X (Kahan's matrices).  R^-1 comes out of the same back
+// substitution, from xn identity columns appended behind B: W needs room for xn + nb + xn columns.
 template <int G, bool SH>
 __device__ __noinline__ void cta_ls_householder_t(double* __restrict__ W, int ldw, int rows, int xn, int nb, double* __restrict__ Y, int ldy,
                                                   double* s_scal, int* cond_flag) {
@@ -389,26 +392,45 @@ __device__ __noinline__ void cta_ls_householder_t(double* __restrict__ W, int ld
         }
         __syncthreads();
     }
-    if (tid == 0) {
+    if (tid == 0) {                      // quick reject: kappa_2 >= max|R_cc| / min|R_cc|
         double mx = 0.0, mn = INFINITY;
         for (int c = 0; c < xn; ++c) { double d = fabs(W[c + (size_t)c * ldw]); mx = fmax(mx, d); mn = fmin(mn, d); }
         *cond_flag = !(mn >= 1e-8 * mx && mx > 0.0);
     }
+    for (int e = tid; e < xn * xn; e += blockDim.x) {                       // identity behind B
+        const int i = e % xn, j = e / xn;
+        W[i + (size_t)(xn + nb + j) * ldw] = (i == j) ? 1.0 : 0.0;
+    }
     __syncthreads();
     if (*cond_flag) return;
-    // back substitution R Y = (Q^T B)(0:xn, :), column oriented and in place in W: step i fixes row i of Y for all
-    // right-hand sides, then removes its contribution from the rows above (xn steps of i * nb independent updates)
+    // back substitution R [Y | R^-1] = [(Q^T B)(0:xn, :) | I], column oriented and in place in W: step i fixes row i for
+    // all right-hand sides, then removes its contribution from the rows above (xn steps of i * nbt independent updates)
+    const int nbt = nb + xn;
     for (int i = xn - 1; i >= 0; --i) {
         const double rii = W[i + (size_t)i * ldw];
-        for (int j = tid; j < nb; j += blockDim.x) W[i + (size_t)(xn + j) * ldw] /= rii;
+        for (int j = tid; j < nbt; j += blockDim.x) W[i + (size_t)(xn + j) * ldw] /= rii;
         __syncthreads();
-        for (int e = tid; e < i * nb; e += blockDim.x) {
+        for (int e = tid; e < i * nbt; e += blockDim.x) {
             const int t = e % i, j = e / i;
             double* bj = W + (size_t)(xn + j) * ldw;
             bj[t] = fma(-W[t + (size_t)i * ldw], bj[i], bj[t]);
         }
         __syncthreads();
     }
+    if (warp == 0) {                     // kappa_F(R)^2 = sum R^2 * sum (R^-1)^2 over the upper triangles, fixed order
+        double r2 = 0.0, i2 = 0.0;
+        for (int e = lane; e < xn * xn; e += 32) {
+            const int i = e % xn, j = e / xn;
+            if (i <= j) {
+                const double a = W[i + (size_t)j * ldw], b = W[i + (size_t)(xn + nb + j) * ldw];
+                r2 = fma(a, a, r2); i2 = fma(b, b, i2);
+            }
+        }
+        r2 = warp_sum(r2); i2 = warp_sum(i2);
+        if (lane == 0) *cond_flag = !(r2 * i2 <= 1e16);
+    }
+    __syncthreads();
+    if (*cond_flag) return;
     for (int e = tid; e < xn * nb; e += blockDim.x) {
         const int i = e % xn, j = e / xn;
         Y[i + (size_t)j * ldy] = W[i + (size_t)(xn + j) * ldw];
@@ -463,7 +485,7 @@ scross_core_kernel(CoreArgs a) {
     // B = R_R^T (k <= l, M = Y) or B = R_C^T (k > l, M = Y^T).  Otherwise the SVD pseudo-inverse below.
     {
         const int ldw = xm | 1;                                       // odd leading dimension: no bank conflicts
-        const bool fits = (size_t)ldw * (xn + xm) <= (size_t)a.smem_doubles;
+        const bool fits = (size_t)ldw * (xn + xm + xn) <= (size_t)a.smem_doubles;
         double* Wls = fits ? dyn_smem : svdw;                         // svdw has room only when core_work is sized for it
         const double* Ro = kle ? a.RR : a.RC; const int64_t ldo = kle ? a.ldrr : a.ldrc;
         if (fits) {
@@ -713,7 +735,7 @@ int scross_core(lrp_ctx* ctx, const CoreArgs& a0) {
     const int T = a.k > a.l ? a.k : a.l, p = a.k > a.l ? a.l : a.k;
     size_t smem = jacobi_smem_bytes(ctx, T, p);
     {
-        size_t ls = (size_t)(T | 1) * (size_t)(p + T) * sizeof(double);
+        size_t ls = (size_t)(T | 1) * (size_t)(p + T + p) * sizeof(double);      // [X | B | I] of the least squares
         size_t cap = (size_t)ctx->smem_optin > 2048 ? (size_t)ctx->smem_optin - 2048 : 0;
         if (ls > smem && ls <= cap) smem = ls;
     }

@@ -167,6 +167,45 @@ def _recon(U, S, V, rows, cols):
     return np.einsum("tk,k,tk->t", U[rows], S, V[cols])
 
 
+def _kahan(m, c):
+    sn = np.sqrt(1.0 - c * c)
+    return (sn ** np.arange(m))[:, None] * (np.eye(m) - c * np.triu(np.ones((m, m)), 1))
+
+
+@pytest.mark.parametrize("m,c", [(64, 0.6), (100, 0.45)])
+def test_scross_numerically_singular_selected_rows_with_a_harmless_r_diagonal(ctx, m, c):
+    """Q(I,:) = a scaled Kahan matrix: numerically singular (sigma_min / sigma_max ~ 1e-20, below the 1e-13 cut of reading
+    Q4) while the diagonal of its unpivoted R spans only 1e-6.  The Householder least-squares shortcut of the core must not
+    be taken on the strength of that diagonal: its condition test is ||R||_F ||R^-1||_F, and the SVD pseudo-inverse (which
+    drops the singular direction, like the oracle) takes over.  m = 64: the shortcut's size range; m = 100: beyond it."""
+    import torch
+    from paper_2607_06021_b200 import lrp
+    n = 4095
+    rng = np.random.default_rng(m)
+    X0 = _kahan(m, c); X0 *= 0.5 / np.linalg.norm(X0, 2)
+    sv = np.linalg.svd(X0, compute_uv=False)
+    d = np.abs(np.diag(np.linalg.qr(X0)[1]))
+    assert sv[-1] < 1e-15 * sv[0] and sv[-2] > 1e-8 * sv[0] and d.min() > 1e-7 * d.max()      # the construction holds
+    w, V = np.linalg.eigh(np.eye(m) - X0.T @ X0)
+    comp = np.linalg.qr(rng.standard_normal((n - m, m)))[0] @ ((V * np.sqrt(w)) @ V.T)       # completes X0 to orthonormal columns
+    I = np.sort(rng.choice(n, m, replace=False)).astype(np.int32)
+    J = np.sort(rng.choice(n, m, replace=False)).astype(np.int32)
+    Cm = np.empty((n, m)); rest = np.ones(n, bool); rest[I] = False
+    Cm[I] = X0; Cm[rest] = comp
+    Rt = rng.standard_normal((n, m)) * np.exp(-np.arange(n) / (n / 6))[:, None]
+    ref = O.scross(Cm, Rt, I, J)
+    out = ctx.scross(lrp.tall_from_numpy(Cm), lrp.tall_from_numpy(Rt), torch.from_numpy(I).cuda(), torch.from_numpy(J).cuda())
+    U = lrp.tall_to_numpy(out["U"]); Vg = lrp.tall_to_numpy(out["V"]); S = out["S"].cpu().numpy()
+    assert out["rank"] == ref.rank
+    tol = 1e-9                                          # measured 1e-11; eps * sigma_1 / sigma_kept,min = 1e-9 .. 1e-10
+    errS = np.abs(S - ref.S).max() / ref.S[0]
+    rows = rng.integers(0, n, 4096); cols = rng.integers(0, n, 4096)
+    a = _recon(U, S, Vg, rows, cols); b = _recon(ref.U, ref.S, ref.V, rows, cols)
+    errW = np.abs(a - b).max() / np.abs(b).max()
+    print(f"Kahan m={m}: rank {out['rank']}, S {errS:.2e}, entries {errW:.2e} (tol {tol:.1e})")
+    assert errS <= tol and errW <= tol
+
+
 @pytest.mark.parametrize("n,rank,k,l", [(255, 4, 12, 13), (4095, 9, 20, 17), (4095, 30, 45, 45), (16383, 12, 33, 40)])
 def test_scross_exact_low_rank(ctx, n, rank, k, l):
     """Skeleton theorem pin carried to the GPU: rank(G) <= #I,#J and rank G(I,J) = rank  =>  U S V^T = G."""
