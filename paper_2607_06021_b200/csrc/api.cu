@@ -808,10 +808,13 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             if (nrI > 0) {
                 cudaStream_t main_stream = ctx->stream;
                 ctx->stream = side;
-                int rc_v = tall_gemm_t(ctx, n, w.Rb, ld, l, w.QrestV, ld, nrI, w.TV, l, 0, w.gemmt_ws2);
-                if (rc_v >= 0) {
+                // Q_rest was orthonormal to the common prefix in last sweep's Q: only the rows of T that belong to this
+                // sweep's new columns are non-zero (the others are rounding, 1e-14), and only those columns are read
+                int rc_v = cudaMemsetAsync(w.TV, 0, sizeof(double) * (size_t)l * nrI, ctx->stream) == cudaSuccess ? LRP_OK : LRP_ERR_CUDA;
+                if (rc_v >= 0 && l > l0) rc_v = tall_gemm_t(ctx, n, w.Rb + (int64_t)l0 * ld, ld, l - l0, w.QrestV, ld, nrI, w.TV + l0, l, 0, w.gemmt_ws2);
+                if (rc_v >= 0 && l > l0) {
                     TallGemmArgs g{};
-                    g.n = n; g.k = l; g.m = nrI; g.mode = TG_SUBTRACT; g.A = w.Rb; g.lda = ld; g.B = w.TV; g.ldb = l;
+                    g.n = n; g.k = l - l0; g.m = nrI; g.mode = TG_SUBTRACT; g.A = w.Rb + (int64_t)l0 * ld; g.lda = ld; g.B = w.TV + l0; g.ldb = l;
                     g.Cin = w.QrestV; g.ldc = ld; g.Out = w.QrestV; g.ldo = ld;
                     rc_v = tall_gemm(ctx, g);
                 }
@@ -821,11 +824,14 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             }
             LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
             if (nrJ > 0) {
-                LRP_TRY(tall_gemm_t(ctx, n, w.Cb, ld, kk, w.QrestU, ld, nrJ, w.TU, kk, 0, w.gemmt_ws));
-                TallGemmArgs g{};
-                g.n = n; g.k = kk; g.m = nrJ; g.mode = TG_SUBTRACT; g.A = w.Cb; g.lda = ld; g.B = w.TU; g.ldb = kk;
-                g.Cin = w.QrestU; g.ldc = ld; g.Out = w.QrestU; g.ldo = ld;
-                LRP_TRY(tall_gemm(ctx, g));
+                LRP_CUDA(ctx, cudaMemsetAsync(w.TU, 0, sizeof(double) * (size_t)kk * nrJ, ctx->stream));
+                if (kk > k0) {
+                    LRP_TRY(tall_gemm_t(ctx, n, w.Cb + (int64_t)k0 * ld, ld, kk - k0, w.QrestU, ld, nrJ, w.TU + k0, kk, 0, w.gemmt_ws));
+                    TallGemmArgs g{};
+                    g.n = n; g.k = kk - k0; g.m = nrJ; g.mode = TG_SUBTRACT; g.A = w.Cb + (int64_t)k0 * ld; g.lda = ld; g.B = w.TU + k0; g.ldb = kk;
+                    g.Cin = w.QrestU; g.ldc = ld; g.Out = w.QrestU; g.ldo = ld;
+                    LRP_TRY(tall_gemm(ctx, g));
+                }
                 LRP_TRY(tall_gemm_t(ctx, n, w.QrestU, ld, nrJ, w.QrestU, ld, nrJ, w.GpU, nrJ, 0, w.gemmt_ws));
             }
             LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
