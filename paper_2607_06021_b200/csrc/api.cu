@@ -529,11 +529,15 @@ static int leverage_cholqr2_pair(lrp_ctx* ctx, int64_t n, int c, const double* A
     const double* srcU = AU; const double* srcV = AV; int64_t lsrc = lda;
     for (int pass = 0; pass < 2; ++pass) {
         LRP_TRY(fork());
+        const bool pin = 2 * gb <= LRP_PINNED_BYTES;          // pageable targets would block the host between the launches
+        double* hU = pin ? ctx->pinned : gU.data();
+        double* hV = pin ? ctx->pinned + (size_t)c * c : gV.data();
         LRP_TRY(tall_gemm_t(ctx, n, srcU, lsrc, c, srcU, lsrc, c, w.GU, c, 0, w.gemmt_ws));
-        LRP_CUDA(ctx, cudaMemcpyAsync(gU.data(), w.GU, gb, cudaMemcpyDeviceToHost, ctx->stream));
         LRP_ON_STREAM(ctx, side, tall_gemm_t(ctx, n, srcV, lsrc, c, srcV, lsrc, c, w.GV, c, 0, w.gemmt_ws2));
-        LRP_CUDA(ctx, cudaMemcpyAsync(gV.data(), w.GV, gb, cudaMemcpyDeviceToHost, side));
+        LRP_CUDA(ctx, cudaMemcpyAsync(hU, w.GU, gb, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, cudaMemcpyAsync(hV, w.GV, gb, cudaMemcpyDeviceToHost, side));
         LRP_TRY(join_sync());
+        if (pin) { memcpy(gU.data(), hU, gb); memcpy(gV.data(), hV, gb); }
         if (!host_chol_inverse(gU, c, iU) || !host_chol_inverse(gV, c, iV)) return 1;
         LRP_CUDA(ctx, cudaMemcpyAsync(w.Amat, iU.data(), gb, cudaMemcpyHostToDevice, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.Bmat, iV.data(), gb, cudaMemcpyHostToDevice, ctx->stream));
@@ -649,6 +653,16 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             int64_t numsel64 = (int64_t)sel_cols + p_os; if (numsel64 > n) numsel64 = n;
             if (numsel64 > 2 * (int64_t)Kc) numsel64 = 2 * (int64_t)Kc;
             const int numsel = (int)numsel64;
+            // deterministic top-k: both sides are enqueued before the one host synchronisation that reads them
+            const bool topk_pair = opts->selection == LRP_SELECT_TOPK && 2 * sizeof(int32_t) * (size_t)numsel <= LRP_PINNED_BYTES;
+            if (topk_pair) {
+                int32_t* hp = reinterpret_cast<int32_t*>(ctx->pinned);
+                LRP_TRY(select_topk(ctx, n, w.scoresU, numsel, w.dIstar, w.sel_ws));
+                LRP_CUDA(ctx, cudaMemcpyAsync(hp, w.dIstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                LRP_TRY(select_topk(ctx, n, w.scoresV, numsel, w.dJstar, w.sel_ws));
+                LRP_CUDA(ctx, cudaMemcpyAsync(hp + numsel, w.dJstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            }
             for (int side = 0; side < 2; ++side) {
                 std::vector<int32_t>& cur = side == 0 ? I_k : J_k;
                 const std::vector<int32_t>& prev = side == 0 ? I_prev : J_prev;
@@ -679,6 +693,8 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
                     LRP_CUDA(ctx, cudaMemcpyAsync(&h_count, d_count, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
                     LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
                     nstar = h_count < cap ? h_count : cap;
+                } else if (topk_pair) {
+                    memcpy(hstar.data(), reinterpret_cast<int32_t*>(ctx->pinned) + (size_t)side * numsel, sizeof(int32_t) * numsel);
                 } else {
                     LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
                     const bool pin = sizeof(int32_t) * (size_t)numsel <= LRP_PINNED_BYTES;

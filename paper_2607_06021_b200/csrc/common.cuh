@@ -23,7 +23,7 @@ static const char* const LRP_KERNEL_NAMES[K_NUM] = {
 };
 struct lrp_prof { int64_t count; double ms, bytes, flops; };
 
-constexpr size_t LRP_PINNED_BYTES = 16384;
+constexpr size_t LRP_PINNED_BYTES = 65536;
 
 struct lrp_ctx {
     int device;
