@@ -273,7 +273,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     // one-time kernel attributes (dynamic shared memory opt-in): not on the per-call path
-    if (tall_qr_init(c) != LRP_OK || lrp_dst1_init(c) != LRP_OK || select_init(c) != LRP_OK) { lrp_destroy(c); return LRP_ERR_CUDA; }
+    if (tall_qr_init(c) != LRP_OK || lrp_dst1_init(c) != LRP_OK || select_init(c) != LRP_OK || core_init(c) != LRP_OK || tall_mma_init(c) != LRP_OK) { lrp_destroy(c); return LRP_ERR_CUDA; }
     *out = c;
     return LRP_OK;
 }

@@ -730,6 +730,21 @@ static size_t jacobi_smem_bytes(const lrp_ctx* ctx, int T, int p) {
     return need <= cap ? need : 0;                 // 0: stay in global memory
 }
 
+// Dynamic shared-memory opt-in of the one-CTA kernels: once per context (lrp_create), to everything the device allows.
+template <typename F> static int core_optin(lrp_ctx* ctx, F fn) {
+    cudaFuncAttributes fa;
+    LRP_CUDA(ctx, cudaFuncGetAttributes(&fa, fn));
+    const int v = ctx->smem_optin - (int)fa.sharedSizeBytes;
+    if (v > 48 * 1024) LRP_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v));
+    return LRP_OK;
+}
+int core_init(lrp_ctx* ctx) {
+    LRP_TRY(core_optin(ctx, scross_core_kernel));
+    LRP_TRY(core_optin(ctx, eta_kernel));
+    LRP_TRY(core_optin(ctx, rho_nested_kernel<true>));
+    return LRP_OK;
+}
+
 int scross_core(lrp_ctx* ctx, const CoreArgs& a0) {
     CoreArgs a = a0;
     const int T = a.k > a.l ? a.k : a.l, p = a.k > a.l ? a.l : a.k;
@@ -740,8 +755,6 @@ int scross_core(lrp_ctx* ctx, const CoreArgs& a0) {
         if (ls > smem && ls <= cap) smem = ls;
     }
     a.smem_doubles = (int)(smem / sizeof(double));
-    if (smem > 48 * 1024)
-        LRP_CUDA(ctx, cudaFuncSetAttribute(scross_core_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_CORE, 0, 0);
     scross_core_kernel<<<1, CORE_NT, smem, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
@@ -759,8 +772,6 @@ int eta_pair(lrp_ctx* ctx, const EtaArgs& a0) {
     const int T = nmax > a.r ? nmax : a.r, p = nmax > a.r ? a.r : nmax;
     const size_t smem = jacobi_smem_bytes(ctx, T, p > 0 ? p : 1);
     a.smem_doubles = (int)(smem / sizeof(double));
-    if (smem > 48 * 1024)
-        LRP_CUDA(ctx, cudaFuncSetAttribute(eta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_ETA, 0, 0);
     eta_kernel<<<2, CORE_NT, smem, ctx->stream>>>(a);
     LRP_LAUNCHED(ctx);
@@ -782,8 +793,6 @@ int rho_nested_prep(lrp_ctx* ctx, int r, int rp, const RhoNestedSide& u, const R
     size_t smem = need(u) > need(v) ? need(u) : need(v);
     a.use_smem = smem <= (size_t)200 * 1024 ? 1 : 0;
     if (!a.use_smem) smem = 0;
-    if (smem > 48 * 1024)
-        LRP_CUDA(ctx, cudaFuncSetAttribute(rho_nested_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_RHO, 0, 0);
     if (a.use_smem) rho_nested_kernel<true><<<2, CORE_NT, smem, ctx->stream>>>(a);
     else rho_nested_kernel<false><<<2, CORE_NT, 0, ctx->stream>>>(a);

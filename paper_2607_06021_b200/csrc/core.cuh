@@ -69,6 +69,7 @@ int leverage_colmask(lrp_ctx* ctx, int k, const double* R, int64_t ldr, double r
 struct SelectBernoulli { int cols; double c; unsigned long long seed; int sweep; int side; };
 size_t select_ws_bytes(const lrp_ctx* ctx, int64_t n, int num);
 int select_init(lrp_ctx* ctx);
+int core_init(lrp_ctx* ctx);                     // one-time kernel attributes (lrp_create)
 int select_topk(lrp_ctx* ctx, int64_t n, const double* scores, int num, int32_t* idx_out, void* ws,
                 const SelectBernoulli* bern = nullptr, int* d_count = nullptr);
 

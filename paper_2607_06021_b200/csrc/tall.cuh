@@ -41,5 +41,6 @@ int tall_lowrank_entries(lrp_ctx* ctx, int r, const double* U, int64_t ldu, cons
 
 // G (m x m) = E^T E with E = Cin - A B formed on the fly (never written).  Returns 1 (nothing launched) when the shape
 // is outside the fused kernel's range; partial_ws as for tall_gemm_t(n, m, m).
+int tall_mma_init(lrp_ctx* ctx);                 // one-time kernel attributes (lrp_create)
 int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k, const double* B, int64_t ldb,
                     const double* Cin, int64_t ldc, int m, double* G, int64_t ldg, double* partial_ws);

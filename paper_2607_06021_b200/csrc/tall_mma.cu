@@ -396,6 +396,26 @@ tall_resid_gram_kernel(int64_t n, const double* __restrict__ A, int64_t lda, int
 
 }  // namespace
 
+// Dynamic shared-memory opt-in of every contraction kernel: once per context (lrp_create).
+template <typename F> static int mma_optin(lrp_ctx* ctx, F fn) {
+    cudaFuncAttributes fa;
+    LRP_CUDA(ctx, cudaFuncGetAttributes(&fa, fn));
+    const int v = ctx->smem_optin - (int)fa.sharedSizeBytes;
+    if (v > 48 * 1024) LRP_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v));
+    return LRP_OK;
+}
+int tall_mma_init(lrp_ctx* ctx) {
+    LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<2, true>)); LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<2, false>));
+    LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<4, true>)); LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<4, false>));
+    LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<5, true>)); LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<5, false>));
+    LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<6, true>)); LRP_TRY(mma_optin(ctx, tall_gemm_mma_kernel<6, false>));
+    LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<1>)); LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<2>));
+    LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<3>)); LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<4>));
+    LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<5>)); LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<6>));
+    LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<7>)); LRP_TRY(mma_optin(ctx, tall_resid_gram_kernel<8>));
+    return LRP_OK;
+}
+
 int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
     if (p.n <= 0 || p.m <= 0) return LRP_OK;
     // column tiles of 8 nj: every tile pass re-reads A, so 33..48 columns (the rebuild U = Q Uc, the first sweep's
@@ -410,10 +430,7 @@ int tall_gemm(lrp_ctx* ctx, const TallGemmArgs& p) {
                                : nj == 5 ? (vec ? tall_gemm_mma_kernel<5, true> : tall_gemm_mma_kernel<5, false>)
                                : nj == 6 ? (vec ? tall_gemm_mma_kernel<6, true> : tall_gemm_mma_kernel<6, false>)
                                          : (vec ? tall_gemm_mma_kernel<4, true> : tall_gemm_mma_kernel<4, false>);
-    if (smem > 48 * 1024) {
-        if (smem > (size_t)ctx->smem_optin) return LRP_ERR_BADARG;
-        LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
+    if (smem > (size_t)ctx->smem_optin) return LRP_ERR_BADARG;       // opt-in set once by tall_mma_init
     int64_t grid = (p.n + MG_THREADS - 1) / MG_THREADS;
     const int64_t resident = (int64_t)lrp_sm_count(ctx) * (nj == 2 ? 5 : (nj <= 4 ? 4 : 3));   // persistent over row slabs (B staged once per column tile per CTA):
     if (grid > resident) grid = resident;            // exactly one resident wave, so that the slabs are balanced
@@ -498,7 +515,6 @@ int tall_resid_gram(lrp_ctx* ctx, int64_t n, const double* A, int64_t lda, int k
         case 5: kern = tall_resid_gram_kernel<5>; break; case 6: kern = tall_resid_gram_kernel<6>; break;
         case 7: kern = tall_resid_gram_kernel<7>; break; default: kern = tall_resid_gram_kernel<8>; break;
     }
-    if (smem > 48 * 1024) LRP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LRP_PROF(ctx, K_RESID_GRAM, 8.0 * n * (k + m), 2.0 * n * m * (k + m));
     kern<<<nblk, RG_THREADS, smem, ctx->stream>>>(n, A, lda, k, B, ldb, Cin, ldc, m, partial_ws, o);
     LRP_LAUNCHED(ctx);
