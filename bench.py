@@ -109,11 +109,11 @@ def solve_roofline(n, rF, trace, r_final, hbm_gbs, p64_tflops, ms_measured):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch over the algorithmic bytes of the same launch, from this round's
 # `ncu --set full` captures (summaries with their commands under profiles/r02_*_ncu.md); None -> "traffic": null
 _SRC = "profiles/r02_solve_ncu.md (ncu --set full, one C4 solve)"
-NCU_TRAFFIC = {"panel_qr": {"dram_over_alg": 0.79, "source": _SRC}, "panel_apply": {"dram_over_alg": 0.83, "source": _SRC},
-               "dst1_fused": {"dram_over_alg": 1.65, "source": _SRC}, "tall_gemm_t": {"dram_over_alg": 1.09, "source": _SRC},
-               "tall_gemm_subtract": {"dram_over_alg": 1.01, "source": _SRC + ", all tall_gemm modes together"},
-               "tall_gemm_plain": {"dram_over_alg": 1.01, "source": _SRC + ", all tall_gemm modes together"},
-               "tall_gemm_sample": {"dram_over_alg": 1.01, "source": _SRC + ", all tall_gemm modes together"}}
+NCU_TRAFFIC = {"panel_qr": {"dram_over_alg": 0.77, "source": _SRC}, "panel_apply": {"dram_over_alg": 0.81, "source": _SRC},
+               "dst1_fused": {"dram_over_alg": 1.65, "source": _SRC}, "tall_gemm_t": {"dram_over_alg": 0.89, "source": _SRC},
+               "tall_gemm_subtract": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"},
+               "tall_gemm_plain": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"},
+               "tall_gemm_sample": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"}}
 
 # kernel class -> (phase, roofline SURVEY.md 8(d) assigns to it)
 PHASE_OF = {"dst1_small": ("dst", "hbm"), "dst1_naive": ("dst", "hbm"), "dst1_fused": ("dst", "hbm"), "dst1_bluestein": ("dst", "hbm"),
