@@ -149,7 +149,7 @@ struct SolveWs {
         QrestU = ar.take<double>(ld * NREST_MAX); QrestV = ar.take<double>(ld * NREST_MAX);
         TU = ar.take<double>((size_t)Kc * NREST_MAX); TV = ar.take<double>((size_t)Kc * NREST_MAX);
         GpU = ar.take<double>(NREST_MAX * NREST_MAX); GpV = ar.take<double>(NREST_MAX * NREST_MAX);
-        rho_out = ar.take<double>(16); eta = rho_out + 8;      // read back together
+        rho_out = ar.take<double>(16 + RHO_MAX_GRID + 2); eta = rho_out + 8;      // [rho, snorm | eta1, eta2] read back together; partial sums and ticket of rho_kernel behind them
         eta_stride = lrp_align_up(eta_work_doubles(Kc, Kc) * sizeof(double)) / sizeof(double);
         eta_work = ar.take<double>(2 * eta_stride);
         eta_iwork = ar.take<int32_t>(2 * (size_t)Kc);
@@ -880,7 +880,7 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
         LRP_CUDA(ctx, cudaEventRecord(ctx->ev_join, side));
         RhoArgs ra{};
         ra.r = rank; ra.rp = r_prev; ra.Sk = w.sc.S; ra.Sp = w.Sprev; ra.A = w.Amat; ra.B = w.Bmat; ra.GU = w.GU; ra.GV = w.GV;
-        ra.out = w.rho_out;
+        ra.out = w.rho_out; ra.partial = w.rho_out + 16; ra.ticket = reinterpret_cast<unsigned*>(w.rho_out + 16 + RHO_MAX_GRID);
         if (r_prev > 0 && !nested) {
             LRP_TRY(tall_gemm_t(ctx, n, Uk, ld, rank, Up, ld, r_prev, w.Amat, rank, 0, w.gemmt_ws));      // U side
             int rc_u = tall_resid_gram(ctx, n, Uk, ld, rank, w.Amat, rank, Up, ld, r_prev, w.GU, r_prev, w.gemmt_ws);

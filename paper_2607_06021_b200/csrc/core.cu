@@ -585,7 +585,10 @@ eta_kernel(EtaArgs a) {
 __global__ void __launch_bounds__(CORE_NT)
 rho_kernel(RhoArgs a) {
     __shared__ double red[32];
-    const int tid = threadIdx.x, nt = blockDim.x;
+    __shared__ unsigned s_last;
+    // the (independent) output elements of the three sums are spread over the grid; per-CTA partial sums are added by the
+    // last CTA to arrive, in block order (deterministic)
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
     const int r = a.r, rp = a.rp;
     double acc = 0.0;
     // T1 = A diag(Sp)  (r x rp);  term1: sum_{i,j} (Sk(i) delta_ij - sum_t T1(i,t) B(j,t))^2
@@ -612,16 +615,25 @@ rho_kernel(RhoArgs a) {
         acc = fma(a.GU[e] * a.Sp[t] * a.Sp[u], a.GV[e], acc);
     }
     acc = warp_sum(acc);
-    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
     __syncthreads();
-    if (tid == 0) {
+    if (threadIdx.x == 0) {
         double t = 0.0;
-        for (int w = 0; w < nt / 32; ++w) t += red[w];
-        double sn = 0.0;
-        for (int c = 0; c < r; ++c) sn = fma(a.Sk[c], a.Sk[c], sn);
-        a.out[0] = sqrt(t > 0.0 ? t : 0.0);
-        a.out[1] = sqrt(sn);
+        for (int w = 0; w < (int)blockDim.x / 32; ++w) t += red[w];
+        a.partial[blockIdx.x] = t;
+        __threadfence();
+        s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
     }
+    __syncthreads();
+    if (!s_last || threadIdx.x != 0) return;
+    __threadfence();
+    double t = 0.0;
+    for (int b = 0; b < (int)gridDim.x; ++b) t += __ldcg(a.partial + b);
+    double sn = 0.0;
+    for (int c = 0; c < r; ++c) sn = fma(a.Sk[c], a.Sk[c], sn);
+    a.out[0] = sqrt(t > 0.0 ? t : 0.0);
+    a.out[1] = sqrt(sn);
+    *a.ticket = 0u;                                   // ready for the next launch
 }
 
 struct RhoNestedArgs { int r, rp, use_smem; RhoNestedSide s0, s1; };
@@ -781,7 +793,12 @@ int eta_pair(lrp_ctx* ctx, const EtaArgs& a0) {
 int rho_small(lrp_ctx* ctx, const RhoArgs& a) {
     LRP_PROF(ctx, K_RHO, 0, 0);
     if (a.rp == 0) snorm_kernel<<<1, 32, 0, ctx->stream>>>(a.r, a.Sk, a.out);
-    else rho_kernel<<<1, CORE_NT, 0, ctx->stream>>>(a);
+    else {
+        int work = a.r * a.r + 2 * a.r * a.rp + a.rp * a.rp;
+        int grid = (work + 255) / 256; if (grid > RHO_MAX_GRID) grid = RHO_MAX_GRID; if (grid < 1) grid = 1;
+        LRP_CUDA(ctx, cudaMemsetAsync(a.ticket, 0, sizeof(unsigned), ctx->stream));
+        rho_kernel<<<grid, 256, 0, ctx->stream>>>(a);
+    }
     LRP_LAUNCHED(ctx);
     return LRP_OK;
 }

@@ -39,7 +39,9 @@ struct RhoArgs {
     const double* A; const double* B;           // r x rp (ld r): U_k^T U_{k-1}, V_k^T V_{k-1}
     const double* GU; const double* GV;         // rp x rp (ld rp): E_U^T E_U, E_V^T E_V
     double* out;                                // [2] device: rho, ||S_k||_2
+    double* partial; unsigned* ticket;          // RHO_MAX_GRID per-CTA partial sums and the arrival counter of the reduction
 };
+constexpr int RHO_MAX_GRID = 64;
 int rho_small(lrp_ctx* ctx, const RhoArgs& a);
 
 // Nested case of the stop test: last sweep's index list is, up to `nrest` = kkp - k0 dropped trailing entries, a prefix
