@@ -181,6 +181,7 @@ typedef struct lrp_solve_opts {
 #define LRP_FLAG_NO_NESTED_RHO  2   /* rho always from the tall iterates (reading R5 off) */
 #define LRP_FLAG_NO_FUSED_RHO   4   /* rho's residual Gram matrix by an update sweep + a Gram sweep instead of the fused kernel */
 #define LRP_FLAG_NO_CHOLQR_LEVERAGE 8 /* leverage scores of the initial guess always through the Householder QR (reading R8 off) */
+#define LRP_FLAG_NO_PRIORITY_STREAMS 16 /* TSQR tree levels on the job's own stream instead of a high-priority one (scheduling only) */
 
 typedef struct lrp_solve_info {
     int32_t rank, sweeps, converged;

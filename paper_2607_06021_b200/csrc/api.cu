@@ -261,6 +261,7 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->prof_on = 0; c->prof_pending = -1; memset(c->prof, 0, sizeof(c->prof));
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
     c->flags = 0; c->solve_ev = new std::vector<cudaEvent_t>();
+    for (int q = 0; q < 2; ++q) { c->hi[q] = nullptr; c->ev_hi[q][0] = nullptr; c->ev_hi[q][1] = nullptr; }
     c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr; c->d_counters = nullptr;
     if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->aux2, cudaStreamNonBlocking) != cudaSuccess ||
@@ -270,6 +271,14 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
         cudaHostAlloc((void**)&c->pinned, LRP_PINNED_BYTES, cudaHostAllocDefault) != cudaSuccess ||
         cudaMalloc((void**)&c->d_counters, 3 * 65 * sizeof(unsigned)) != cudaSuccess ||
         cudaMemset(c->d_counters, 0, 3 * 65 * sizeof(unsigned)) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
+    {
+        int lo = 0, hiprio = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hiprio);
+        for (int q = 0; q < 2; ++q)
+            if (cudaStreamCreateWithPriority(&c->hi[q], cudaStreamNonBlocking, hiprio) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_hi[q][0], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_hi[q][1], cudaEventDisableTiming) != cudaSuccess) { lrp_destroy(c); return LRP_ERR_CUDA; }
+    }
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
     // one-time kernel attributes (dynamic shared memory opt-in): not on the per-call path
@@ -283,6 +292,11 @@ int lrp_destroy(lrp_ctx* ctx) {
     if (ctx->ev) { for (auto e : *ctx->ev) cudaEventDestroy(e); delete ctx->ev; }
     if (ctx->solve_ev) { for (auto e : *ctx->solve_ev) cudaEventDestroy(e); delete ctx->solve_ev; }
     if (ctx->d_counters) cudaFree(ctx->d_counters);
+    for (int q = 0; q < 2; ++q) {
+        if (ctx->hi[q]) cudaStreamDestroy(ctx->hi[q]);
+        if (ctx->ev_hi[q][0]) cudaEventDestroy(ctx->ev_hi[q][0]);
+        if (ctx->ev_hi[q][1]) cudaEventDestroy(ctx->ev_hi[q][1]);
+    }
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     if (ctx->aux2) cudaStreamDestroy(ctx->aux2);
     if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);

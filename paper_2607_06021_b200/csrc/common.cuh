@@ -41,6 +41,8 @@ struct lrp_ctx {
     cudaStream_t aux;                     // library-owned second stream: independent sub-steps of a sweep overlap on it
     cudaStream_t aux2;                    // third stream: the one-CTA eta SVDs beside the two rho contractions
     cudaEvent_t ev_fork, ev_join, ev_join2;
+    cudaStream_t hi[2];                   // high-priority streams (one per QR job): the small tree levels of the TSQR run here, so
+    cudaEvent_t ev_hi[2][2];              // that they do not queue behind the other job's leaf CTAs; [job][to hi / back]
     unsigned* d_counters;                 // 3 x 65 arrival counters (one set per stream) of the in-kernel reductions; zero between launches
     double* pinned;                       // LRP_PINNED_BYTES of pinned host memory: target of the small read-backs of a sweep
     std::vector<cudaEvent_t>* ev;         // event pool: pairs (start, end)

@@ -23,6 +23,7 @@ LRP_ERR_STATIC_LIMIT = -5
 TOPK_STATIC_MAX_N, TOPK_STATIC_MAX_NUM = 4194304, 256
 MAX_SWEEPS_INFO = 32
 LRP_FLAG_NO_QR_REUSE, LRP_FLAG_NO_NESTED_RHO, LRP_FLAG_NO_FUSED_RHO, LRP_FLAG_NO_CHOLQR_LEVERAGE = 1, 2, 4, 8
+LRP_FLAG_NO_PRIORITY_STREAMS = 16
 LRP_G_POISSON, LRP_G_HILBERT, LRP_G_KMATRIX = 0, 1, 2
 SELECTIONS = {"topk": 0, "bernoulli": 1, "qdeim": 2, "deim": 3}
 MATRIX_KINDS = {"hilbert": LRP_G_HILBERT, "kmatrix": LRP_G_KMATRIX}
