@@ -27,6 +27,15 @@
 #include <math.h>
 #include <cuda/atomic>
 
+#ifdef LRP_DST_STATS
+__device__ unsigned long long g_sub[32];
+#define SUBT(i) do { if (threadIdx.x == 0) { long long t_ = clock64(); atomicAdd(&g_sub[i], (unsigned long long)(t_ - tsub)); tsub = t_; } } while (0)
+#define SUBT0() long long tsub = clock64()
+extern "C" int lrp_debug_dst_sub(unsigned long long* out) { cudaDeviceSynchronize(); int rc = (int)cudaMemcpyFromSymbol(out, g_sub, sizeof(g_sub)); unsigned long long z[32] = {0}; cudaMemcpyToSymbol(g_sub, z, sizeof(z)); return rc; }
+#else
+#define SUBT(i) do {} while (0)
+#define SUBT0() do {} while (0)
+#endif
 namespace {
 
 constexpr int SC_CHUNK = 4096;                                  // k's per chunk of phase C = anchor spacing
@@ -60,7 +69,14 @@ template <int Q1, int TL> struct PACfg {
 //   gB   [2 L2]          exp(-i pi m / N), m = 2 j2 + b
 //   g4lo [L2][32]        exp(-2 pi i j2 l / L)
 //   g4hi [L2][L1/32]     exp(-2 pi i j2 (32 h) / L)
-struct ATables { const double2* gB; const double2* g4lo; const double2* g4hi; };
+//   twA  [64 + NHI_A]    two-level table (tw_get) of exp(-2 pi i u / (2 L1)): lo[64] then hi[2 L1 / 64 + 1]
+//   twB  [64 + NHI_B]    the same for exp(-2 pi i u / (2 L2))   (phase B)
+struct ATables { const double2* gB; const double2* g4lo; const double2* g4hi; const double2* twA; const double2* twB; };
+
+// copy a two-level twiddle table (tw_get layout: lo[64], hi[nhi]) from the per-call global table into shared memory
+__device__ __forceinline__ void tw_fetch(double2* lo, double2* hi, const double2* __restrict__ src, int nhi, int tid, int nt) {
+    for (int i = tid; i < 64 + nhi; i += nt) { const double2 v = __ldg(src + i); if (i < 64) lo[i] = v; else hi[i - 64] = v; }
+}
 
 // tile c of one column: x -> W (L complex), ypart[2 j2 + b] (2 L2 complex): the CTA's folded anchor sums
 template <int Q1, int TL>
@@ -95,14 +111,16 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
             y1[i] = __ldcs(x + N - m0 - 2);
         }
     };
+    SUBT0();
     load_half(0);
-    tw_build(lo, hi, 2 * L1, C::NHI, tid, NT);
+    tw_fetch(lo, hi, tabs.twA, C::NHI, tid, NT);
     for (int i = tid; i < 2 * T2; i += NT) tB[i] = __ldg(tabs.gB + 2 * j2_of(i >> 1) + (i & 1));
     for (int i = tid; i < T2 * (C::TW_LO + C::TW_HI); i += NT) {
         if (i < T2 * C::TW_LO) { const int s = i / C::TW_LO, kk = i % C::TW_LO; t4lo[s * C::SLO + kk] = __ldg(tabs.g4lo + (int64_t)j2_of(s) * C::TW_LO + kk); }
         else { const int q = i - T2 * C::TW_LO, s = q / C::TW_HI, h = q % C::TW_HI; t4hi[s * C::SHI + h] = __ldg(tabs.g4hi + (int64_t)j2_of(s) * C::TW_HI + h); }
     }
     __syncthreads();
+    SUBT(0);
     // fold: t_m = sin(pi m/N)(x_m + x_{N-m}) + (x_m - x_{N-m})/2 for m = 2j, 2j+1;  z_j = t_{2j} + i t_{2j+1}
     // anchors: ya[b] += (x_m + x_{N-m}) e^{+i pi m/N} for m = m0 + b < L  (the thread's s = tid % T2 is the same for all its e)
     double2 ya0 = make_double2(0.0, 0.0), ya1 = make_double2(0.0, 0.0);
@@ -128,11 +146,13 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
         }
     }
     __syncthreads();
+    SUBT(1);
     {
         const int g = tid / GS, gt = tid % GS;
         fft_smem<Q1, NT / GS>(re + g * RS, im + g * RS, gt, g, lo, hi, 2);
     }
     __syncthreads();                                  // the sub-FFTs synchronise per group; the store below reads across groups
+    SUBT(2);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         int e = tid + i * NT;
@@ -142,6 +162,7 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
         __stcg(&Wc[(int64_t)k1 * L2 + j2_of(s)], cmul(v, w));
     }
     __syncthreads();
+    SUBT(3);
     // anchor partials: sum over the NT / T2 threads that share s (fixed order), one entry per (j2, b)
     double* red = re;                                 // [NT][4]
     red[4 * tid + 0] = ya0.x; red[4 * tid + 1] = ya0.y; red[4 * tid + 2] = ya1.x; red[4 * tid + 3] = ya1.y;
@@ -152,15 +173,28 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
         for (int q = 0; q < NT / T2; ++q) { ar += red[4 * (s + q * T2) + 2 * b]; ai += red[4 * (s + q * T2) + 2 * b + 1]; }
         __stcg(&ypart[2 * j2_of(s) + b], make_double2(ar, ai));
     }
+    SUBT(4);
 }
 
 // one thread per table entry; exact arguments (powers of two), sincospi
-__global__ void dst1_tables_kernel(int log2N, int q1, double2* __restrict__ gB, double2* __restrict__ g4lo, double2* __restrict__ g4hi) {
+__global__ void dst1_tables_kernel(int log2N, int q1, double2* __restrict__ gB, double2* __restrict__ g4lo, double2* __restrict__ g4hi,
+                                   double2* __restrict__ twA, double2* __restrict__ twB) {
     const int64_t N = (int64_t)1 << log2N, L = N >> 1, L2 = L >> q1;
     const int nhi = ((1 << q1) + 31) / 32;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t nB = 2 * L2, nlo = L2 * 32, nh = L2 * nhi;
     double sn, cs;
+    if (blockIdx.x == 0) {                            // the two-level tables of the sub-FFTs: M = 2 L1 and M = 2 L2
+        for (int t = threadIdx.x; t < 2 * 64 + 2 + (int)((2 << q1) / 64) + (int)(2 * L2 / 64); t += blockDim.x) {
+            const int nA = 64 + (int)((2 << q1) / 64) + 1;
+            const bool isA = t < nA;
+            const int u = isA ? t : t - nA;
+            const double inv = 1.0 / (double)(isA ? ((int64_t)2 << q1) : 2 * L2);       // powers of two: exact arguments
+            const double arg = u < 64 ? -2.0 * (double)u * inv : -2.0 * (double)((u - 64) * 64) * inv;
+            sincospi(arg, &sn, &cs);
+            (isA ? twA : twB)[u] = make_double2(cs, sn);
+        }
+    }
     if (i < nB) { sincospi(-(double)i / (double)N, &sn, &cs); gB[i] = make_double2(cs, sn); }
     else if (i < nB + nlo) {
         const int64_t e = i - nB, j2 = e / 32, kk = e % 32;
@@ -223,12 +257,21 @@ __device__ __forceinline__ void phase_d(unsigned char* smem_raw, int log2N, int 
 }
 
 // ------------------------------------------------------------------------------------------------ phase B
+// Rows of L2 >= 512 points (SPLIT): decimation in frequency by 8.  The first radix-8 butterfly runs on the registers the
+// coalesced row load delivers (v[r] = row[gt + r L2/8]), its outputs are twiddled and stored as EIGHT CONTIGUOUS blocks
+// of Ls = L2/8 points (block r' at r' * BS), and block r' is then an independent length-Ls FFT whose result is
+// X[8 k' + r'] -- one warp (or less) per block, so the remaining passes synchronise with __syncwarp instead of a
+// 256-thread named barrier per pass.  POS(k2) is where X[k2] ends up; BS = Ls + 2 keeps the untangle's and the store
+// loop's consecutive k2 (8 blocks x 2 neighbouring k') on 16 different banks.
 template <int Q2, int TL> struct PBCfg {
     static constexpr int L2 = 1 << Q2, GS = L2 / 8;
     static constexpr int R2 = (1 << TL) / L2, T = R2 / 2;        // rows per CTA: T rows k1 + their T mirror rows
     static constexpr int NT = (1 << TL) / 8;
-    static constexpr int RS = row_stride(L2, R2);
+    static constexpr bool SPLIT = Q2 >= 9;
+    static constexpr int LS = L2 / 8, BS = LS + 2;
+    static constexpr int RS = SPLIT ? 8 * BS : row_stride(L2, R2);
     static constexpr int IMOFF = R2 * RS + 8;
+    __device__ __forceinline__ static int POS(int k2) { return SPLIT ? (k2 & 7) * BS + PADI(k2 >> 3) : PADI(k2); }
     static constexpr int NHI = (2 * L2) / 64 + 1;
     static constexpr size_t SMEM = sizeof(double2) * (64 + NHI + R2) + sizeof(double) * ((size_t)2 * IMOFF);
 };
@@ -246,7 +289,7 @@ __device__ __forceinline__ void untangle_pair(double2& zk, double2& zm, double2 
 // tile c of one column: rows of W -> (R_k, X_{2k}) in place, scaled;  *xlast = scale X_{N-1}  (tile 0)
 template <int Q2, int TL>
 __device__ __forceinline__ void phase_b(unsigned char* smem_raw, int log2N, int c, double2* __restrict__ Wc, double scale,
-                                        double* __restrict__ xlast) {
+                                        double* __restrict__ xlast, const ATables tabs) {
     using C = PBCfg<Q2, TL>;
     constexpr int L2 = C::L2, GS = C::GS, R2 = C::R2, T = C::T, RS = C::RS, NT = C::NT;
     const int64_t N = (int64_t)1 << log2N, L = N >> 1;
@@ -263,42 +306,63 @@ __device__ __forceinline__ void phase_b(unsigned char* smem_raw, int log2N, int 
     };
     const int g = tid / GS, gt = tid % GS;           // group g transforms row slot g; v[r] = row[gt + r*GS]: first-pass operands
     double2 v[8];
+    SUBT0();
     {
         const double2* row = Wc + (int64_t)row_of(g) * L2;
 #pragma unroll
         for (int r = 0; r < 8; ++r) v[r] = ldcg2(row + gt + r * GS);
     }
-    tw_build(lo, hi, 2 * L2, C::NHI, tid, NT);        // exp(-2 pi i u/(2 L2)) = exp(-2 pi i (L1 u)/N)
+    tw_fetch(lo, hi, tabs.twB, C::NHI, tid, NT);      // exp(-2 pi i u/(2 L2)) = exp(-2 pi i (L1 u)/N)
     for (int i = tid; i < R2; i += NT) {
         double sn, cs; sincospi(-2.0 * (double)row_of(i) / (double)N, &sn, &cs); rowtw[i] = make_double2(cs, sn);
     }
-    fft_smem_from_regs<Q2, NT / GS>(v, re + g * RS, im + g * RS, gt, g, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
+    if constexpr (C::SPLIT) {
+        constexpr int QS = Q2 - 3, GSS = C::LS / 8;                   // sub-FFT: 2^QS points, GSS threads
+        Bfly<8>::run(v);
+        {   // v[r'] *= exp(-2 pi i gt r'/L2) = tw(2 gt r'); the shared tables are not published yet: w1 from the global copy
+            const int u = 2 * gt;
+            const double2 w1 = cmul(__ldg(tabs.twB + 64 + (u >> 6)), __ldg(tabs.twB + (u & 63)));
+            const double2 w2 = cmul(w1, w1), w3 = cmul(w2, w1), w4 = cmul(w2, w2);
+            const double2 w5 = cmul(w4, w1), w6 = cmul(w4, w2), w7 = cmul(w4, w3);
+            v[1] = cmul(v[1], w1); v[2] = cmul(v[2], w2); v[3] = cmul(v[3], w3); v[4] = cmul(v[4], w4);
+            v[5] = cmul(v[5], w5); v[6] = cmul(v[6], w6); v[7] = cmul(v[7], w7);
+        }
+        double* rg = re + g * RS; double* ig = im + g * RS;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) { const int idx = r * C::BS + PADI(gt); rg[idx] = v[r].x; ig[idx] = v[r].y; }
+        __syncthreads();                              // blocks complete (written by the whole row group); tables published
+        const int sg = gt / GSS, lt = gt % GSS;
+        fft_smem<QS, NT / GSS>(rg + sg * C::BS, ig + sg * C::BS, lt, tid / GSS, lo, hi, 16);      // exp(-2 pi i mm/Ls) = tw(16 mm)
+    } else {
+        fft_smem_from_regs<Q2, NT / GS>(v, re + g * RS, im + g * RS, gt, g, lo, hi, 2);      // exp(-2 pi i mm/L2) = tw(2 mm)
+    }
     __syncthreads();                                  // per-group barriers inside; the untangle pairs rows of different groups
+    SUBT(8);
     // untangle: thread owns the pair {(slot r, k2), its mirror}; k = row + L1*k2
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         int e = tid + i * NT;
         int r = e / L2, k2 = e % L2;
         if (c * T + r >= 1) {                                      // general rows: mirror is (slot T+r, L2-1-k2)
-            int ia = r * RS + PADI(k2), ib = (T + r) * RS + PADI(L2 - 1 - k2);
+            int ia = r * RS + C::POS(k2), ib = (T + r) * RS + C::POS(L2 - 1 - k2);
             double2 zk = make_double2(re[ia], im[ia]), zm = make_double2(re[ib], im[ib]);
             untangle_pair(zk, zm, cmul(rowtw[r], tw_get(lo, hi, k2)));
             re[ia] = zk.x; im[ia] = zk.y; re[ib] = zm.x; im[ib] = zm.y;
         } else {
             // row 0 pairs with itself: (k2, L2-k2), k2 = 1..L2/2; k2 = 0 holds T_0
             if (k2 == 0) {
-                double a = re[0], b = im[0];
+                double a = re[0], b = im[0];                    // POS(0) = 0
                 re[0] = 0.5 * (a + b); im[0] = 0.0;               // R_0 := X_1 = T_0/2
                 *xlast = scale * 0.5 * (b - a);                    // X_{N-1} = -T_L/2: where the last chunk's backward sum starts
             } else if (k2 <= L2 / 2) {
-                int ia = PADI(k2), ib = PADI(L2 - k2);
+                int ia = C::POS(k2), ib = C::POS(L2 - k2);
                 double2 zk = make_double2(re[ia], im[ia]), zm = make_double2(re[ib], im[ib]);
                 untangle_pair(zk, zm, tw_get(lo, hi, k2));
                 re[ia] = zk.x; im[ia] = zk.y; re[ib] = zm.x; im[ib] = zm.y;
             }
             // slot T holds row L1/2, which also pairs with itself: (k2, L2-1-k2), k2 < L2/2
             if (k2 < L2 / 2) {
-                int ia = T * RS + PADI(k2), ib = T * RS + PADI(L2 - 1 - k2);
+                int ia = T * RS + C::POS(k2), ib = T * RS + C::POS(L2 - 1 - k2);
                 double2 zk = make_double2(re[ia], im[ia]), zm = make_double2(re[ib], im[ib]);
                 untangle_pair(zk, zm, cmul(rowtw[T], tw_get(lo, hi, k2)));
                 re[ia] = zk.x; im[ia] = zk.y; re[ib] = zm.x; im[ib] = zm.y;
@@ -306,14 +370,16 @@ __device__ __forceinline__ void phase_b(unsigned char* smem_raw, int log2N, int 
         }
     }
     __syncthreads();
+    SUBT(9);
     // (R_k, X_{2k}) back into the CTA's own rows of W
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         int e = tid + i * NT;
         int slot = e / L2, k2 = e % L2;
-        int ia = slot * RS + PADI(k2);
+        int ia = slot * RS + C::POS(k2);
         __stcg(&Wc[(int64_t)row_of(slot) * L2 + k2], make_double2(scale * re[ia], scale * im[ia]));
     }
+    SUBT(10);
 }
 
 // ------------------------------------------------------------------------------------------------ phase C
@@ -345,6 +411,7 @@ __device__ __forceinline__ void phase_c(unsigned char* smem_raw, int log2N, int 
     const int64_t k2base = L1 >= SC_CHUNK ? ((int64_t)c * SC_CHUNK) / L1 : (int64_t)c * CW;
     const int k1base = L1 >= SC_CHUNK ? (int)(((int64_t)c * SC_CHUNK) % L1) : 0;
     constexpr int PER = SC_CHUNK / NT;
+    SUBT0();
     {
         double2 v[PER];
 #pragma unroll
@@ -371,6 +438,7 @@ __device__ __forceinline__ void phase_c(unsigned char* smem_raw, int log2N, int 
         base = __ldcg(anchors + c + 1) - ldcg2(Wc + (kn & (L1 - 1)) * L2 + (kn >> log2L1)).x;
     } else base = __ldcg(anchors + nch);                               // X_{N-1}
     __syncthreads();
+    SUBT(16);
     // both halves: inclusive scan of a sequence whose first term is dropped (forward u_q = R_q, q >= 1; backward
     // w_j = R_{CH-j}, j >= 1): P_q = base + incl (forward),  P_{CH-1-j} = base - incl (backward)
     double loc[PER]; double run = 0.0;
@@ -389,6 +457,7 @@ __device__ __forceinline__ void phase_c(unsigned char* smem_raw, int log2N, int 
         else sR[sc_pad(SC_CHUNK - 1 - q, log2K1C, PM)] = base - (off + loc[i]);
     }
     __syncthreads();
+    SUBT(17);
     // natural order: X_{2k} at o[2k-1], P_k = X_{2k+1} at o[2k]; the chunk's 8192 outputs are contiguous from o[2 k0 - 1]
     const int64_t obase = 2 * (int64_t)c * SC_CHUNK - 1;
 #pragma unroll
@@ -398,6 +467,7 @@ __device__ __forceinline__ void phase_c(unsigned char* smem_raw, int log2N, int 
         const double val2 = (j & 1) ? sR[ix] : sX[ix];
         if (obase + j >= 0) __stcs(o + obase + j, val2);
     }
+    SUBT(18);
 }
 
 // ------------------------------------------------------------------------------------------------ the persistent kernel
@@ -504,7 +574,7 @@ dst1_fused_kernel(LargeArgs a) {
         double* anc = a.anchors + (int64_t)slot * (nch + 1);
         const double* x = a.in + (int64_t)col * a.ld_in;
         if (phase == PH_A) phase_a<Q1, TL>(smem_raw, a.log2N, tile, x, Wc, yp, a.tabs);
-        else if (phase == PH_B) phase_b<Q2, TL>(smem_raw, a.log2N, tile, Wc, a.scale, anc + nch);
+        else if (phase == PH_B) phase_b<Q2, TL>(smem_raw, a.log2N, tile, Wc, a.scale, anc + nch, a.tabs);
         else if (phase == PH_D) phase_d<NT, FusedCfg<Q1, Q2, TL>::QM>(smem_raw, a.log2N, Q1, x, yp, a.scale, anc);
         else phase_c<NT>(smem_raw, a.log2N, Q1, tile, Wc, a.out + (int64_t)col * a.ld_out, anc);
         __syncthreads();                                   // every thread's global writes of this item ...
@@ -530,6 +600,9 @@ Plan plan(int log2N) {
     p.nC = (int)(((int64_t)1 << q) / SC_CHUNK);
     return p;
 }
+
+// entries of the two sub-FFT twiddle tables (twA, twB): 64 + NHI each
+size_t sub_table_entries(int q1, int q2) { return (size_t)(64 + ((2 << q1) / 64 + 1)) + (size_t)(64 + ((2 << q2) / 64 + 1)); }
 
 // columns per ring slot
 int group_cols(int64_t N, int batch) {
@@ -566,7 +639,7 @@ size_t dst1_large_ws(int64_t N, int32_t batch) {
     const int64_t L = N / 2;
     const Plan p = plan(lrp_ilog2(N));
     const int64_t L2 = (int64_t)1 << p.q2;
-    const size_t tab = (size_t)(2 * L2 + L2 * 32 + L2 * (((int64_t)1 << p.q1) + 31) / 32);
+    const size_t tab = (size_t)(2 * L2 + L2 * 32 + L2 * (((int64_t)1 << p.q1) + 31) / 32) + sub_table_entries(p.q1, p.q2);
     return lrp_align_up(tab * sizeof(double2)) + lrp_align_up((size_t)2 * gc * L * sizeof(double2)) + lrp_align_up((size_t)2 * gc * 2 * L2 * sizeof(double2)) +
            lrp_align_up((size_t)2 * gc * (p.nC + 1) * sizeof(double)) + lrp_align_up((size_t)(1 + 4 * (size_t)batch + 32) * sizeof(int));
 }
@@ -592,8 +665,10 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
     lrp_arena ar(ws, ws_bytes);
     const int64_t nhi = (((int64_t)1 << p.q1) + 31) / 32;
     const int64_t ntab = 2 * L2 + L2 * 32 + L2 * nhi;
-    double2* twt = ar.take<double2>((size_t)ntab);
+    double2* twt = ar.take<double2>((size_t)ntab + sub_table_entries(p.q1, p.q2));
     a.tabs.gB = twt; a.tabs.g4lo = twt + 2 * L2; a.tabs.g4hi = twt + 2 * L2 + L2 * 32;
+    double2* twA = twt + ntab; double2* twB = twA + 64 + ((2 << p.q1) / 64 + 1);
+    a.tabs.twA = twA; a.tabs.twB = twB;
     a.W = ar.take<double2>((size_t)2 * a.gc * L);
     a.ypart = ar.take<double2>((size_t)2 * a.gc * 2 * L2);
     a.anchors = ar.take<double>((size_t)2 * a.gc * (p.nC + 1));
@@ -612,7 +687,7 @@ int dst1_large(lrp_ctx* ctx, int log2N, int32_t batch, const double* d_in, int64
 #endif
     {
         LRP_PROF(ctx, K_DST_FUSED, 0, 0);
-        dst1_tables_kernel<<<(unsigned)((ntab + 255) / 256), 256, 0, ctx->stream>>>(log2N, p.q1, twt, twt + 2 * L2, twt + 2 * L2 + L2 * 32);
+        dst1_tables_kernel<<<(unsigned)((ntab + 255) / 256), 256, 0, ctx->stream>>>(log2N, p.q1, twt, twt + 2 * L2, twt + 2 * L2 + L2 * 32, twA, twB);
         LRP_LAUNCHED(ctx);
     }
     LRP_PROF(ctx, K_DST_FUSED, 16.0 * (double)N * batch, 0);
