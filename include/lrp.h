@@ -217,6 +217,27 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
                          int32_t* h_trace_I, int32_t* h_trace_J, uint8_t* h_trace_keepI, uint8_t* h_trace_keepJ,
                          double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat);
 
+/* The same solve for a batch of `nprob` INDEPENDENT problems whose factors live in HOST memory (the end-to-end form:
+ * section 3.2, applied to problem after problem; independent problems need no exchange).
+ * Problem p: h_UF[p], h_VF[p] (n x rF, ld = ldu / ldv >= n, column-major), h_SF[p] (rF); results h_UW[p], h_VW[p]
+ * (room for max_rank columns, ld = lduw / ldvw >= n; the leading info[p].rank columns are written), h_SW[p] (max_rank
+ * values of room), info[p].  All problems share n, rF and *opts (opts->d_U0 / d_V0, if set, are DEVICE pointers as usual).
+ * The call owns the copies: the host->device copy of problem p+1 and the device->host copy of problem p-1 run on two
+ * library-owned copy streams while problem p is being solved, through two staging slots carved from the workspace
+ * behind the solve's own (size it with lrp_solve_host_workspace_bytes).  The overlap needs PINNED (page-locked) host
+ * buffers; pageable ones give the same results with the copies serialised.  Output pointers may repeat between
+ * problems that are at least two apart only if the caller no longer needs the earlier result (downloads are ordered).
+ * Synchronous: every result is in host memory on return.  Returns the first error (negative; later problems are then not
+ * run) or else the largest warning code over the batch (LRP_WARN_NOCONV: see info[p].converged). */
+size_t lrp_solve_host_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample);
+int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
+                              const double* const* h_UF, int64_t ldu, const double* const* h_SF,
+                              const double* const* h_VF, int64_t ldv,
+                              const lrp_solve_opts* opts,
+                              double* const* h_UW, int64_t lduw, double* const* h_SW,
+                              double* const* h_VW, int64_t ldvw,
+                              lrp_solve_info* info);
+
 /* Generic function-handle Cross-DEIM (Alg. 4; "G(i,j) as a function handle") on the
  * paper's closed-form test matrices, eq. (6), PAPER.md:264-267 (0-based i, j; square n x n, any n >= K_cap):
  *     LRP_G_HILBERT:  H(i,j) = 1 / (1 + i + j)                        (rapid singular value decay)

@@ -30,6 +30,42 @@ int check_n(int64_t n) {
     return dst1_bluestein_supported(n) ? LRP_OK : LRP_ERR_UNSUPPORTED_N;      // general n: Bluestein, n + 1 <= 2^23
 }
 
+// ------------------------------------------------------------------------------------------------ small copies of a sweep
+// The read-backs (a few KB into ctx->pinned) and uploads (index lists, 32 x 32 factors) of a sweep normally go through
+// cudaMemcpyAsync.  Inside lrp_cross_deim_solve_host the copy engines are busy with the neighbouring problems' factors
+// (hundreds of MB, submitted earlier, served first), so there (ctx->host_pipeline) a read-back is a one-CTA kernel that
+// writes through the device alias of the pinned buffer and an upload travels as kernel parameters.
+constexpr int SMALL_UP_WORDS = 960;                                  // 3840 bytes of payload per launch (parameter space: 4 KB)
+struct SmallPayload { uint32_t w[SMALL_UP_WORDS]; };
+__global__ void __launch_bounds__(256) small_upload_kernel(uint32_t* __restrict__ dst, int nwords, const SmallPayload pl) {
+    for (int i = threadIdx.x; i < nwords; i += blockDim.x) dst[i] = pl.w[i];
+}
+__global__ void __launch_bounds__(256) small_readback_kernel(uint32_t* __restrict__ host_alias, const uint32_t* __restrict__ src, int nwords) {
+    for (int i = threadIdx.x; i < nwords; i += blockDim.x) host_alias[i] = src[i];
+}
+cudaError_t d2h_small(lrp_ctx* ctx, void* h, const void* d, size_t bytes, cudaStream_t s) {
+    const char* pb = (const char*)ctx->pinned;
+    if (ctx->host_pipeline && (bytes & 3) == 0 && bytes <= LRP_PINNED_BYTES && (const char*)h >= pb && (const char*)h + bytes <= pb + LRP_PINNED_BYTES) {
+        small_readback_kernel<<<1, 256, 0, s>>>((uint32_t*)h, (const uint32_t*)d, (int)(bytes / 4));   // cudaHostAlloc memory: same address on the device (UVA)
+        ctx->launches++;
+        return cudaGetLastError();
+    }
+    return cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, s);
+}
+cudaError_t h2d_small(lrp_ctx* ctx, void* d, const void* h, size_t bytes, cudaStream_t s) {
+    if (ctx->host_pipeline && (bytes & 3) == 0 && bytes <= 65536) {
+        for (size_t o = 0; o < bytes; o += sizeof(SmallPayload)) {
+            const size_t len = bytes - o < sizeof(SmallPayload) ? bytes - o : sizeof(SmallPayload);
+            SmallPayload pl;
+            memcpy(pl.w, (const char*)h + o, len);
+            small_upload_kernel<<<1, 256, 0, s>>>((uint32_t*)((char*)d + o), (int)(len / 4), pl);
+            ctx->launches++;
+        }
+        return cudaGetLastError();
+    }
+    return cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, s);
+}
+
 // ------------------------------------------------------------------------------------------------ scross on owned buffers
 struct ScrossWs {
     double *RC, *RR, *Uc, *S, *Vc, *rC, *rR, *scal_d, *core_work, *qr_ws, *qr_ws2;
@@ -74,7 +110,7 @@ int scross_factor(lrp_ctx* ctx, int64_t n, double* Qb, int64_t ldq, int k, int k
     std::vector<double> pageable;
     double* hb = ctx->pinned;
     if (blk > LRP_PINNED_BYTES) { pageable.resize(blk / sizeof(double)); hb = pageable.data(); }
-    LRP_CUDA(ctx, cudaMemcpyAsync(hb, w.S, blk, cudaMemcpyDeviceToHost, ctx->stream));
+    LRP_CUDA(ctx, d2h_small(ctx, hb, w.S, blk, ctx->stream));
     LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     memcpy(h_S, hb, sizeof(double) * p);
     memcpy(h_rC, hb + w.Kblk, sizeof(double) * k);
@@ -262,6 +298,8 @@ int lrp_create(lrp_ctx** out, int device, void* cuda_stream) {
     c->ev = new std::vector<cudaEvent_t>(); c->ev_id = new std::vector<int>(); c->ev_used = 0;
     c->flags = 0; c->solve_ev = new std::vector<cudaEvent_t>();
     for (int q = 0; q < 2; ++q) { c->hi[q] = nullptr; c->ev_hi[q][0] = nullptr; c->ev_hi[q][1] = nullptr; }
+    c->cp_in = nullptr; c->cp_out = nullptr; c->host_pipeline = 0;
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) c->ev_cp[a][b] = nullptr;
     c->aux = nullptr; c->aux2 = nullptr; c->ev_fork = nullptr; c->ev_join = nullptr; c->ev_join2 = nullptr; c->pinned = nullptr; c->d_counters = nullptr;
     if (cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->aux2, cudaStreamNonBlocking) != cudaSuccess ||
@@ -297,6 +335,9 @@ int lrp_destroy(lrp_ctx* ctx) {
         if (ctx->ev_hi[q][0]) cudaEventDestroy(ctx->ev_hi[q][0]);
         if (ctx->ev_hi[q][1]) cudaEventDestroy(ctx->ev_hi[q][1]);
     }
+    if (ctx->cp_in) cudaStreamDestroy(ctx->cp_in);
+    if (ctx->cp_out) cudaStreamDestroy(ctx->cp_out);
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) if (ctx->ev_cp[a][b]) cudaEventDestroy(ctx->ev_cp[a][b]);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     if (ctx->aux2) cudaStreamDestroy(ctx->aux2);
     if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);
@@ -548,13 +589,13 @@ static int leverage_cholqr2_pair(lrp_ctx* ctx, int64_t n, int c, const double* A
         double* hV = pin ? ctx->pinned + (size_t)c * c : gV.data();
         LRP_TRY(tall_gemm_t(ctx, n, srcU, lsrc, c, srcU, lsrc, c, w.GU, c, 0, w.gemmt_ws));
         LRP_ON_STREAM(ctx, side, tall_gemm_t(ctx, n, srcV, lsrc, c, srcV, lsrc, c, w.GV, c, 0, w.gemmt_ws2));
-        LRP_CUDA(ctx, cudaMemcpyAsync(hU, w.GU, gb, cudaMemcpyDeviceToHost, ctx->stream));
-        LRP_CUDA(ctx, cudaMemcpyAsync(hV, w.GV, gb, cudaMemcpyDeviceToHost, side));
+        LRP_CUDA(ctx, d2h_small(ctx, hU, w.GU, gb, ctx->stream));
+        LRP_CUDA(ctx, d2h_small(ctx, hV, w.GV, gb, side));
         LRP_TRY(join_sync());
         if (pin) { memcpy(gU.data(), hU, gb); memcpy(gV.data(), hV, gb); }
         if (!host_chol_inverse(gU, c, iU) || !host_chol_inverse(gV, c, iV)) return 1;
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.Amat, iU.data(), gb, cudaMemcpyHostToDevice, ctx->stream));
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.Bmat, iV.data(), gb, cudaMemcpyHostToDevice, ctx->stream));
+        LRP_CUDA(ctx, h2d_small(ctx, w.Amat, iU.data(), gb, ctx->stream));
+        LRP_CUDA(ctx, h2d_small(ctx, w.Bmat, iV.data(), gb, ctx->stream));
         LRP_TRY(fork());
         if (pass == 0) {
             LRP_TRY(rebuild(ctx, n, srcU, lsrc, c, w.Amat, c, c, w.Ua, ld, nullptr));
@@ -672,9 +713,9 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             if (topk_pair) {
                 int32_t* hp = reinterpret_cast<int32_t*>(ctx->pinned);
                 LRP_TRY(select_topk(ctx, n, w.scoresU, numsel, w.dIstar, w.sel_ws));
-                LRP_CUDA(ctx, cudaMemcpyAsync(hp, w.dIstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                LRP_CUDA(ctx, d2h_small(ctx, hp, w.dIstar, sizeof(int32_t) * numsel, ctx->stream));
                 LRP_TRY(select_topk(ctx, n, w.scoresV, numsel, w.dJstar, w.sel_ws));
-                LRP_CUDA(ctx, cudaMemcpyAsync(hp + numsel, w.dJstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                LRP_CUDA(ctx, d2h_small(ctx, hp + numsel, w.dJstar, sizeof(int32_t) * numsel, ctx->stream));
                 LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
             }
             for (int side = 0; side < 2; ++side) {
@@ -712,7 +753,7 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
                 } else {
                     LRP_TRY(select_topk(ctx, n, sc, numsel, dstar, w.sel_ws));
                     const bool pin = sizeof(int32_t) * (size_t)numsel <= LRP_PINNED_BYTES;
-                    LRP_CUDA(ctx, cudaMemcpyAsync(pin ? (void*)ctx->pinned : (void*)hstar.data(), dstar, sizeof(int32_t) * numsel, cudaMemcpyDeviceToHost, ctx->stream));
+                    LRP_CUDA(ctx, d2h_small(ctx, pin ? (void*)ctx->pinned : (void*)hstar.data(), dstar, sizeof(int32_t) * numsel, ctx->stream));
                     LRP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
                     if (pin) memcpy(hstar.data(), ctx->pinned, sizeof(int32_t) * numsel);
                 }
@@ -747,8 +788,8 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             LRP_TRY(validate_indices(J_k.data(), nJ, n));
         }
         const int l = (int)I_k.size(), kk = (int)J_k.size();
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.dI, I_k.data(), sizeof(int32_t) * l, cudaMemcpyHostToDevice, ctx->stream));
-        LRP_CUDA(ctx, cudaMemcpyAsync(w.dJ, J_k.data(), sizeof(int32_t) * kk, cudaMemcpyHostToDevice, ctx->stream));
+        LRP_CUDA(ctx, h2d_small(ctx, w.dI, I_k.data(), sizeof(int32_t) * l, ctx->stream));
+        LRP_CUDA(ctx, h2d_small(ctx, w.dJ, J_k.data(), sizeof(int32_t) * kk, ctx->stream));
         cudaEvent_t e1 = ep.rec(ctx);
         // ---- O4: fibers  C = G(:,J) (n x kk), Rt = G(I,:)^T (n x l)
         // the two sides of a sweep are independent until the small core: they run on the main and the auxiliary stream
@@ -812,8 +853,8 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
             cudaStream_t main_stream = ctx->stream;
             ctx->stream = side2;
             int rc_eta = LRP_OK;
-            cudaError_t e1 = cudaMemcpyAsync(w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
-            cudaError_t e2 = cudaMemcpyAsync(w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), cudaMemcpyHostToDevice, ctx->stream);
+            cudaError_t e1 = h2d_small(ctx, w.dIpr, I_pr.data(), sizeof(int32_t) * I_pr.size(), ctx->stream);
+            cudaError_t e2 = h2d_small(ctx, w.dJpr, J_pr.data(), sizeof(int32_t) * J_pr.size(), ctx->stream);
             if (e1 != cudaSuccess || e2 != cudaSuccess) { ctx->last_cuda = (int)(e1 != cudaSuccess ? e1 : e2); rc_eta = LRP_ERR_CUDA; }
             if (rc_eta == LRP_OK) {
                 EtaArgs ea{};
@@ -911,7 +952,7 @@ static int solve_impl(lrp_ctx* ctx, int kind, int64_t n, int32_t rF, const doubl
         LRP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join2, 0));
         LRP_TRY(rho_small(ctx, ra));
         double h_rho[2], h_eta[2];
-        LRP_CUDA(ctx, cudaMemcpyAsync(ctx->pinned, w.rho_out, sizeof(double) * 16, cudaMemcpyDeviceToHost, ctx->stream));
+        LRP_CUDA(ctx, d2h_small(ctx, ctx->pinned, w.rho_out, sizeof(double) * 16, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.Sprev, w.sc.S, sizeof(double) * rank, cudaMemcpyDeviceToDevice, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.UcPrev, w.sc.Uc, sizeof(double) * (size_t)kk * rank, cudaMemcpyDeviceToDevice, ctx->stream));
         LRP_CUDA(ctx, cudaMemcpyAsync(w.VcPrev, w.sc.Vc, sizeof(double) * (size_t)l * rank, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -985,6 +1026,97 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF, const double* d_UF
                          double* d_Uhat, double* d_Shat, double* d_Vhat, int64_t ld_hat) {
     return solve_impl(ctx, LRP_G_POISSON, n, rF, d_UF, ldu, d_SF, d_VF, ldv, opts, d_UW, lduw, d_SW, d_VW, ldvw, info,
                       h_trace_I, h_trace_J, h_trace_keepI, h_trace_keepJ, d_Uhat, d_Shat, d_Vhat, ld_hat);
+}
+
+// ------------------------------------------------------------------------------------------------ host-buffer pipeline
+// Staging after the solve's own workspace: two slots of (UF, VF, SF) and two of (UW, VW, SW), ld = n.
+namespace {
+struct HostStage { double* UF[2]; double* VF[2]; double* SF[2]; double* UW[2]; double* VW[2]; double* SW[2]; };
+bool carve_stage(lrp_arena& ar, int64_t n, int rF, int max_rank, HostStage* st) {
+    for (int s = 0; s < 2; ++s) {
+        double* a = ar.take<double>((size_t)n * rF); double* b = ar.take<double>((size_t)n * rF); double* c = ar.take<double>((size_t)rF);
+        double* d = ar.take<double>((size_t)n * max_rank); double* e = ar.take<double>((size_t)n * max_rank); double* f = ar.take<double>((size_t)max_rank);
+        if (st) { st->UF[s] = a; st->VF[s] = b; st->SF[s] = c; st->UW[s] = d; st->VW[s] = e; st->SW[s] = f; }
+    }
+    return ar.ok();
+}
+// tall block (cols columns of n doubles) between host and device on a copy engine
+cudaError_t copy_tall_async(double* dst, int64_t ldd, const double* src, int64_t lds, int64_t n, int cols, cudaMemcpyKind kind, cudaStream_t s) {
+    if (cols <= 0) return cudaSuccess;
+    if (ldd == n && lds == n) return cudaMemcpyAsync(dst, src, sizeof(double) * (size_t)n * cols, kind, s);
+    return cudaMemcpy2DAsync(dst, sizeof(double) * (size_t)ldd, src, sizeof(double) * (size_t)lds, sizeof(double) * (size_t)n, (size_t)cols, kind, s);
+}
+}  // namespace
+
+size_t lrp_solve_host_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample) {
+    const size_t base = lrp_workspace_bytes(n, rF, max_rank, oversample);
+    if (!base) return 0;
+    lrp_arena ar((void*)256, (size_t)-1 / 2);
+    carve_stage(ar, n, rF, max_rank, nullptr);
+    return lrp_align_up(base) + ar.off + 256;
+}
+
+int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
+                              const double* const* h_UF, int64_t ldu, const double* const* h_SF, const double* const* h_VF, int64_t ldv,
+                              const lrp_solve_opts* opts,
+                              double* const* h_UW, int64_t lduw, double* const* h_SW, double* const* h_VW, int64_t ldvw,
+                              lrp_solve_info* info) {
+    if (!ctx || !opts || !info || nprob < 0 || !h_UF || !h_SF || !h_VF || !h_UW || !h_SW || !h_VW) return LRP_ERR_BADARG;
+    if (ldu < n || ldv < n || lduw < n || ldvw < n || rF < 1 || opts->max_rank < 1) return LRP_ERR_BADARG;
+    for (int p = 0; p < nprob; ++p)
+        if (!h_UF[p] || !h_SF[p] || !h_VF[p] || !h_UW[p] || !h_SW[p] || !h_VW[p]) return LRP_ERR_BADARG;
+    LRP_TRY(check_n(n));
+    if (nprob == 0) return LRP_OK;
+    const int max_rank = opts->max_rank;
+    const size_t base = lrp_workspace_bytes(n, rF, max_rank, opts->oversample);
+    if (!base || ctx->ws_bytes < lrp_solve_host_workspace_bytes(n, rF, max_rank, opts->oversample)) return LRP_ERR_WORKSPACE;
+    HostStage st;
+    {
+        const size_t off = lrp_align_up(base);
+        lrp_arena ar((char*)ctx->ws + off, ctx->ws_bytes - off);
+        if (!carve_stage(ar, n, rF, max_rank, &st)) return LRP_ERR_WORKSPACE;
+    }
+    if (!ctx->cp_in) {                                   // first call on this ctx: two copy streams, four events
+        LRP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cp_in, cudaStreamNonBlocking));
+        LRP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cp_out, cudaStreamNonBlocking));
+        for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) LRP_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_cp[a][b], cudaEventDisableTiming));
+    }
+    // The solve carves only the first `base` bytes of the workspace; the staging slots behind them are this call's own.
+    auto upload = [&](int p) -> int {
+        const int s = p & 1;
+        LRP_CUDA(ctx, copy_tall_async(st.UF[s], n, h_UF[p], ldu, n, rF, cudaMemcpyHostToDevice, ctx->cp_in));
+        LRP_CUDA(ctx, copy_tall_async(st.VF[s], n, h_VF[p], ldv, n, rF, cudaMemcpyHostToDevice, ctx->cp_in));
+        LRP_CUDA(ctx, cudaMemcpyAsync(st.SF[s], h_SF[p], sizeof(double) * rF, cudaMemcpyHostToDevice, ctx->cp_in));
+        LRP_CUDA(ctx, cudaEventRecord(ctx->ev_cp[0][s], ctx->cp_in));
+        return LRP_OK;
+    };
+    int worst = LRP_OK, rc = upload(0);
+    for (int p = 0; p < nprob && rc >= 0; ++p) {
+        const int s = p & 1;
+        if (cudaStreamWaitEvent(ctx->stream, ctx->ev_cp[0][s], 0) != cudaSuccess) rc = LRP_ERR_CUDA;         // inputs of p are on the device
+        // slot s^1 was read by solve p-1, complete on return: problem p+1 uploads while problem p is solved
+        if (rc >= 0 && p + 1 < nprob) rc = upload(p + 1);
+        // slot s of the outputs was drained by the download of problem p-2
+        if (rc >= 0 && p >= 2 && cudaStreamWaitEvent(ctx->stream, ctx->ev_cp[1][s], 0) != cudaSuccess) rc = LRP_ERR_CUDA;
+        if (rc < 0) break;
+        ctx->host_pipeline = 1;                          // the sweep's small copies keep off the copy engines (d2h_small / h2d_small)
+        rc = lrp_cross_deim_solve(ctx, n, rF, st.UF[s], n, st.SF[s], st.VF[s], n, opts, st.UW[s], n, st.SW[s], st.VW[s], n, &info[p],
+                                  nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+        ctx->host_pipeline = 0;
+        if (rc < 0) break;
+        if (rc > worst) worst = rc;
+        const int r = info[p].rank;                      // the solve is synchronous: rank known, outputs complete
+        cudaError_t e = cudaSuccess;
+        if (e == cudaSuccess) e = copy_tall_async(h_UW[p], lduw, st.UW[s], n, n, r, cudaMemcpyDeviceToHost, ctx->cp_out);
+        if (e == cudaSuccess) e = copy_tall_async(h_VW[p], ldvw, st.VW[s], n, n, r, cudaMemcpyDeviceToHost, ctx->cp_out);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_SW[p], st.SW[s], sizeof(double) * r, cudaMemcpyDeviceToHost, ctx->cp_out);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_cp[1][s], ctx->cp_out);
+        if (e != cudaSuccess) { ctx->last_cuda = (int)e; rc = LRP_ERR_CUDA; }
+    }
+    // drain both copy streams whatever happened: nothing of this call is in flight on return
+    cudaError_t e1 = cudaStreamSynchronize(ctx->cp_in), e2 = cudaStreamSynchronize(ctx->cp_out);
+    if (rc >= 0 && (e1 != cudaSuccess || e2 != cudaSuccess)) { ctx->last_cuda = (int)(e1 != cudaSuccess ? e1 : e2); rc = LRP_ERR_CUDA; }
+    return rc < 0 ? rc : worst;
 }
 
 int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve_opts* opts,

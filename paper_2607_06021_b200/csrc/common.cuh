@@ -49,6 +49,9 @@ struct lrp_ctx {
     std::vector<int>* ev_id;
     size_t ev_used;
     std::vector<cudaEvent_t>* solve_ev;   // timing events of lrp_cross_deim_solve (created once, reused by every solve)
+    int host_pipeline;                    // 1 while lrp_cross_deim_solve_host runs its solves: small copies avoid the copy engines
+    cudaStream_t cp_in, cp_out;           // copy streams of lrp_cross_deim_solve_host (created on its first call)
+    cudaEvent_t ev_cp[2][2];              // [inputs arrived / outputs copied][staging slot]
 };
 
 // call right before a kernel launch: accounts the launch and, when profiling is on, records its start event

@@ -34,7 +34,8 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_leverage_select", "lrp_scross", "lrp_cross_deim_solve", "lrp_lowrank_entries",
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
            "lrp_profile_timeline", "lrp_fp64_peak", "lrp_matrix_workspace_bytes", "lrp_cross_deim_matrix",
-           "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson", "lrp_topk_static"]
+           "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson", "lrp_topk_static",
+           "lrp_solve_host_workspace_bytes", "lrp_cross_deim_solve_host"]
 
 
 class SolveOpts(C.Structure):
@@ -92,6 +93,9 @@ def load_library():
     lib.lrp_cross_deim_solve.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64,
                                          C.POINTER(SolveInfo), vp, vp, vp, vp, vp, vp, vp, i64]
     lib.lrp_cross_deim_solve.restype = C.c_int
+    lib.lrp_solve_host_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_solve_host_workspace_bytes.restype = sz
+    lib.lrp_cross_deim_solve_host.argtypes = [vp, i64, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+    lib.lrp_cross_deim_solve_host.restype = C.c_int
     lib.lrp_matrix_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_matrix_workspace_bytes.restype = sz
     lib.lrp_cross_deim_matrix.argtypes = [vp, i32, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64, C.POINTER(SolveInfo),
                                           vp, vp, vp, vp, vp, vp, vp, i64]
@@ -371,6 +375,55 @@ class Context:
         return self._run_solve(n, UF.device, 2 * (max_rank + oversample), max_rank, call, tol=tol, oversample=oversample,
                                max_sweeps=max_sweeps, safeguard=safeguard, tol_mode=tol_mode, U0=U0, V0=V0, replay=replay,
                                want_spectral=want_spectral, flags=flags, selection=selection, ls_seed=ls_seed, ls_c=ls_c)
+
+    def cross_deim_solve_host(self, problems, outputs, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
+                              tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0):
+        """lrp_cross_deim_solve_host: a batch of independent low-rank Poisson solves whose factors live in HOST memory.
+        problems: list of (UF, SF, VF) CPU float64 tensors, UF / VF tall (rF, n) with contiguous rows, SF (rF,);
+        outputs: list of (UW, SW, VW) CPU tensors of the same length, UW / VW (max_rank, n), SW (max_rank,) -- entries may
+        repeat (a pool of >= 2 buffers) when earlier results are no longer needed.  Pinned tensors let the copies of the
+        neighbouring problems overlap the solve; pageable ones work without overlap.  Returns one dict per problem
+        (rank, sweeps, converged, info); the leading `rank` rows of its output tensors hold the factors."""
+        torch = _torch()
+
+        def chk(t, name, rows=None):
+            if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+                raise ValueError(f"{name}: expected a contiguous CPU float64 tensor")
+            if rows is not None and (t.dim() != 2 or t.shape[0] != rows[0] or t.shape[1] != rows[1]):
+                raise ValueError(f"{name}: expected shape {rows}")
+        if len(problems) != len(outputs):
+            raise ValueError("problems and outputs must have the same length")
+        if not problems:
+            return []
+        rF, n = problems[0][0].shape
+        for UF, SF, VF in problems:
+            chk(UF, "UF", (rF, n)); chk(VF, "VF", (rF, n)); chk(SF, "SF")
+            if SF.numel() != rF:
+                raise ValueError("SF: expected rF values")
+        for UW, SW, VW in outputs:
+            chk(UW, "UW", (max_rank, n)); chk(VW, "VW", (max_rank, n)); chk(SW, "SW")
+            if SW.numel() < max_rank:
+                raise ValueError("SW: expected max_rank values of room")
+        self.ensure_workspace(self.lib.lrp_solve_host_workspace_bytes(n, rF, max_rank, oversample))
+        o = SolveOpts()
+        o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
+        o.flags = int(flags)
+        o.selection = SELECTIONS[selection] if isinstance(selection, str) else int(selection)
+        o.ls_seed, o.ls_c = int(ls_seed), float(ls_c)
+        sg = None
+        if safeguard is not None:
+            sg = np.ascontiguousarray(safeguard, dtype=np.int32)
+            o.h_safeguard, o.n_safeguard = sg.ctypes.data, sg.size
+        P = len(problems)
+        arr = lambda ts: (C.c_void_p * P)(*[t.data_ptr() for t in ts])
+        hUF, hSF, hVF = arr([p[0] for p in problems]), arr([p[1] for p in problems]), arr([p[2] for p in problems])
+        hUW, hSW, hVW = arr([q[0] for q in outputs]), arr([q[1] for q in outputs]), arr([q[2] for q in outputs])
+        infos = (SolveInfo * P)()
+        rc = self._check(self.lib.lrp_cross_deim_solve_host(self.h, n, rF, P, hUF, n, hSF, hVF, n, C.byref(o),
+                                                            hUW, n, hSW, hVW, n, infos), "lrp_cross_deim_solve_host")
+        del sg
+        return [dict(rank=infos[p].rank, sweeps=infos[p].sweeps, converged=bool(infos[p].converged), code=rc, info=infos[p])
+                for p in range(P)]
 
     def cross_deim_matrix(self, kind, n, U0, V0, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
                           tol_mode=0, replay=None, want_spectral=False, flags=0, selection="topk", ls_seed=0, ls_c=0.0):
