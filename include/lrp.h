@@ -222,14 +222,19 @@ int lrp_cross_deim_solve(lrp_ctx* ctx, int64_t n, int32_t rF,
  * Problem p: h_UF[p], h_VF[p] (n x rF, ld = ldu / ldv >= n, column-major), h_SF[p] (rF); results h_UW[p], h_VW[p]
  * (room for max_rank columns, ld = lduw / ldvw >= n; the leading info[p].rank columns are written), h_SW[p] (max_rank
  * values of room), info[p].  All problems share n, rF and *opts (opts->d_U0 / d_V0, if set, are DEVICE pointers as usual).
- * The call owns the copies: the host->device copy of problem p+1 and the device->host copy of problem p-1 run on two
- * library-owned copy streams while problem p is being solved, through two staging slots carved from the workspace
- * behind the solve's own (size it with lrp_solve_host_workspace_bytes).  The overlap needs PINNED (page-locked) host
- * buffers; pageable ones give the same results with the copies serialised.  Output pointers may repeat between
- * problems that are at least two apart only if the caller no longer needs the earlier result (downloads are ordered).
- * Synchronous: every result is in host memory on return.  Returns the first error (negative; later problems are then not
- * run) or else the largest warning code over the batch (LRP_WARN_NOCONV: see info[p].converged). */
-size_t lrp_solve_host_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample);
+ * The call owns the copies.  A LANE solves its problems one after the other through two staging slots carved from the
+ * workspace behind the solve's own, with the host->device copy of its next problem and the device->host copy of its
+ * previous one on two library-owned copy streams while the current one is solved.  With a workspace of
+ * lrp_solve_host_workspace_bytes(..., 2) and nprob >= 2 there are TWO lanes (even / odd problems; the second on a
+ * library-owned context and stream, driven by a worker thread that lives for the call): two solves in flight fill the
+ * SMs that one leaves idle.  With lrp_solve_host_workspace_bytes(..., 1) there is one lane.  Results do not depend on the
+ * number of lanes.  The overlap needs PINNED (page-locked) host buffers; pageable ones give the same results with the
+ * copies serialised.  Output pointers may repeat between problems p and q only if p - q is a multiple of 2 and the
+ * earlier result is no longer needed (downloads of one lane are ordered).
+ * Synchronous: every result is in host memory on return.  Returns the first error of a lane (negative; that lane's later
+ * problems are then not run) or else the largest warning code over the batch (LRP_WARN_NOCONV: see info[p].converged). */
+#define LRP_HOST_LANES_MAX 2
+size_t lrp_solve_host_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample, int32_t lanes);
 int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
                               const double* const* h_UF, int64_t ldu, const double* const* h_SF,
                               const double* const* h_VF, int64_t ldv,

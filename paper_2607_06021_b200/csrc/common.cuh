@@ -50,6 +50,8 @@ struct lrp_ctx {
     size_t ev_used;
     std::vector<cudaEvent_t>* solve_ev;   // timing events of lrp_cross_deim_solve (created once, reused by every solve)
     int host_pipeline;                    // 1 while lrp_cross_deim_solve_host runs its solves: small copies avoid the copy engines
+    lrp_ctx* lane2;                       // second solver lane of lrp_cross_deim_solve_host: library-owned context + its stream
+    cudaStream_t lane2_stream;
     cudaStream_t cp_in, cp_out;           // copy streams of lrp_cross_deim_solve_host (created on its first call)
     cudaEvent_t ev_cp[2][2];              // [inputs arrived / outputs copied][staging slot]
 };

@@ -93,7 +93,7 @@ def load_library():
     lib.lrp_cross_deim_solve.argtypes = [vp, i64, i32, vp, i64, vp, vp, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64,
                                          C.POINTER(SolveInfo), vp, vp, vp, vp, vp, vp, vp, i64]
     lib.lrp_cross_deim_solve.restype = C.c_int
-    lib.lrp_solve_host_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_solve_host_workspace_bytes.restype = sz
+    lib.lrp_solve_host_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]; lib.lrp_solve_host_workspace_bytes.restype = sz
     lib.lrp_cross_deim_solve_host.argtypes = [vp, i64, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_cross_deim_solve_host.restype = C.c_int
     lib.lrp_matrix_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_matrix_workspace_bytes.restype = sz
@@ -237,9 +237,11 @@ class Context:
                 out[name.value.decode()] = dict(count=cnt.value, ms=ms.value, bytes=by.value, flops=fl.value)
         return out
 
-    def ensure_workspace(self, nbytes: int):
+    def ensure_workspace(self, nbytes: int, exact: bool = False):
+        """Grow the workspace tensor to nbytes (exact: make it exactly nbytes -- lrp_cross_deim_solve_host reads the
+        number of lanes off the workspace size)."""
         torch = _torch()
-        if self._ws is None or self._ws.numel() < nbytes:
+        if self._ws is None or self._ws.numel() < nbytes or (exact and self._ws.numel() != nbytes):
             self._ws = None
             self._ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
             self._check(self.lib.lrp_set_workspace(self.h, _ptr(self._ws), self._ws.numel()), "lrp_set_workspace")
@@ -377,13 +379,14 @@ class Context:
                                want_spectral=want_spectral, flags=flags, selection=selection, ls_seed=ls_seed, ls_c=ls_c)
 
     def cross_deim_solve_host(self, problems, outputs, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                              tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0):
+                              tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0, lanes=2):
         """lrp_cross_deim_solve_host: a batch of independent low-rank Poisson solves whose factors live in HOST memory.
         problems: list of (UF, SF, VF) CPU float64 tensors, UF / VF tall (rF, n) with contiguous rows, SF (rF,);
         outputs: list of (UW, SW, VW) CPU tensors of the same length, UW / VW (max_rank, n), SW (max_rank,) -- entries may
         repeat (a pool of >= 2 buffers) when earlier results are no longer needed.  Pinned tensors let the copies of the
         neighbouring problems overlap the solve; pageable ones work without overlap.  Returns one dict per problem
-        (rank, sweeps, converged, info); the leading `rank` rows of its output tensors hold the factors."""
+        (rank, sweeps, converged, info); the leading `rank` rows of its output tensors hold the factors.  lanes: 1 or 2
+        solves in flight (sizes the workspace; include/lrp.h); outputs may repeat only between problems an even distance apart."""
         torch = _torch()
 
         def chk(t, name, rows=None):
@@ -404,7 +407,10 @@ class Context:
             chk(UW, "UW", (max_rank, n)); chk(VW, "VW", (max_rank, n)); chk(SW, "SW")
             if SW.numel() < max_rank:
                 raise ValueError("SW: expected max_rank values of room")
-        self.ensure_workspace(self.lib.lrp_solve_host_workspace_bytes(n, rF, max_rank, oversample))
+        need = self.lib.lrp_solve_host_workspace_bytes(n, rF, max_rank, oversample, int(lanes))
+        if need == 0:
+            raise LrpError(-1, "lrp_solve_host_workspace_bytes (unsupported n, rank cap or lane count)")
+        self.ensure_workspace(need, exact=True)
         o = SolveOpts()
         o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
         o.flags = int(flags)

@@ -34,19 +34,19 @@ def _host_output(w, pinned):
     return tuple(t.pin_memory() if pinned else t for t in (UW, SW, VW))
 
 
-@pytest.mark.parametrize("pinned", [True, False])
-def test_host_batch_matches_device_call(ctx, pinned):
-    """Five problems (different seeds) through two staging slots: every slot is reused at least once; results equal the
-    device-pointer call's, problem by problem."""
+@pytest.mark.parametrize("pinned,lanes", [(True, 2), (True, 1), (False, 2)])
+def test_host_batch_matches_device_call(ctx, pinned, lanes):
+    """Seven problems (different seeds) through the staging slots of one or two lanes: every slot is reused at least
+    once; results equal the device-pointer call's, problem by problem, whatever the number of lanes."""
     import torch
     from paper_2607_06021_b200 import lrp
-    ws = [W.make("C2", seed) for seed in range(5)]
+    ws = [W.make("C2", seed) for seed in range(7)]
     w0 = ws[0]
     kw = dict(tol=w0.tol, max_rank=w0.max_rank, oversample=w0.oversample, max_sweeps=w0.max_sweeps, safeguard=w0.safeguard)
     probs = [_host_problem(w, pinned) for w in ws]
     outs = [_host_output(w, pinned) for w in ws]
-    res = ctx.cross_deim_solve_host(probs, outs, **kw)
-    assert len(res) == 5
+    res = ctx.cross_deim_solve_host(probs, outs, lanes=lanes, **kw)
+    assert len(res) == 7
     for w, r, (UW, SW, VW) in zip(ws, res, outs):
         dev = ctx.cross_deim_solve(lrp.tall_from_numpy(w.UF), torch.from_numpy(w.SF).cuda(), lrp.tall_from_numpy(w.VF), **kw)
         k = r["rank"]
@@ -57,8 +57,9 @@ def test_host_batch_matches_device_call(ctx, pinned):
 
 
 def test_host_batch_output_pool_and_oracle(ctx):
-    """Outputs drawn from a pool of two buffers (the documented reuse): the last two problems' results survive; one of
-    them is compared with the CPU oracle entry by entry at the parity bar of the converged C2 runs (1e-10)."""
+    """Outputs drawn from a pool of two buffers, problem p in buffer p mod 2 (the documented reuse: same lane, ordered
+    downloads): the last two problems' results survive; one of them is compared with the CPU oracle entry by entry at the
+    parity bar of the converged C2 runs (1e-10)."""
     from paper_2607_06021_b200 import lrp
     ws = [W.make("C2", seed) for seed in (3, 4, 5, 6)]
     w0 = ws[0]
@@ -83,10 +84,12 @@ def test_host_batch_argument_errors(ctx):
     import torch
     from paper_2607_06021_b200 import lrp
     w = W.make("C1", 0)
-    need = ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], w.max_rank, w.oversample)
+    need = ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], w.max_rank, w.oversample, 1)
     base = ctx.lib.lrp_workspace_bytes(w.n, w.UF.shape[1], w.max_rank, w.oversample)
     assert need > base > 0
-    assert ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], 1, 0) == 0      # K_cap = 2 < rF + 1: the first selection would not fit
+    assert ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], w.max_rank, w.oversample, 2) == 2 * need
+    assert ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], w.max_rank, w.oversample, 3) == 0     # at most two lanes
+    assert ctx.lib.lrp_solve_host_workspace_bytes(w.n, w.UF.shape[1], 1, 0, 1) == 0      # K_cap = 2 < rF + 1: the first selection would not fit
     small = torch.empty(base, dtype=torch.uint8, device="cuda")
     ctx.lib.lrp_set_workspace(ctx.h, C.c_void_p(small.data_ptr()), small.numel())
     ctx._ws = small
