@@ -252,7 +252,7 @@ def run_reference(args):
     return 0
 
 
-def dst_measure(ctx, torch, dev, stream, p: int, batch: int, inplace: bool, hbm_peak: float, reps: int = 10):
+def dst_measure(ctx, torch, dev, stream, p: int, batch: int, inplace: bool, hbm_peak: float, reps: int = 10, library: bool = False):
     """Batched DST-I at n = 2^p - 1: buffer sets rotate over >= 4x the L2 so that every repetition starts L2-cold."""
     nd = (1 << p) - 1
     per_set = batch * nd * 8 * (1 if inplace else 2)
@@ -271,8 +271,42 @@ def dst_measure(ctx, torch, dev, stream, p: int, batch: int, inplace: bool, hbm_
     d1.record(stream); torch.cuda.synchronize(dev)
     dms = d0.elapsed_time(d1) / reps
     gbs = 16.0 * nd * batch / (dms * 1e-3) / 1e9
-    return {"p": p, "n": nd, "batch": batch, "in_place": inplace, "ms": dms, "alg_GBps": gbs, "frac_of_hbm_peak": gbs / hbm_peak,
-            "frac_of_8TBps": gbs / 8000.0, "buffer_sets": nsets, "footprint_MB": nsets * per_set / 1e6}
+    out = {"p": p, "n": nd, "batch": batch, "in_place": inplace, "ms": dms, "alg_GBps": gbs, "frac_of_hbm_peak": gbs / hbm_peak,
+           "frac_of_8TBps": gbs / 8000.0, "buffer_sets": nsets, "footprint_MB": nsets * per_set / 1e6}
+    if library and not inplace:
+        x0 = xs[0]; y0 = ys[0].clone()
+        del xs, ys
+        out["library_route"] = dst_library_route(torch, dev, stream, x0, y0, reps)
+    return out
+
+
+def dst_library_route(torch, dev, stream, x, ours, reps: int):
+    """The route the paper itself takes (library FFT calls from PyTorch), timed beside the
+    kernel as a baseline, never on the product path: DST-I of every row of x (batch, n) as the imaginary part of a real
+    FFT of the odd extension of length 2(n+1), torch.fft.rfft = cuFFT D2Z.  `ms` covers extension + FFT + extraction,
+    `rfft_only_ms` the library transform alone; `max_rel_diff` compares its result with lrp_dst1_batched's."""
+    batch, nd = x.shape
+    N = nd + 1
+    def route():
+        ext = torch.zeros((batch, 2 * N), dtype=torch.float64, device=dev)
+        ext[:, 1:N] = x
+        ext[:, N + 1:] = -torch.flip(x, dims=(1,))
+        return ext, -0.5 * torch.fft.rfft(ext, dim=1).imag[:, 1:N]
+    ext, lib = route()
+    diff = float((lib - ours).abs().max() / ours.abs().max())
+    del lib
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    torch.cuda.synchronize(dev)
+    reps = max(3, min(reps, 10))
+    e0.record(stream)
+    for _ in range(reps):
+        ext, lib = route(); del lib
+    e1.record(stream)
+    for _ in range(reps):
+        f = torch.fft.rfft(ext, dim=1); del f
+    e2.record(stream); torch.cuda.synchronize(dev)
+    return {"kind": "torch.fft.rfft (cuFFT D2Z) of the odd extension of length 2(n+1): the paper's own route, PAPER.md:226-228",
+            "ms": e0.elapsed_time(e1) / reps, "rfft_only_ms": e1.elapsed_time(e2) / reps, "max_rel_diff": diff}
 
 
 def main():
@@ -312,7 +346,7 @@ def main():
         if rank == 0:
             for p_ in range(12, 23):
                 for inplace in (False, True):
-                    print(json.dumps(dst_measure(ctx, torch, dev, stream, p_, 128, inplace, hbm_peak)), flush=True)
+                    print(json.dumps(dst_measure(ctx, torch, dev, stream, p_, 128, inplace, hbm_peak, library=True)), flush=True)
         ctx.close()
         return 0
 
@@ -428,7 +462,7 @@ def main():
     dst = []
     try:
         for p_ in [int(v) for v in args.dst_p.split(",") if v]:
-            dst.append(dst_measure(ctx, torch, dev, stream, p_, 128, False, hbm_peak))
+            dst.append(dst_measure(ctx, torch, dev, stream, p_, 128, False, hbm_peak, library=True))
     except Exception as ex:                       # never lose the main line because of the side measurement
         dst.append({"error": str(ex)})
 
