@@ -123,25 +123,36 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
     SUBT(0);
     // fold: t_m = sin(pi m/N)(x_m + x_{N-m}) + (x_m - x_{N-m})/2 for m = 2j, 2j+1;  z_j = t_{2j} + i t_{2j+1}
     // anchors: ya[b] += (x_m + x_{N-m}) e^{+i pi m/N} for m = m0 + b < L  (the thread's s = tid % T2 is the same for all its e)
+    // The thread's elements share s = tid % T2 and have j1 = q + (L1/8) i, q = tid / T2: e^{-i pi m/N} for m = m0 + b is
+    // e^{-i pi q/L1} e^{-i pi (2 j2 + b)/N} (once per thread) times e^{-i pi i/8} (compile-time constants; i + 4: times -i).
     double2 ya0 = make_double2(0.0, 0.0), ya1 = make_double2(0.0, 0.0);
+    static_assert(NT / T2 == L1 / 8 && C::CH == 4, "j1 = q + (L1/8) i");
+    const int fs = tid % T2, fq = tid / T2;
+    double2 ab0, ab1;
+    {
+        const double2 aq = tw_get(lo, hi, fq);                    // exp(-i pi q / L1)
+        ab0 = cmul(aq, tB[2 * fs]); ab1 = cmul(aq, tB[2 * fs + 1]);
+    }
+    constexpr double W16C[4] = {1.0, 0.92387953251128675613, 0.70710678118654752440, 0.38268343236508977173};
+    constexpr double W16S[4] = {0.0, -0.38268343236508977173, -0.70710678118654752440, -0.92387953251128675613};
 #pragma unroll 1
     for (int i0 = 0; i0 < 8; i0 += C::CH) {
-        if (i0 > 0) load_half(i0);
+        if (i0 > 0) {
+            load_half(i0);
+            ab0 = make_double2(ab0.y, -ab0.x); ab1 = make_double2(ab1.y, -ab1.x);      // times e^{-i pi/2}
+        }
 #pragma unroll
         for (int i = 0; i < C::CH; ++i) {
-            int e = tid + (i0 + i) * NT;
-            int s = e % T2, j1 = e / T2;
-            double2 a = tw_get(lo, hi, j1);                       // exp(-i pi j1 / L1)
-            double2 b0 = tB[2 * s], b1 = tB[2 * s + 1];
-            double s0 = -(a.x * b0.y + a.y * b0.x);               // sin(pi m0 / N)
-            double s1 = -(a.x * b1.y + a.y * b1.x);
+            const int j1 = fq + (i0 + i) * (L1 / 8);
+            const double2 wi = make_double2(W16C[i], W16S[i]);
+            const double2 e0 = i == 0 ? ab0 : cmul(ab0, wi), e1 = i == 0 ? ab1 : cmul(ab1, wi);     // (cos, -sin)(pi m / N)
+            const double s0 = -e0.y, s1 = -e1.y;
             const double sum0 = x0[i] + y0[i], sum1 = x1[i] + y1[i];
-            re[s * RS + PADI(j1)] = s0 * sum0 + 0.5 * (x0[i] - y0[i]);
-            im[s * RS + PADI(j1)] = s1 * sum1 + 0.5 * (x1[i] - y1[i]);
+            re[fs * RS + PADI(j1)] = s0 * sum0 + 0.5 * (x0[i] - y0[i]);
+            im[fs * RS + PADI(j1)] = s1 * sum1 + 0.5 * (x1[i] - y1[i]);
             if (j1 < L1 / 2) {                                    // m0, m0 + 1 < L
-                double c0 = a.x * b0.x - a.y * b0.y, c1 = a.x * b1.x - a.y * b1.y;     // cos(pi m / N)
-                ya0.x = fma(sum0, c0, ya0.x); ya0.y = fma(sum0, s0, ya0.y);
-                ya1.x = fma(sum1, c1, ya1.x); ya1.y = fma(sum1, s1, ya1.y);
+                ya0.x = fma(sum0, e0.x, ya0.x); ya0.y = fma(sum0, s0, ya0.y);
+                ya1.x = fma(sum1, e1.x, ya1.x); ya1.y = fma(sum1, s1, ya1.y);
             }
         }
     }
@@ -153,13 +164,17 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
     }
     __syncthreads();                                  // the sub-FFTs synchronise per group; the store below reads across groups
     SUBT(2);
+    {
+        // k1 = q + (L1/8) i: for L1 = 256 the low table entry (k1 & 31 = q) and the column j2 are the thread's own
+        const double2 wlo = t4lo[fs * C::SLO + (fq & 31)];
+        const int j2s = j2_of(fs);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int e = tid + i * NT;
-        int s = e % T2, k1 = e / T2;
-        double2 v = make_double2(re[s * RS + PADI(k1)], im[s * RS + PADI(k1)]);
-        double2 w = cmul(t4hi[s * C::SHI + (k1 >> 5)], t4lo[s * C::SLO + (k1 & 31)]);
-        __stcg(&Wc[(int64_t)k1 * L2 + j2_of(s)], cmul(v, w));
+        for (int i = 0; i < 8; ++i) {
+            const int k1 = fq + i * (L1 / 8);
+            const double2 v = make_double2(re[fs * RS + PADI(k1)], im[fs * RS + PADI(k1)]);
+            const double2 w = cmul(t4hi[fs * C::SHI + (k1 >> 5)], (L1 / 8) % 32 == 0 ? wlo : t4lo[fs * C::SLO + (k1 & 31)]);
+            __stcg(&Wc[(int64_t)k1 * L2 + j2s], cmul(v, w));
+        }
     }
     __syncthreads();
     SUBT(3);
