@@ -110,7 +110,7 @@ def solve_roofline(n, rF, trace, r_final, hbm_gbs, p64_tflops, ms_measured):
 # `ncu --set full` captures (summaries with their commands under profiles/r02_*_ncu.md); None -> "traffic": null
 _SRC = "profiles/r02_solve_ncu.md (ncu --set full, one C4 solve)"
 NCU_TRAFFIC = {"panel_qr": {"dram_over_alg": 0.77, "source": _SRC}, "panel_apply": {"dram_over_alg": 0.81, "source": _SRC},
-               "dst1_fused": {"dram_over_alg": 1.65, "source": _SRC}, "tall_gemm_t": {"dram_over_alg": 0.89, "source": _SRC},
+               "dst1_fused": {"dram_over_alg": 1.74, "source": _SRC + ", final-state addendum"}, "tall_gemm_t": {"dram_over_alg": 0.89, "source": _SRC},
                "tall_gemm_subtract": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"},
                "tall_gemm_plain": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"},
                "tall_gemm_sample": {"dram_over_alg": 0.97, "source": _SRC + ", all tall_gemm modes together"}}
@@ -402,8 +402,11 @@ def main():
     pool = [(torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory(), torch.empty(w.max_rank, dtype=torch.float64).pin_memory(),
              torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory()) for _ in range(2)]
 
+    torch.cuda.empty_cache()
+    lanes = 2 if ctx.lib.lrp_solve_host_workspace_bytes(n, rF, w.max_rank, w.oversample, 2) < 64e9 else 1      # C5: one lane (2 x 66 GB otherwise)
+
     def e2e_batch(k):
-        return ctx.cross_deim_solve_host([hprob] * k, [pool[p & 1] for p in range(k)], **kw)
+        return ctx.cross_deim_solve_host([hprob] * k, [pool[p & 1] for p in range(k)], lanes=lanes, **kw)
     e2e_batch(2)                                       # warm-up: workspace, copy streams
     R.barrier(dist); torch.cuda.synchronize(dev)
     t0 = time.perf_counter()
@@ -416,6 +419,7 @@ def main():
     e2e_single_ms = 1e3 * (time.perf_counter() - t0)
     agg_e2e = R.throughput(dist, e2e_ms, float(n) ** 2 * steps, dev)
     del pool, hprob
+    ctx.release_workspace(); torch.cuda.empty_cache()  # the staging slots are not needed any more (the next call sizes a new workspace)
 
     if args.timeline and rank == 0:                 # start/end of every launch of one solve, streams NOT serialised
         ctx.profile_reset(); ctx.profile_enable(2)
@@ -520,7 +524,8 @@ def main():
                 "clocks": clk,
                 "e2e": {"value": agg_e2e["per_s"], "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": d2h,
                         "ms_per_step": agg_e2e["ms"] / steps, "single_call_ms": e2e_single_ms,
-                        "call": "lrp_cross_deim_solve_host: one call for all steps, copies of steps i-1 / i+1 overlap solve i"},
+                        "lanes": lanes,
+                        "call": "lrp_cross_deim_solve_host: one call for all steps; per lane the copies of its previous / next step overlap its solve"},
                 "gpu_launches": int(launches),
                 "roofline": roof, "solve_roofline": solve_roof, "phases": phases, "fp64_peak_measured": pk,
                 "kernels": kernels, "dst1": dst, "seeds": seeds, "cpu_baseline": cpu}

@@ -246,6 +246,11 @@ class Context:
             self._ws = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
             self._check(self.lib.lrp_set_workspace(self.h, _ptr(self._ws), self._ws.numel()), "lrp_set_workspace")
 
+    def release_workspace(self):
+        """Drop the workspace tensor (the next call sizes a new one)."""
+        self._check(self.lib.lrp_set_workspace(self.h, C.c_void_p(0), 0), "lrp_set_workspace")
+        self._ws = None
+
     # ------------------------------------------------------------------ the five calls of the boundary
     def dst1_batched(self, x, out=None, scale: float = 1.0):
         """out(:, b) = scale * DST-I(x(:, b)); x, out tall tensors of shape (batch, n).  out may be x."""
