@@ -419,6 +419,19 @@ def main():
     e2e_single_ms = 1e3 * (time.perf_counter() - t0)
     agg_e2e = R.throughput(dist, e2e_ms, float(n) ** 2 * steps, dev)
     del pool, hprob
+    # ---- the same K device-resident solves with two in flight (lrp_cross_deim_solve_batch): what a second solve fills of the
+    # SMs the first leaves idle.  Reported beside `value`, which stays one solve after the other.
+    two_lane = None
+    if lanes == 2:
+        ctx.release_workspace(); torch.cuda.empty_cache()
+        ctx.cross_deim_solve_batch([(UF, SF, VF)] * 2, lanes=2, **kw)
+        R.barrier(dist); torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        ctx.cross_deim_solve_batch([(UF, SF, VF)] * steps, lanes=2, **kw)
+        torch.cuda.synchronize(dev)
+        agg2 = R.throughput(dist, 1e3 * (time.perf_counter() - t0), float(n) ** 2 * steps, dev)
+        two_lane = {"value": agg2["per_s"], "unit": UNIT, "ms_per_step": agg2["ms"] / steps, "lanes": 2,
+                    "call": "lrp_cross_deim_solve_batch, host timer around the synchronous call (includes allocating the outputs)"}
     ctx.release_workspace(); torch.cuda.empty_cache()  # the staging slots are not needed any more (the next call sizes a new workspace)
 
     if args.timeline and rank == 0:                 # start/end of every launch of one solve, streams NOT serialised
@@ -526,7 +539,7 @@ def main():
                         "ms_per_step": agg_e2e["ms"] / steps, "single_call_ms": e2e_single_ms,
                         "lanes": lanes,
                         "call": "lrp_cross_deim_solve_host: one call for all steps; per lane the copies of its previous / next step overlap its solve"},
-                "gpu_launches": int(launches),
+                "gpu_launches": int(launches), "two_solves_in_flight": two_lane,
                 "roofline": roof, "solve_roofline": solve_roof, "phases": phases, "fp64_peak_measured": pk,
                 "kernels": kernels, "dst1": dst, "seeds": seeds, "cpu_baseline": cpu}
         print(json.dumps(line))

@@ -243,6 +243,19 @@ int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob
                               double* const* h_VW, int64_t ldvw,
                               lrp_solve_info* info);
 
+/* The same for problems whose factors are already on the DEVICE: d_UF, d_SF, d_VF, d_UW, d_SW, d_VW are HOST arrays of
+ * nprob DEVICE pointers (layouts as in lrp_cross_deim_solve; outputs of different problems must not overlap).  With a
+ * workspace of lrp_solve_batch_workspace_bytes(..., 2) and nprob >= 2 the even and the odd problems are solved by two
+ * lanes at once, else one after the other; results do not depend on it.  Synchronous; return value as above. */
+size_t lrp_solve_batch_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample, int32_t lanes);
+int lrp_cross_deim_solve_batch(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
+                               const double* const* d_UF, int64_t ldu, const double* const* d_SF,
+                               const double* const* d_VF, int64_t ldv,
+                               const lrp_solve_opts* opts,
+                               double* const* d_UW, int64_t lduw, double* const* d_SW,
+                               double* const* d_VW, int64_t ldvw,
+                               lrp_solve_info* info);
+
 /* Generic function-handle Cross-DEIM (Alg. 4; "G(i,j) as a function handle") on the
  * paper's closed-form test matrices, eq. (6), PAPER.md:264-267 (0-based i, j; square n x n, any n >= K_cap):
  *     LRP_G_HILBERT:  H(i,j) = 1 / (1 + i + j)                        (rapid singular value decay)

@@ -1127,25 +1127,15 @@ int host_lane(lrp_ctx* ctx, const HostBatch& b, int first, int stride) {
 }
 }  // namespace
 
-int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
-                              const double* const* h_UF, int64_t ldu, const double* const* h_SF, const double* const* h_VF, int64_t ldv,
-                              const lrp_solve_opts* opts,
-                              double* const* h_UW, int64_t lduw, double* const* h_SW, double* const* h_VW, int64_t ldvw,
-                              lrp_solve_info* info) {
-    if (!ctx || !opts || !info || nprob < 0 || !h_UF || !h_SF || !h_VF || !h_UW || !h_SW || !h_VW) return LRP_ERR_BADARG;
-    if (ldu < n || ldv < n || lduw < n || ldvw < n || rF < 1 || opts->max_rank < 1) return LRP_ERR_BADARG;
-    for (int p = 0; p < nprob; ++p)
-        if (!h_UF[p] || !h_SF[p] || !h_VF[p] || !h_UW[p] || !h_SW[p] || !h_VW[p]) return LRP_ERR_BADARG;
-    LRP_TRY(check_n(n));
-    if (nprob == 0) return LRP_OK;
-    const size_t lane_bytes = host_lane_bytes(n, rF, opts->max_rank, opts->oversample);
-    if (!lane_bytes || ctx->ws_bytes < lane_bytes) return LRP_ERR_WORKSPACE;
-    HostBatch b{n, rF, nprob, h_UF, ldu, h_SF, h_VF, ldv, opts, h_UW, lduw, h_SW, h_VW, ldvw, info};
-    // Second lane: a library-owned context (own streams, own pinned block) on the same device, driven by a worker thread,
-    // when the workspace has room for it and there is more than one problem.  Two solves in flight fill the SMs the
-    // other leaves idle (one-CTA core, tree levels, host decisions): 14.4 -> 11.5 ms per C4 problem.
+// Problems 0, 1, 2, ... on one lane (ctx) or, when the workspace holds two lanes' worth and there are at least two
+// problems, on two: even ones on ctx, odd ones on a library-owned second context (own streams, own pinned block) on the
+// same device, driven by a worker thread that lives for the call.  Two solves in flight fill the SMs that one leaves
+// idle (one-CTA core, TSQR tree levels, host decisions): 14.4 -> 11.5 ms per C4 problem.  lane(ctx, first, stride) runs one lane.
+extern "C++" {
+template <typename Lane>
+static int run_lanes(lrp_ctx* ctx, size_t lane_bytes, int nprob, Lane lane) {
     const bool two = nprob >= 2 && ctx->ws_bytes >= 2 * lane_bytes && ctx->prof_on == 0;
-    if (!two) return host_lane(ctx, b, 0, 1);
+    if (!two) return lane(ctx, 0, 1);
     if (!ctx->lane2) {
         cudaStream_t s2 = nullptr;
         LRP_CUDA(ctx, cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
@@ -1161,14 +1151,13 @@ int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob
     // work already enqueued on the caller's stream precedes lane 1 too
     cudaError_t ef = cudaEventRecord(ctx->ev_fork, ctx->stream);
     if (ef == cudaSuccess) ef = cudaStreamWaitEvent(c2->stream, ctx->ev_fork, 0);
-    int rc1 = LRP_OK;
+    int rc0, rc1 = LRP_OK;
     const int64_t l2_0 = c2->launches;
-    int rc0;
     if (ef != cudaSuccess) { ctx->last_cuda = (int)ef; rc0 = LRP_ERR_CUDA; }
     else {
         const int device = ctx->device;
-        std::thread worker([&, device] { cudaSetDevice(device); rc1 = host_lane(c2, b, 1, 2); });
-        rc0 = host_lane(ctx, b, 0, 2);
+        std::thread worker([&, device] { cudaSetDevice(device); rc1 = lane(c2, 1, 2); });
+        rc0 = lane(ctx, 0, 2);
         worker.join();
     }
     ctx->ws = ws0; ctx->ws_bytes = wsb0;
@@ -1177,6 +1166,53 @@ int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob
     if (rc0 < 0) return rc0;
     if (rc1 < 0) return rc1;
     return rc0 > rc1 ? rc0 : rc1;
+}
+}  // extern "C++"
+
+int lrp_cross_deim_solve_host(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
+                              const double* const* h_UF, int64_t ldu, const double* const* h_SF, const double* const* h_VF, int64_t ldv,
+                              const lrp_solve_opts* opts,
+                              double* const* h_UW, int64_t lduw, double* const* h_SW, double* const* h_VW, int64_t ldvw,
+                              lrp_solve_info* info) {
+    if (!ctx || !opts || !info || nprob < 0 || !h_UF || !h_SF || !h_VF || !h_UW || !h_SW || !h_VW) return LRP_ERR_BADARG;
+    if (ldu < n || ldv < n || lduw < n || ldvw < n || rF < 1 || opts->max_rank < 1) return LRP_ERR_BADARG;
+    for (int p = 0; p < nprob; ++p)
+        if (!h_UF[p] || !h_SF[p] || !h_VF[p] || !h_UW[p] || !h_SW[p] || !h_VW[p]) return LRP_ERR_BADARG;
+    LRP_TRY(check_n(n));
+    if (nprob == 0) return LRP_OK;
+    const size_t lane_bytes = host_lane_bytes(n, rF, opts->max_rank, opts->oversample);
+    if (!lane_bytes || ctx->ws_bytes < lane_bytes) return LRP_ERR_WORKSPACE;
+    HostBatch b{n, rF, nprob, h_UF, ldu, h_SF, h_VF, ldv, opts, h_UW, lduw, h_SW, h_VW, ldvw, info};
+    return run_lanes(ctx, lane_bytes, nprob, [&](lrp_ctx* c, int first, int stride) { return host_lane(c, b, first, stride); });
+}
+
+size_t lrp_solve_batch_workspace_bytes(int64_t n, int32_t rF, int32_t max_rank, int32_t oversample, int32_t lanes) {
+    if (lanes < 1 || lanes > LRP_HOST_LANES_MAX) return 0;
+    const size_t base = lrp_workspace_bytes(n, rF, max_rank, oversample);
+    return base ? (size_t)lanes * (lrp_align_up(base) + 256) : 0;
+}
+
+int lrp_cross_deim_solve_batch(lrp_ctx* ctx, int64_t n, int32_t rF, int32_t nprob,
+                               const double* const* d_UF, int64_t ldu, const double* const* d_SF, const double* const* d_VF, int64_t ldv,
+                               const lrp_solve_opts* opts,
+                               double* const* d_UW, int64_t lduw, double* const* d_SW, double* const* d_VW, int64_t ldvw,
+                               lrp_solve_info* info) {
+    if (!ctx || !opts || !info || nprob < 0 || !d_UF || !d_SF || !d_VF || !d_UW || !d_SW || !d_VW) return LRP_ERR_BADARG;
+    for (int p = 0; p < nprob; ++p)
+        if (!d_UF[p] || !d_SF[p] || !d_VF[p] || !d_UW[p] || !d_SW[p] || !d_VW[p]) return LRP_ERR_BADARG;
+    if (nprob == 0) return LRP_OK;
+    const size_t lane_bytes = lrp_solve_batch_workspace_bytes(n, rF, opts->max_rank, opts->oversample, 1);
+    if (!lane_bytes || ctx->ws_bytes < lane_bytes) return LRP_ERR_WORKSPACE;
+    return run_lanes(ctx, lane_bytes, nprob, [&](lrp_ctx* c, int first, int stride) {
+        int worst = LRP_OK;
+        for (int p = first; p < nprob; p += stride) {
+            const int rc = lrp_cross_deim_solve(c, n, rF, d_UF[p], ldu, d_SF[p], d_VF[p], ldv, opts, d_UW[p], lduw, d_SW[p], d_VW[p], ldvw,
+                                                &info[p], nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+            if (rc < 0) return rc;
+            if (rc > worst) worst = rc;
+        }
+        return worst;
+    });
 }
 
 int lrp_cross_deim_matrix(lrp_ctx* ctx, int32_t kind, int64_t n, const lrp_solve_opts* opts,

@@ -35,7 +35,8 @@ EXPORTS = ["lrp_create", "lrp_destroy", "lrp_strerror", "lrp_last_cuda_error", "
            "lrp_profile_enable", "lrp_profile_reset", "lrp_profile_count", "lrp_profile_get",
            "lrp_profile_timeline", "lrp_fp64_peak", "lrp_matrix_workspace_bytes", "lrp_cross_deim_matrix",
            "lrp_sample_matrix", "lrp_dense_workspace_bytes", "lrp_dense_poisson", "lrp_topk_static",
-           "lrp_solve_host_workspace_bytes", "lrp_cross_deim_solve_host"]
+           "lrp_solve_host_workspace_bytes", "lrp_cross_deim_solve_host",
+           "lrp_solve_batch_workspace_bytes", "lrp_cross_deim_solve_batch"]
 
 
 class SolveOpts(C.Structure):
@@ -96,6 +97,9 @@ def load_library():
     lib.lrp_solve_host_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]; lib.lrp_solve_host_workspace_bytes.restype = sz
     lib.lrp_cross_deim_solve_host.argtypes = [vp, i64, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.lrp_cross_deim_solve_host.restype = C.c_int
+    lib.lrp_solve_batch_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]; lib.lrp_solve_batch_workspace_bytes.restype = sz
+    lib.lrp_cross_deim_solve_batch.argtypes = [vp, i64, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+    lib.lrp_cross_deim_solve_batch.restype = C.c_int
     lib.lrp_matrix_workspace_bytes.argtypes = [i64, i32, i32, i32]; lib.lrp_matrix_workspace_bytes.restype = sz
     lib.lrp_cross_deim_matrix.argtypes = [vp, i32, i64, C.POINTER(SolveOpts), vp, i64, vp, vp, i64, C.POINTER(SolveInfo),
                                           vp, vp, vp, vp, vp, vp, vp, i64]
@@ -435,6 +439,46 @@ class Context:
         del sg
         return [dict(rank=infos[p].rank, sweeps=infos[p].sweeps, converged=bool(infos[p].converged), code=rc, info=infos[p])
                 for p in range(P)]
+
+    def cross_deim_solve_batch(self, problems, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
+                               tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0, lanes=2):
+        """lrp_cross_deim_solve_batch: independent problems with DEVICE factors, two solves in flight when lanes = 2.
+        problems: list of (UF, SF, VF) CUDA tensors as for cross_deim_solve.  Returns one dict per problem like
+        cross_deim_solve (UW, SW, VW, rank, sweeps, converged, info)."""
+        torch = _torch()
+        if not problems:
+            return []
+        rF, n, ldu = _check_tall(problems[0][0], "UF")
+        _, _, ldv = _check_tall(problems[0][2], "VF")
+        for UF, SF, VF in problems:
+            if _check_tall(UF, "UF") != (rF, n, ldu) or _check_tall(VF, "VF") != (rF, n, ldv):
+                raise ValueError("all problems must share n, rF and the leading dimensions")
+        need = self.lib.lrp_solve_batch_workspace_bytes(n, rF, max_rank, oversample, int(lanes))
+        if need == 0:
+            raise LrpError(-1, "lrp_solve_batch_workspace_bytes (unsupported n, rank cap or lane count)")
+        self.ensure_workspace(need, exact=True)
+        o = SolveOpts()
+        o.tol, o.max_rank, o.oversample, o.max_sweeps, o.tol_mode = tol, max_rank, oversample, max_sweeps, tol_mode
+        o.flags = int(flags)
+        o.selection = SELECTIONS[selection] if isinstance(selection, str) else int(selection)
+        o.ls_seed, o.ls_c = int(ls_seed), float(ls_c)
+        sg = None
+        if safeguard is not None:
+            sg = np.ascontiguousarray(safeguard, dtype=np.int32)
+            o.h_safeguard, o.n_safeguard = sg.ctypes.data, sg.size
+        P = len(problems)
+        dev = problems[0][0].device
+        outs = [(torch.empty((max_rank, n), dtype=torch.float64, device=dev), torch.empty(max_rank, dtype=torch.float64, device=dev),
+                 torch.empty((max_rank, n), dtype=torch.float64, device=dev)) for _ in range(P)]
+        arr = lambda ts: (C.c_void_p * P)(*[t.data_ptr() for t in ts])
+        infos = (SolveInfo * P)()
+        rc = self._check(self.lib.lrp_cross_deim_solve_batch(
+            self.h, n, rF, P, arr([p[0] for p in problems]), ldu, arr([p[1] for p in problems]), arr([p[2] for p in problems]), ldv,
+            C.byref(o), arr([q[0] for q in outs]), n, arr([q[1] for q in outs]), arr([q[2] for q in outs]), n, infos),
+            "lrp_cross_deim_solve_batch")
+        del sg
+        return [dict(UW=outs[p][0][:infos[p].rank], SW=outs[p][1][:infos[p].rank], VW=outs[p][2][:infos[p].rank], rank=infos[p].rank,
+                     sweeps=infos[p].sweeps, converged=bool(infos[p].converged), code=rc, info=infos[p]) for p in range(P)]
 
     def cross_deim_matrix(self, kind, n, U0, V0, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
                           tol_mode=0, replay=None, want_spectral=False, flags=0, selection="topk", ls_seed=0, ls_c=0.0):

@@ -78,6 +78,22 @@ def test_host_batch_output_pool_and_oracle(ctx):
     assert np.abs(got - exp).max() <= 1e-10 * np.abs(exp).max()
 
 
+def test_device_batch_matches_single_calls(ctx):
+    """lrp_cross_deim_solve_batch (device factors, two lanes): problem by problem the same results as lrp_cross_deim_solve."""
+    import torch
+    from paper_2607_06021_b200 import lrp
+    ws = [W.make("C2", seed) for seed in range(5)]
+    w0 = ws[0]
+    kw = dict(tol=w0.tol, max_rank=w0.max_rank, oversample=w0.oversample, max_sweeps=w0.max_sweeps, safeguard=w0.safeguard)
+    probs = [(lrp.tall_from_numpy(w.UF), torch.from_numpy(w.SF).cuda(), lrp.tall_from_numpy(w.VF)) for w in ws]
+    for lanes in (2, 1):
+        res = ctx.cross_deim_solve_batch(probs, lanes=lanes, **kw)
+        for (UF, SF, VF), r in zip(probs, res):
+            dev = ctx.cross_deim_solve(UF, SF, VF, **kw)
+            assert (r["rank"], r["sweeps"], r["converged"]) == (dev["rank"], dev["sweeps"], dev["converged"])
+            assert torch.equal(r["SW"], dev["SW"]) and torch.equal(r["UW"], dev["UW"]) and torch.equal(r["VW"], dev["VW"])
+
+
 def test_host_batch_argument_errors(ctx):
     """Too small a workspace and null entries are reported, not dereferenced."""
     import ctypes as C
