@@ -105,10 +105,10 @@ __device__ __forceinline__ void phase_a(unsigned char* smem_raw, int log2N, int 
             int e = tid + (i0 + i) * NT;
             int s = e % T2, j1 = e / T2;
             int64_t m0 = 2 * ((int64_t)j1 * L2 + j2_of(s));
-            x0[i] = (m0 >= 1) ? __ldcs(x + m0 - 1) : 0.0;
-            x1[i] = __ldcs(x + m0);
-            y0[i] = (m0 >= 1) ? __ldcs(x + N - m0 - 1) : 0.0;
-            y1[i] = __ldcs(x + N - m0 - 2);
+            x0[i] = (m0 >= 1) ? __ldca(x + m0 - 1) : 0.0;
+            x1[i] = __ldca(x + m0);
+            y0[i] = (m0 >= 1) ? __ldca(x + N - m0 - 1) : 0.0;
+            y1[i] = __ldca(x + N - m0 - 2);
         }
     };
     SUBT0();
