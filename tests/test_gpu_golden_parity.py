@@ -1,5 +1,5 @@
 """GPU <-> oracle parity at the sizes the oracle cannot reach inside a test: BASELINE.json's C3 and C4 at full size
-and C5-shaped cases at n = 65535 / 2^18-1.  The oracle's FREE RUN was computed once by
+and C5-shaped cases at n = 65535 / 2^18-1 / 2^20-1.  The oracle's FREE RUN was computed once by
 tests/golden/make_solve_golden.py (oracle + input generators only) and reduced to the trace of discrete decisions, the
 singular values, 4096 physical-space entries and the selected fibers at 1024 positions (+ whole-fiber norms).
 
@@ -21,9 +21,10 @@ GOLDEN_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 TOL = 1e-10
 
 # (config, seed, n) -- n = None: the config's own size.  C5 at its own size (n = 2^22 - 1) has no stored oracle run: scaled
-# from the n = 2^18 - 1 case (1269 s, 3.5 GB on 8 cores) it needs ~5.6 h and ~56 GB of the build box's 62 GB; C5 is covered
-# by its two smaller shapes here and by the size-independent properties of tests/test_gpu_full_size.py.
-CASES = [("C3", 0, None), ("C5", 0, 65535), ("C5", 0, (1 << 18) - 1), ("C4", 0, None)]
+# from the n = 2^20 - 1 case (5162 s, 13.8 GB on 8 cores) it needs ~5.7 h and ~55 GB of the build box's 62 GB; C5 is covered
+# by its three smaller shapes here (the largest a quarter of its size: four-step DST-I, five-level TSQR tree, several
+# waves of row slabs, K up to 95 of K_cap = 272) and by the size-independent properties of tests/test_gpu_full_size.py.
+CASES = [("C3", 0, None), ("C5", 0, 65535), ("C5", 0, (1 << 18) - 1), ("C5", 0, (1 << 20) - 1), ("C4", 0, None)]
 
 
 @pytest.fixture(scope="module")
