@@ -1156,9 +1156,12 @@ static int run_lanes(lrp_ctx* ctx, size_t lane_bytes, int nprob, Lane lane) {
     if (ef != cudaSuccess) { ctx->last_cuda = (int)ef; rc0 = LRP_ERR_CUDA; }
     else {
         const int device = ctx->device;
-        std::thread worker([&, device] { cudaSetDevice(device); rc1 = lane(c2, 1, 2); });
-        rc0 = lane(ctx, 0, 2);
-        worker.join();
+        bool started = true;
+        std::thread worker;
+        try { worker = std::thread([&, device] { cudaSetDevice(device); rc1 = lane(c2, 1, 2); }); }
+        catch (...) { started = false; }                 // no thread to be had: one lane after all
+        if (started) { rc0 = lane(ctx, 0, 2); worker.join(); }
+        else { ctx->ws_bytes = wsb0; rc0 = lane(ctx, 0, 1); }
     }
     ctx->ws = ws0; ctx->ws_bytes = wsb0;
     ctx->launches += c2->launches - l2_0;

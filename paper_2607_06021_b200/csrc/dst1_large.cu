@@ -19,7 +19,7 @@
 // Dependencies (A -> D, A -> B, B + D -> C, C of the group two back -> A: ring slot free) are per-column arrival counters;
 // items are queued in an order in which every dependency points backwards, and a CTA that holds an item is running, so
 // the waits cannot deadlock whatever the number of resident CTAs.
-// Measured alternatives (profiles/r02_l2_dsmem_microbench.md): distributed shared memory in a 16-CTA cluster exchanges
+// Measured alternatives (scratch microbenchmarks, figures in DESIGN.md section 4): distributed shared memory in a 16-CTA cluster exchanges
 // 3.2 TB/s over the 112 SMs such clusters can occupy, L2-resident traffic 12 TB/s over all 148 -- hence L2, not DSMEM,
 // also for the sizes (N <= 2^18) whose column would fit a cluster.
 #include "common.cuh"
