@@ -397,41 +397,51 @@ def main():
     # pinned host memory and every step's result is read back to pinned host memory inside the timed region; the call
     # overlaps the copies of the neighbouring steps with the solve (two staging slots).  `single_call_ms` is one isolated
     # call (copy in, solve, copy out, nothing to overlap with).
-    hprob = tuple(t.pin_memory() for t in (torch.from_numpy(np.ascontiguousarray(w.UF.T)), torch.from_numpy(np.ascontiguousarray(w.SF)),
-                                           torch.from_numpy(np.ascontiguousarray(w.VF.T))))
-    pool = [(torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory(), torch.empty(w.max_rank, dtype=torch.float64).pin_memory(),
-             torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory()) for _ in range(2)]
+    e2e_error = None
+    lanes, d2h, e2e_single_ms, two_lane = 1, 0, None, None
+    agg_e2e = {"per_s": None, "ms": None}
+    try:
+        hprob = tuple(t.pin_memory() for t in (torch.from_numpy(np.ascontiguousarray(w.UF.T)), torch.from_numpy(np.ascontiguousarray(w.SF)),
+                                               torch.from_numpy(np.ascontiguousarray(w.VF.T))))
+        pool = [(torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory(), torch.empty(w.max_rank, dtype=torch.float64).pin_memory(),
+                 torch.empty((w.max_rank, n), dtype=torch.float64).pin_memory()) for _ in range(2)]
 
-    torch.cuda.empty_cache()
-    lanes = 2 if ctx.lib.lrp_solve_host_workspace_bytes(n, rF, w.max_rank, w.oversample, 2) < 64e9 else 1      # C5: one lane (2 x 66 GB otherwise)
+        torch.cuda.empty_cache()
+        lanes = 2 if ctx.lib.lrp_solve_host_workspace_bytes(n, rF, w.max_rank, w.oversample, 2) < 64e9 else 1      # C5: one lane (2 x 66 GB otherwise)
 
-    def e2e_batch(k):
-        return ctx.cross_deim_solve_host([hprob] * k, [pool[p & 1] for p in range(k)], lanes=lanes, **kw)
-    e2e_batch(2)                                       # warm-up: workspace, copy streams
-    R.barrier(dist); torch.cuda.synchronize(dev)
-    t0 = time.perf_counter()
-    hres = e2e_batch(steps)
-    e2e_ms = 1e3 * (time.perf_counter() - t0)
-    R.barrier(dist)
-    d2h = (2 * n * hres[-1]["rank"] + hres[-1]["rank"]) * 8
-    t0 = time.perf_counter()
-    e2e_batch(1)
-    e2e_single_ms = 1e3 * (time.perf_counter() - t0)
-    agg_e2e = R.throughput(dist, e2e_ms, float(n) ** 2 * steps, dev)
-    del pool, hprob
-    # ---- the same K device-resident solves with two in flight (lrp_cross_deim_solve_batch): what a second solve fills of the
-    # SMs the first leaves idle.  Reported beside `value`, which stays one solve after the other.
-    two_lane = None
-    if lanes == 2:
-        ctx.release_workspace(); torch.cuda.empty_cache()
-        ctx.cross_deim_solve_batch([(UF, SF, VF)] * 2, lanes=2, **kw)
+        def e2e_batch(k):
+            return ctx.cross_deim_solve_host([hprob] * k, [pool[p & 1] for p in range(k)], lanes=lanes, **kw)
+        e2e_batch(2)                                       # warm-up: workspace, copy streams
         R.barrier(dist); torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
-        ctx.cross_deim_solve_batch([(UF, SF, VF)] * steps, lanes=2, **kw)
-        torch.cuda.synchronize(dev)
-        agg2 = R.throughput(dist, 1e3 * (time.perf_counter() - t0), float(n) ** 2 * steps, dev)
-        two_lane = {"value": agg2["per_s"], "unit": UNIT, "ms_per_step": agg2["ms"] / steps, "lanes": 2,
-                    "call": "lrp_cross_deim_solve_batch, host timer around the synchronous call (includes allocating the outputs)"}
+        hres = e2e_batch(steps)
+        e2e_ms = 1e3 * (time.perf_counter() - t0)
+        R.barrier(dist)
+        d2h = (2 * n * hres[-1]["rank"] + hres[-1]["rank"]) * 8
+        t0 = time.perf_counter()
+        e2e_batch(1)
+        e2e_single_ms = 1e3 * (time.perf_counter() - t0)
+        agg_e2e = R.throughput(dist, e2e_ms, float(n) ** 2 * steps, dev)
+        del pool, hprob
+        # ---- the same K device-resident solves with two in flight (lrp_cross_deim_solve_batch): what a second solve fills of the
+        # SMs the first leaves idle.  Reported beside `value`, which stays one solve after the other.
+        if lanes == 2:
+            ctx.release_workspace(); torch.cuda.empty_cache()
+            bouts = [(torch.empty((w.max_rank, n), dtype=torch.float64, device=dev), torch.empty(w.max_rank, dtype=torch.float64, device=dev),
+                      torch.empty((w.max_rank, n), dtype=torch.float64, device=dev)) for _ in range(steps)]
+            ctx.cross_deim_solve_batch([(UF, SF, VF)] * 2, lanes=2, outputs=bouts[:2], **kw)
+            R.barrier(dist); torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            ctx.cross_deim_solve_batch([(UF, SF, VF)] * steps, lanes=2, outputs=bouts, **kw)
+            torch.cuda.synchronize(dev)
+            agg2 = R.throughput(dist, 1e3 * (time.perf_counter() - t0), float(n) ** 2 * steps, dev)
+            two_lane = {"value": agg2["per_s"], "unit": UNIT, "ms_per_step": agg2["ms"] / steps, "lanes": 2,
+                        "call": "lrp_cross_deim_solve_batch, host timer around the synchronous call (outputs preallocated)"}
+            del bouts
+    except Exception as ex:                            # e.g. no pinned host memory to be had: the device-resident line still prints
+        if dist is not None:
+            raise
+        e2e_error = f"{type(ex).__name__}: {ex}"[:300]
     ctx.release_workspace(); torch.cuda.empty_cache()  # the staging slots are not needed any more (the next call sizes a new workspace)
 
     if args.timeline and rank == 0:                 # start/end of every launch of one solve, streams NOT serialised
@@ -536,7 +546,7 @@ def main():
                           "ms": {k: getattr(info, "ms_" + k) for k in ("dst_fwd", "select", "sample", "qr", "core", "rebuild", "stop", "dst_inv", "total")}},
                 "clocks": clk,
                 "e2e": {"value": agg_e2e["per_s"], "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": d2h,
-                        "ms_per_step": agg_e2e["ms"] / steps, "single_call_ms": e2e_single_ms,
+                        "ms_per_step": (agg_e2e["ms"] / steps) if agg_e2e["ms"] is not None else None, "single_call_ms": e2e_single_ms, "error": e2e_error,
                         "lanes": lanes,
                         "call": "lrp_cross_deim_solve_host: one call for all steps; per lane the copies of its previous / next step overlap its solve"},
                 "gpu_launches": int(launches), "two_solves_in_flight": two_lane,

@@ -441,10 +441,11 @@ class Context:
                 for p in range(P)]
 
     def cross_deim_solve_batch(self, problems, *, tol, max_rank, oversample=8, max_sweeps=20, safeguard=None,
-                               tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0, lanes=2):
+                               tol_mode=0, flags=0, selection="topk", ls_seed=0, ls_c=0.0, lanes=2, outputs=None):
         """lrp_cross_deim_solve_batch: independent problems with DEVICE factors, two solves in flight when lanes = 2.
         problems: list of (UF, SF, VF) CUDA tensors as for cross_deim_solve.  Returns one dict per problem like
-        cross_deim_solve (UW, SW, VW, rank, sweeps, converged, info)."""
+        cross_deim_solve (UW, SW, VW, rank, sweeps, converged, info).  outputs: optional list of preallocated
+        (UW (max_rank, n), SW (max_rank,), VW (max_rank, n)) CUDA tensors, one distinct triple per problem."""
         torch = _torch()
         if not problems:
             return []
@@ -468,8 +469,11 @@ class Context:
             o.h_safeguard, o.n_safeguard = sg.ctypes.data, sg.size
         P = len(problems)
         dev = problems[0][0].device
-        outs = [(torch.empty((max_rank, n), dtype=torch.float64, device=dev), torch.empty(max_rank, dtype=torch.float64, device=dev),
-                 torch.empty((max_rank, n), dtype=torch.float64, device=dev)) for _ in range(P)]
+        outs = outputs if outputs is not None else [
+            (torch.empty((max_rank, n), dtype=torch.float64, device=dev), torch.empty(max_rank, dtype=torch.float64, device=dev),
+             torch.empty((max_rank, n), dtype=torch.float64, device=dev)) for _ in range(P)]
+        if len(outs) != P or any(q[0].shape != (max_rank, n) or q[2].shape != (max_rank, n) or q[1].numel() < max_rank for q in outs):
+            raise ValueError("outputs: one (UW (max_rank, n), SW (max_rank,), VW (max_rank, n)) triple per problem")
         arr = lambda ts: (C.c_void_p * P)(*[t.data_ptr() for t in ts])
         infos = (SolveInfo * P)()
         rc = self._check(self.lib.lrp_cross_deim_solve_batch(
