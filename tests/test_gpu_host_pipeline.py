@@ -94,6 +94,39 @@ def test_device_batch_matches_single_calls(ctx):
             assert torch.equal(r["SW"], dev["SW"]) and torch.equal(r["UW"], dev["UW"]) and torch.equal(r["VW"], dev["VW"])
 
 
+def test_host_batch_padded_leading_dimensions(ctx):
+    """Host factors and results with ld > n (the pitched copies of the call): same results as the device-pointer call."""
+    import ctypes as C
+    import torch
+    from paper_2607_06021_b200 import lrp
+    ws = [W.make("C2", seed) for seed in (7, 8, 9)]
+    w0 = ws[0]
+    n, rF, R = w0.n, w0.UF.shape[1], w0.max_rank
+    ldi, ldo = n + 3, n + 5
+    kw = dict(tol=w0.tol, max_rank=R, oversample=w0.oversample, max_sweeps=w0.max_sweeps, safeguard=w0.safeguard)
+    ins, outs = [], []
+    for w in ws:
+        UF = torch.zeros((rF, ldi), dtype=torch.float64).pin_memory(); VF = torch.zeros((rF, ldi), dtype=torch.float64).pin_memory()
+        UF[:, :n] = torch.from_numpy(np.ascontiguousarray(w.UF.T)); VF[:, :n] = torch.from_numpy(np.ascontiguousarray(w.VF.T))
+        ins.append((UF, torch.from_numpy(np.ascontiguousarray(w.SF)).pin_memory(), VF))
+        outs.append((torch.full((R, ldo), np.nan, dtype=torch.float64).pin_memory(), torch.full((R,), np.nan, dtype=torch.float64).pin_memory(),
+                     torch.full((R, ldo), np.nan, dtype=torch.float64).pin_memory()))
+    ctx.ensure_workspace(ctx.lib.lrp_solve_host_workspace_bytes(n, rF, R, w0.oversample, 2), exact=True)
+    o = lrp.SolveOpts(); o.tol, o.max_rank, o.oversample, o.max_sweeps = w0.tol, R, w0.oversample, w0.max_sweeps
+    sg = np.ascontiguousarray(w0.safeguard, dtype=np.int32); o.h_safeguard, o.n_safeguard = sg.ctypes.data, sg.size
+    arr = lambda ts: (C.c_void_p * len(ts))(*[t.data_ptr() for t in ts])
+    info = (lrp.SolveInfo * len(ws))()
+    rc = ctx.lib.lrp_cross_deim_solve_host(ctx.h, n, rF, len(ws), arr([p[0] for p in ins]), ldi, arr([p[1] for p in ins]), arr([p[2] for p in ins]), ldi,
+                                           C.byref(o), arr([q[0] for q in outs]), ldo, arr([q[1] for q in outs]), arr([q[2] for q in outs]), ldo, info)
+    assert rc >= 0
+    for w, (UW, SW, VW), inf in zip(ws, outs, info):
+        dev = ctx.cross_deim_solve(lrp.tall_from_numpy(w.UF), torch.from_numpy(w.SF).cuda(), lrp.tall_from_numpy(w.VF), **kw)
+        k = inf.rank
+        assert k == dev["rank"] and inf.sweeps == dev["sweeps"]
+        assert torch.equal(UW[:k, :n], dev["UW"].cpu()) and torch.equal(VW[:k, :n], dev["VW"].cpu()) and torch.equal(SW[:k], dev["SW"].cpu())
+        assert torch.isnan(UW[:, n:]).all() and torch.isnan(VW[k:]).all()                 # padding and unused columns untouched
+
+
 def test_host_batch_argument_errors(ctx):
     """Too small a workspace and null entries are reported, not dereferenced."""
     import ctypes as C
