@@ -56,10 +56,12 @@ def test_dst1_four_step_regime(ctx, n):
     assert _rel(lrp.tall_to_numpy(t), x) < 1e-12
 
 
-@pytest.mark.parametrize("p", [20, 22, 24, 25])
+@pytest.mark.parametrize("p", [17, 19, 20, 21, 22, 23, 24, 25])
 def test_dst1_full_size_sampled(ctx, p):
-    """BASELINE sizes n = 2^20-1, 2^22-1 and the largest sizes the call accepts (2^24-1, 2^25-1): sampled outputs against
-    the O(n) definition sum per entry."""
+    """BASELINE sizes n = 2^20-1, 2^22-1, the largest sizes the call accepts (2^24-1, 2^25-1) and the sizes in between
+    whose four-step split is not met elsewhere (every instantiation of the persistent kernel from L = 2^16 = 256 x 256 to
+    2^24 = 4096 x 4096 is run by this test or by test_dst1_four_step_regime): sampled outputs against the O(n) definition
+    sum per entry."""
     import torch
     from paper_2607_06021_b200 import lrp
     n = (1 << p) - 1
