@@ -22,6 +22,10 @@ def _worker(rank, world, port, q):
     units = 100.0 + rank
     agg = R.throughput(dist, local_ms, units)
     R.barrier(dist)
+    # a batch of 5 independent problems split over the ranks; per-problem integers collected in problem order
+    lo, hi = R.shard(5, rank, world)
+    agg["shard"] = (lo, hi)
+    agg["ranks_of_batch"] = R.gather_ints(dist, [100 * rank + p for p in range(lo, hi)], 5)
     q.put((rank, agg))
     dist.destroy_process_group()
 
@@ -41,6 +45,20 @@ def test_two_rank_aggregate_gloo():
         assert res[r]["ms"] == 20.0                       # max over ranks
         assert res[r]["units"] == 201.0                   # whole-job units
         assert abs(res[r]["per_s"] - 201.0 / 0.020) < 1e-9
+        assert res[r]["ranks_of_batch"] == [0, 1, 2, 103, 104]     # rank 0 solved problems 0-2, rank 1 problems 3-4
+    assert res[0]["shard"] == (0, 3) and res[1]["shard"] == (3, 5)
+
+
+def test_shard_covers_every_problem_once():
+    from paper_2607_06021_b200 import replicas as R
+    for nprob in (0, 1, 2, 7, 8, 64, 1000):
+        for world in (1, 2, 3, 8):
+            blocks = [R.shard(nprob, r, world) for r in range(world)]
+            assert blocks[0][0] == 0 and blocks[-1][1] == nprob
+            assert all(blocks[r][1] == blocks[r + 1][0] for r in range(world - 1))
+            sizes = [hi - lo for lo, hi in blocks]
+            assert max(sizes) - min(sizes) <= 1
+    assert R.gather_ints(None, [4, 5], 2) == [4, 5]
 
 
 def test_single_process_defaults():
