@@ -1,7 +1,7 @@
 """Writes tests/golden/solve_<cfg>_n<n>_s<seed>.npz (+ a .txt header beside it): the CPU oracle's FREE RUN of the
 Cross-DEIM low-rank Poisson solve (Alg. 4; section 3.2) on one seeded workload
 at a size where the oracle is too slow to be called from a test (C3/C4/C5 at BASELINE.json's full sizes, C5-shaped
-cases at n = 65535 and 2^18-1), reduced to what the `-m gpu` parity tests need:
+cases at n = 65535, 2^18-1 and 2^20-1), reduced to what the `-m gpu` parity tests need:
 
   * the trace of discrete decisions (I_k, J_k, prune masks, rank, rho, ind, eta, S_min per sweep, the leverage
     selections I*, J* and the sorted top scores that decide them) -- the GPU free run is compared with it and the
@@ -18,6 +18,7 @@ it writes) comes from the CUDA path.
 Run (from the repo root; wall time and peak memory end up in the .txt header):
     python tests/golden/make_solve_golden.py C4 --seed 0
     python tests/golden/make_solve_golden.py C5 --seed 0 --n 65535
+    python tests/golden/make_solve_golden.py C5 --seed 0 --n 1048575      # 86 min, 13.8 GB on 8 cores
 """
 import argparse
 import os
